@@ -1,0 +1,326 @@
+/*
+ * rfoe_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * Plain, slow, obviously-correct CPU FP64 implementation of the recursive Fermi-operator
+ * expansion (RFOE) hot path of arXiv 2301.04642, written from the paper.  Only tests/,
+ * __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may use it.
+ * It shares no code, header, table or helper with the CUDA library under
+ * paper_2301_04642_b200/csrc/ and neither includes the other.
+ *
+ * What it follows (PAPER.md line : section):
+ *   - X_{n+1} = X_n +/- (X_n - X_n^2), i.e. X^2 or 2X - X^2, sign chosen so that the trace
+ *     converges to N_occ                                   PAPER.md:35-39 (sec. II.B.1, Eq. 1)
+ *   - Tr(X) by diagonal traversal, Tr(X^2) = ||X||_F^2      PAPER.md:72    (sec. III.B)
+ *   - RelTr = trace change relative to the previous iterate PAPER.md:64, 92 (sec. III.A, IV)
+ *   - mixed precision: FP32 steps far from convergence,
+ *     FP64 afterwards, switch tied to RelTr
+ *   - truncated expansion G_m (T-RFOE): stop after m steps  PAPER.md:47-52 (sec. II.B.3, Eq. 2)
+ *   - accelerated (shifted/scaled) SP2 from HOMO/LUMO       PAPER.md:43    (sec. II.B.2)
+ *   - D = theta(mu I - H): a projector, eigenvalues 0/1     PAPER.md:27    (sec. II.A)
+ * Where the paper is silent the readings R1..R16 of DESIGN.md are taken (initial affine map with
+ * Gershgorin bounds, tie rule, stop rules A and B, the McWeeny-style switch).
+ *
+ * Arithmetic rules (so a reader can check it by eye): every product and sum is a separate
+ * IEEE-754 double operation (compile with -ffp-contract=off, no -ffast-math); X_n^2 is the
+ * naive triple loop with the contraction index l ascending.  rfoe_oracle_square_ijk is the literal
+ * i-j-l loop nest; rfoe_oracle_square is the same arithmetic with the loops interchanged
+ * (i-l-j, upper triangle, then mirrored) which is faster and bit-identical -- each Y_ij still adds
+ * the products X_il*X_lj one at a time in ascending l; a CPU test pins the two to each other.
+ *
+ * Pins (tests/test_oracle_pins.py, -m "not gpu"): Jacobi-eigendecomposition projector on tiny
+ * inputs; construction-exact projector Q_occ Q_occ^T; diagonal-H closed form (scalar recursion);
+ * per-step invariants; scalar eigenvalue-space model for branch strings and iteration counts;
+ * the paper's printed iteration counts on the paper's matrix.
+ * Not pinned: the exact bit patterns of X_n (the paper prints no worked example) -- "parity
+ * unpinned" for bits, covered by tolerances.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#define ORACLE_MAX_STEPS 256
+
+enum { ORC_SP2 = 0, ORC_MCWEENY = 1, ORC_SP2_MIXED = 2, ORC_SP2_ACCEL = 3 };
+enum { ORC_RULE_A = 0, ORC_RULE_B = 1 };
+
+typedef struct {
+    /* inputs */
+    int32_t variant;      /* ORC_* */
+    int32_t stop_rule;    /* ORC_RULE_A: e_n = ||X_n^2 - X_n||_F <= tol ; ORC_RULE_B: RelTr <= tol */
+    int32_t max_iter;     /* cap on recursion steps (<= ORACLE_MAX_STEPS) */
+    int32_t use_bounds;   /* 1: take emin/emax below instead of Gershgorin */
+    double tol;
+    double emin, emax;    /* in: override when use_bounds; out: the bounds used */
+    double mixed_head;    /* mixed: FP64 while (t - s) >= mixed_head  (0 => no FP64 head, paper schedule) */
+    double mixed_reltr;   /* mixed: FP32 steps until RelTr <= mixed_reltr (paper: 5e-4), then FP64 */
+    double homo, lumo;    /* accelerated SP2: eigenvalue estimates of H (lumo > homo) */
+    /* outputs */
+    int32_t iterations;   /* recursion steps taken */
+    int32_t multiplications;
+    int32_t mcweeny_steps;
+    int32_t fp32_steps;
+    int32_t converged;
+    int32_t pad_;
+    double tr_PH;         /* sum_ij P_ij H_ij */
+    double t[ORACLE_MAX_STEPS + 1];   /* t[n] = Tr X_n */
+    double s[ORACLE_MAX_STEPS + 1];   /* s[n] = sum_ij X_n,ij^2 */
+    double e[ORACLE_MAX_STEPS];       /* e[n] = ||X_n^2 - X_n||_F */
+    double reltr[ORACLE_MAX_STEPS];   /* |t[n+1]-t[n]| / |t[n]| */
+    char branch[ORACLE_MAX_STEPS + 1];/* 'S' (X^2), 'L' (2X - X^2), 'M' (McWeeny), lower case = FP32 step */
+} oracle_run_t;
+
+/* ---- O1: Gershgorin bounds (reading R3) ------------------------------------------------- */
+void rfoe_oracle_bounds(const double* H, int64_t k, double* emin, double* emax)
+{
+    double lo = 0.0, hi = 0.0;
+    for (int64_t i = 0; i < k; ++i) {
+        double r = 0.0;
+        for (int64_t j = 0; j < k; ++j)
+            if (j != i) r = r + fabs(H[i * k + j]);
+        double a = H[i * k + i] - r, b = H[i * k + i] + r;
+        if (i == 0 || a < lo) lo = a;
+        if (i == 0 || b > hi) hi = b;
+    }
+    *emin = lo;
+    *emax = hi;
+}
+
+/* ---- O2: affine initial map X0 = (emax I - H)/(emax - emin) (reading R2; true division) --- */
+void rfoe_oracle_affine(const double* H, int64_t k, double emin, double emax, double* X)
+{
+    double w = emax - emin;
+    for (int64_t i = 0; i < k; ++i)
+        for (int64_t j = 0; j < k; ++j) {
+            double num = (i == j) ? (emax - H[i * k + j]) : (-H[i * k + j]);
+            X[i * k + j] = num / w;
+        }
+}
+
+/* ---- O3: scalars.  Row sums first, then rows ascending (a fixed order) ------------------- */
+double rfoe_oracle_trace(const double* X, int64_t k)
+{
+    double t = 0.0;
+    for (int64_t i = 0; i < k; ++i) t = t + X[i * k + i];
+    return t;
+}
+
+double rfoe_oracle_sumsq(const double* X, int64_t k)
+{
+    double s = 0.0;
+    for (int64_t i = 0; i < k; ++i) {
+        double r = 0.0;
+        for (int64_t j = 0; j < k; ++j) r = r + X[i * k + j] * X[i * k + j];
+        s = s + r;
+    }
+    return s;
+}
+
+static double sumsq_diff(const double* Y, const double* X, int64_t k)
+{
+    double s = 0.0;
+    for (int64_t i = 0; i < k; ++i) {
+        double r = 0.0;
+        for (int64_t j = 0; j < k; ++j) {
+            double d = Y[i * k + j] - X[i * k + j];
+            r = r + d * d;
+        }
+        s = s + r;
+    }
+    return s;
+}
+
+/* ---- naive products ---------------------------------------------------------------------- */
+/* literal: Y_ij = sum_{l=0..k-1} A_il * B_lj, l ascending */
+void rfoe_oracle_matmul_ijk(const double* A, const double* B, int64_t k, double* Y)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < k; ++i)
+        for (int64_t j = 0; j < k; ++j) {
+            double acc = 0.0;
+            for (int64_t l = 0; l < k; ++l) acc = acc + A[i * k + l] * B[l * k + j];
+            Y[i * k + j] = acc;
+        }
+}
+
+void rfoe_oracle_square_ijk(const double* X, int64_t k, double* Y)
+{
+    rfoe_oracle_matmul_ijk(X, X, k, Y);
+}
+
+/* same arithmetic, loops interchanged (i, l, j): row Y_i accumulates X_il * (row l of B), l ascending.
+ * upper != 0: only j >= i is computed and the result mirrored (valid when the exact product is
+ * symmetric AND A, B are bitwise symmetric and A == B, see header); else the full matrix. */
+static void matmul_ilj(const double* A, const double* B, int64_t k, double* Y, int upper)
+{
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int64_t i = 0; i < k; ++i) {
+        int64_t j0 = upper ? i : 0;
+        double* y = Y + i * k;
+        for (int64_t j = j0; j < k; ++j) y[j] = 0.0;
+        for (int64_t l = 0; l < k; ++l) {
+            const double a = A[i * k + l];
+            const double* b = B + l * k;
+            for (int64_t j = j0; j < k; ++j) y[j] = y[j] + a * b[j];
+        }
+    }
+    if (upper) {
+#pragma omp parallel for schedule(static)
+        for (int64_t i = 1; i < k; ++i)
+            for (int64_t j = 0; j < i; ++j) Y[i * k + j] = Y[j * k + i];
+    }
+}
+
+void rfoe_oracle_square(const double* X, int64_t k, double* Y) { matmul_ilj(X, X, k, Y, 1); }
+void rfoe_oracle_matmul(const double* A, const double* B, int64_t k, double* Y) { matmul_ilj(A, B, k, Y, 0); }
+
+/* FP32 step of the mixed variant: X rounded to float, float products, float accumulation */
+static void square_f32(const double* X, int64_t k, double* Y, float* xf, float* yf)
+{
+    for (int64_t i = 0; i < k * k; ++i) xf[i] = (float)X[i];
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int64_t i = 0; i < k; ++i) {
+        float* y = yf + i * k;
+        for (int64_t j = i; j < k; ++j) y[j] = 0.0f;
+        for (int64_t l = 0; l < k; ++l) {
+            const float a = xf[i * k + l];
+            const float* b = xf + l * k;
+            for (int64_t j = i; j < k; ++j) y[j] = y[j] + a * b[j];
+        }
+    }
+    for (int64_t i = 0; i < k; ++i)
+        for (int64_t j = i; j < k; ++j) {
+            Y[i * k + j] = (double)yf[i * k + j];
+            Y[j * k + i] = (double)yf[i * k + j];
+        }
+}
+
+int rfoe_oracle_is_symmetric(const double* X, int64_t k)
+{
+    for (int64_t i = 0; i < k; ++i)
+        for (int64_t j = i + 1; j < k; ++j)
+            if (memcmp(&X[i * k + j], &X[j * k + i], sizeof(double)) != 0) return 0;
+    return 1;
+}
+
+/* ---- O4/O5: the expansion ---------------------------------------------------------------- */
+/* returns 0 on success (converged or max_iter reached; see run->converged), <0 on bad arguments */
+int rfoe_oracle_expand(const double* H, int64_t k, int64_t nocc, oracle_run_t* run, double* P)
+{
+    if (!H || !P || !run || k < 1 || nocc < 0 || nocc > k) return -1;
+    if (run->max_iter < 0 || run->max_iter > ORACLE_MAX_STEPS) return -1;
+    if (!rfoe_oracle_is_symmetric(H, k)) return -2;
+
+    double emin, emax;
+    if (run->use_bounds) { emin = run->emin; emax = run->emax; }
+    else rfoe_oracle_bounds(H, k, &emin, &emax);
+    run->emin = emin; run->emax = emax;
+    if (!(emax > emin)) return -3;
+
+    const size_t n2 = (size_t)k * (size_t)k;
+    double* X = (double*)malloc(n2 * sizeof(double));
+    double* Y = (double*)malloc(n2 * sizeof(double));
+    double* Z = (run->variant == ORC_MCWEENY) ? (double*)malloc(n2 * sizeof(double)) : NULL;
+    float *xf = NULL, *yf = NULL;
+    if (run->variant == ORC_SP2_MIXED) { xf = (float*)malloc(n2 * sizeof(float)); yf = (float*)malloc(n2 * sizeof(float)); }
+    if (!X || !Y) return -4;
+
+    rfoe_oracle_affine(H, k, emin, emax, X);
+    double t = rfoe_oracle_trace(X, k), s = rfoe_oracle_sumsq(X, k);
+    run->t[0] = t; run->s[0] = s;
+    run->iterations = run->multiplications = run->mcweeny_steps = run->fp32_steps = 0;
+    run->converged = 0;
+    memset(run->branch, 0, sizeof(run->branch));
+
+    /* accelerated SP2 (reading R-ACC): images of LUMO (beta, near 0) and HOMO (bbar,
+     * near 1) under the same maps steer a shift-and-scale of each SP2 polynomial. */
+    double beta = 0.0, bbar = 1.0;
+    if (run->variant == ORC_SP2_ACCEL) {
+        beta = (emax - run->lumo) / (emax - emin);
+        bbar = (emax - run->homo) / (emax - emin);
+    }
+    int mcweeny_phase = 0;
+    int mixed_phase = (run->variant == ORC_SP2_MIXED) ? (run->mixed_head > 0.0 ? 0 : 1) : 2;  /* 0 FP64 head, 1 FP32, 2 FP64 */
+    double reltr_prev = INFINITY;
+
+    for (int n = 0; n < run->max_iter; ++n) {
+        const int sq = (t > (double)nocc);           /* S iff Tr X_n > N_occ; tie -> L (R4, R5) */
+        if (mixed_phase == 0 && (t - s) < run->mixed_head) mixed_phase = 1;
+        if (mixed_phase == 1 && reltr_prev <= run->mixed_reltr) mixed_phase = 2;
+        const int fp32 = (mixed_phase == 1);
+        if (run->variant == ORC_MCWEENY && !mcweeny_phase)
+            if ((t - s) < 3.0 / 16.0 && fabs(t - (double)nocc) < 0.5) mcweeny_phase = 1;   /* R11 */
+
+        if (fp32) square_f32(X, k, Y, xf, yf); else rfoe_oracle_square(X, k, Y);
+        run->multiplications++;
+        double e = sqrt(sumsq_diff(Y, X, k));
+
+        if (mcweeny_phase) {
+            /* X' = 3 X^2 - 2 X^3, X^3 = (X^2) X as a second naive product */
+            rfoe_oracle_matmul(Y, X, k, Z);
+            run->multiplications++;
+            for (int64_t i = 0; i < k; ++i)
+                for (int64_t j = i; j < k; ++j) {
+                    /* X^2 and X commute and are symmetric, but (X^2 X)_ij and (X^2 X)_ji need not round
+                     * alike: keep the upper triangle and mirror it so that X stays bitwise symmetric */
+                    double v = 3.0 * Y[i * k + j] - 2.0 * Z[i * k + j];
+                    X[i * k + j] = v; X[j * k + i] = v;
+                }
+            run->branch[n] = 'M';
+            run->mcweeny_steps++;
+        } else if (run->variant == ORC_SP2_ACCEL) {
+            /* S-type: X' = ((1-a) I + a X)^2 = a^2 X^2 + 2a(1-a) X + (1-a)^2 I,  a = 2/(2-beta)
+             * L-type: X' = 2 a X - a^2 X^2,                                      a = 2/(1+bbar) */
+            if (sq) {
+                const double a = 2.0 / (2.0 - beta);
+                const double c2 = a * a, c1 = 2.0 * a * (1.0 - a), c0 = (1.0 - a) * (1.0 - a);
+                for (int64_t i = 0; i < k; ++i)
+                    for (int64_t j = 0; j < k; ++j) {
+                        double v = c2 * Y[i * k + j] + c1 * X[i * k + j];
+                        X[i * k + j] = (i == j) ? v + c0 : v;
+                    }
+                double u = (1.0 - a) + a * beta; beta = u * u;
+                u = (1.0 - a) + a * bbar; bbar = u * u;
+            } else {
+                const double a = 2.0 / (1.0 + bbar);
+                const double c2 = -(a * a), c1 = 2.0 * a;
+                for (size_t q = 0; q < n2; ++q) X[q] = c2 * Y[q] + c1 * X[q];
+                beta = 2.0 * a * beta - a * a * beta * beta;
+                bbar = 2.0 * a * bbar - a * a * bbar * bbar;
+            }
+            run->branch[n] = sq ? 'S' : 'L';
+        } else if (sq) {
+            memcpy(X, Y, n2 * sizeof(double));
+            run->branch[n] = fp32 ? 's' : 'S';
+        } else {
+            for (size_t q = 0; q < n2; ++q) X[q] = 2.0 * X[q] - Y[q];
+            run->branch[n] = fp32 ? 'l' : 'L';
+        }
+        if (fp32) run->fp32_steps++;
+
+        double t1 = rfoe_oracle_trace(X, k), s1 = rfoe_oracle_sumsq(X, k);
+        double reltr = fabs(t1 - t) / fabs(t);
+        run->e[n] = e; run->reltr[n] = reltr;
+        run->t[n + 1] = t1; run->s[n + 1] = s1;
+        t = t1; s = s1; reltr_prev = reltr;
+        run->iterations = n + 1;
+        /* mixed: an FP32 step never terminates the expansion (its e, RelTr sit on the FP32 floor) */
+        if (!fp32) {
+            if (run->stop_rule == ORC_RULE_A ? (e <= run->tol) : (reltr <= run->tol)) { run->converged = 1; break; }
+        }
+    }
+
+    memcpy(P, X, n2 * sizeof(double));
+    double acc = 0.0;
+    for (int64_t i = 0; i < k; ++i) {
+        double r = 0.0;
+        for (int64_t j = 0; j < k; ++j) r = r + P[i * k + j] * H[i * k + j];
+        acc = acc + r;
+    }
+    run->tr_PH = acc;
+    free(X); free(Y); free(Z); free(xf); free(yf);
+    return 0;
+}
+
+int rfoe_oracle_sizeof_run(void) { return (int)sizeof(oracle_run_t); }
+int rfoe_oracle_max_steps(void) { return ORACLE_MAX_STEPS; }
