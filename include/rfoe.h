@@ -1,0 +1,147 @@
+/*
+ * rfoe.h -- C ABI of librfoe: recursive Fermi-operator expansion (RFOE) on one B200 (sm_100a).
+ *
+ * Problem statement (arXiv 2301.04642; sec. II.A, sec. III.A): given the dense
+ * symmetric FP64 projected Kohn-Sham Hamiltonian H^p (k x k) and the number of occupied states
+ * N_occ, produce the density matrix D = theta(mu I - H^p), i.e. the projector P onto the N_occ lowest
+ * eigenvectors, WITHOUT diagonalising: a trace-steered recursion of dense matrix squarings
+ * X_{n+1} = X_n^2 or 2 X_n - X_n^2 (SP2, Eq. 1) and the variants listed below.
+ *
+ * Conventions for every entry point
+ *   - Matrices are contiguous row-major k x k FP64 with leading dimension k.  "device" pointers are
+ *     CUDA device pointers owned by the caller (e.g. torch data_ptr()); "host" pointers are ordinary
+ *     host memory.  The library never frees or keeps caller pointers after a call returns.
+ *   - `stream` is a cudaStream_t (0 = the legacy default stream).  All device work of a call is
+ *     issued on it.  Calls block the host until their result is complete (rfoe_expand reads one
+ *     scalar per recursion step from the device).
+ *   - Every function returns an rfoe_status_t.  There are no exceptions, no output on stdout/stderr
+ *     and no CPU fallback: without a usable CUDA device rfoe_create fails with RFOE_ERR_CUDA.
+ *   - A handle may be used by one host thread at a time.
+ */
+#ifndef RFOE_H_
+#define RFOE_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct rfoe_handle_s* rfoe_handle_t;
+typedef struct CUstream_st* rfoe_stream_t; /* == cudaStream_t */
+
+typedef enum {
+    RFOE_OK = 0,
+    RFOE_ERR_INVALID_ARG = 1,   /* null pointer, k < 1 or k > k_max, nocc outside (0,k), tol not finite/negative */
+    RFOE_ERR_ALLOC = 2,         /* device or pinned allocation failed */
+    RFOE_ERR_CUDA = 3,          /* a CUDA call failed; the cudaError_t is in rfoe_stats_t.cuda_error */
+    RFOE_ERR_BAD_BOUNDS = 4,    /* eps_max <= eps_min (e.g. H^p is a multiple of the identity) or not finite */
+    RFOE_ERR_NOT_SYMMETRIC = 5, /* H^p is not bitwise symmetric (the squaring X X^T relies on it) */
+    RFOE_ERR_UNSUPPORTED = 6,   /* unknown variant / option, or device is not compute capability 10.x */
+    RFOE_ERR_NOT_CONVERGED = 7  /* max_iter steps taken; P holds the last iterate, stats are complete */
+} rfoe_status_t;
+
+/* Recursion variants.
+ *  SP2        Z-RFOE with second-order projection polynomials           PAPER.md:35-39 (sec. II.B.1)
+ *  MCWEENY    SP2 until (Tr X - Tr X^2) < 3/16 and |Tr X - N_occ| < 1/2, then X <- 3X^2 - 2X^3
+ *             (purification, cited only: PAPER.md:23; reading R11 in DESIGN.md)
+ *  SP2_MIXED  FP32 squarings far from convergence, FP64 afterwards, switch tied to RelTr
+ *                                                                       PAPER.md:66, 92
+ *  SP2_ACCEL  A-Z-RFOE: shifted-and-scaled SP2 polynomials from HOMO/LUMO estimates
+ *                                                                       PAPER.md:43 (sec. II.B.2)
+ * T-RFOE (Eq. 2) is SP2 with RFOE_OPT_MAX_ITER = m and tol = 0: the truncated
+ * expansion G_m(H^p) is returned with status RFOE_ERR_NOT_CONVERGED. */
+enum { RFOE_VARIANT_SP2 = 0, RFOE_VARIANT_MCWEENY = 1, RFOE_VARIANT_SP2_MIXED = 2, RFOE_VARIANT_SP2_ACCEL = 3 };
+
+/* Options (rfoe_set_option).  Values are doubles; integer options are rounded. */
+enum {
+    RFOE_OPT_STOP_RULE = 0,    /* 0 (default) rule A: stop after the step whose e_n = ||X_n^2 - X_n||_F <= tol;
+                                  1 rule B (paper): RelTr_n = |Tr X_{n+1} - Tr X_n| / |Tr X_n| <= tol */
+    RFOE_OPT_MAX_ITER = 1,     /* cap on recursion steps, 1..RFOE_MAX_STEPS (default 100) */
+    RFOE_OPT_EPS_MIN = 2,      /* caller-supplied spectral bounds; used instead of Gershgorin when   */
+    RFOE_OPT_EPS_MAX = 3,      /*   both are set and eps_max > eps_min.  NaN (default) = unset          */
+    RFOE_OPT_CHECK_SYMMETRY = 4, /* 1 (default): one pass over H^p comparing (i,j) with (j,i) bitwise */
+    RFOE_OPT_MIXED_HEAD = 5,   /* SP2_MIXED: FP64 while (Tr X - Tr X^2) >= value; 0 (default) = paper schedule */
+    RFOE_OPT_MIXED_RELTR = 6,  /* SP2_MIXED: FP32 steps until RelTr <= value (default 5e-4) */
+    RFOE_OPT_HOMO = 7,         /* SP2_ACCEL: estimate of the highest occupied eigenvalue of H^p */
+    RFOE_OPT_LUMO = 8          /* SP2_ACCEL: estimate of the lowest unoccupied eigenvalue of H^p */
+};
+
+#define RFOE_MAX_STEPS 256
+
+typedef struct {
+    int32_t status;          /* rfoe_status_t of the last rfoe_expand / rfoe_bounds */
+    int32_t cuda_error;      /* last cudaError_t seen (0 = cudaSuccess) */
+    int32_t variant;
+    int32_t stop_rule;
+    int32_t iterations;      /* recursion steps taken (= squarings of X_n) */
+    int32_t multiplications; /* dense products launched (McWeeny steps take two) */
+    int32_t mcweeny_steps;
+    int32_t fp32_steps;
+    int32_t converged;
+    int32_t square_launches; /* launches of the symmetric squaring / product kernel */
+    int64_t k;
+    int64_t nocc;
+    int64_t gpu_launches;    /* kernels launched by the last call */
+    double tol;
+    double eps_min, eps_max; /* the bounds used for X_0 */
+    double tr_PH;            /* sum_ij P_ij H^p_ij (band energy) */
+    double device_ms;        /* CUDA-event time of the last rfoe_expand on its stream */
+    double square_ms;        /* CUDA-event time summed over its squaring / product kernel launches */
+    double t[RFOE_MAX_STEPS + 1];   /* t[n] = Tr X_n */
+    double s[RFOE_MAX_STEPS + 1];   /* s[n] = ||X_n||_F^2 = Tr X_n^2 */
+    double e[RFOE_MAX_STEPS];       /* e[n] = ||X_n^2 - X_n||_F (idempotency error of the step's input) */
+    double reltr[RFOE_MAX_STEPS];   /* |t[n+1] - t[n]| / |t[n]| */
+    char branch[RFOE_MAX_STEPS + 8];/* per step: 'S' X^2, 'L' 2X - X^2, 'M' McWeeny; lower case = FP32 step */
+} rfoe_stats_t;
+
+/* Create a handle on CUDA device `device` able to expand matrices up to k_max x k_max.
+ * Allocates (device) three zero-padded work matrices of ceil(k_max/128)*128 squared doubles (the third
+ * lazily, on the first McWeeny or mixed call), per-tile reduction scratch and one pinned host page.
+ * Errors: INVALID_ARG (h null, k_max < 1), CUDA (no device / wrong device), UNSUPPORTED (not sm_100),
+ * ALLOC. */
+int rfoe_create(rfoe_handle_t* h, int device, int64_t k_max);
+
+/* Gershgorin spectral bounds of H^p (reading R3; the paper only says "spectral bound estimates",
+ * PAPER.md:56): eps_min = min_i (H_ii - r_i), eps_max = max_i (H_ii + r_i), r_i = sum_{j != i} |H_ij|.
+ * Hp: device, k x k, read only.  eps_min / eps_max: HOST doubles, written on success.  Pure query. */
+int rfoe_bounds(rfoe_handle_t h, const double* Hp, int64_t k, double* eps_min, double* eps_max, rfoe_stream_t stream);
+
+/* The expansion.  Hp: device, k x k, bitwise symmetric, never written.  P: device, k x k, overwritten
+ * with the final iterate (bitwise symmetric); must not overlap Hp.  0 < nocc < k.  tol: threshold of
+ * the active stop rule (finite, >= 0).  Steps: Gershgorin bounds (or the override) -> X_0 =
+ * (eps_max I - H^p)/(eps_max - eps_min) -> recursion steered by Tr X_n vs N_occ (S iff Tr X_n > N_occ,
+ * PAPER.md:39) -> P, tr(P H^p).  Returns OK, NOT_CONVERGED (P and stats still valid) or an error
+ * (P unspecified). */
+int rfoe_expand(rfoe_handle_t h, const double* Hp, int64_t k, int64_t nocc, int variant, double tol, double* P,
+                rfoe_stream_t stream);
+
+/* Same as rfoe_expand with HOST buffers: copies Hp host->device, expands, copies P device->host
+ * (staging buffers owned by the handle, sized for k_max).  Hp_host / P_host may be pageable or pinned. */
+int rfoe_expand_host(rfoe_handle_t h, const double* Hp_host, int64_t k, int64_t nocc, int variant, double tol,
+                     double* P_host, rfoe_stream_t stream);
+
+/* One recursion step exposed on its own (kernel-level tests and roofline timing):
+ * Xout = c2 * (X X) + c1 * X + c0 * I for a bitwise-symmetric device matrix X (k x k), computed by the
+ * symmetric squaring kernel (upper-triangle tiles + mirror).  X and Xout must not overlap.
+ * scalars (HOST, 5 doubles): Tr Xout, ||Xout||_F^2, ||X X - X||_F^2, Tr(X X), sum_ij (X X)_ij X_ij.
+ * kernel_ms (HOST, may be null): CUDA-event time of the squaring kernel alone (padding copies excluded). */
+int rfoe_square(rfoe_handle_t h, const double* X, int64_t k, double c2, double c1, double c0, double* Xout,
+                double* scalars, float* kernel_ms, rfoe_stream_t stream);
+
+/* Symmetric product for commuting symmetric A, B (k x k, device): Cout = c2 * (A B) + c1 * A + c0 * I, upper
+ * triangle computed and mirrored (the McWeeny step uses it with A = X^2, B = X).  scalars as in rfoe_square
+ * with X replaced by A in the last three. */
+int rfoe_symm_product(rfoe_handle_t h, const double* A, const double* B, int64_t k, double c2, double c1, double c0,
+                      double* Cout, double* scalars, float* kernel_ms, rfoe_stream_t stream);
+
+int rfoe_set_option(rfoe_handle_t h, int key, double value); /* INVALID_ARG on bad value, UNSUPPORTED on bad key */
+int rfoe_get_stats(rfoe_handle_t h, rfoe_stats_t* out);      /* copies the stats of the last call */
+int rfoe_destroy(rfoe_handle_t h);                           /* frees everything the handle owns; h may be null */
+const char* rfoe_strerror(int status);                       /* static string, never null */
+int rfoe_version(void);                                      /* ABI version (major*100 + minor) */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RFOE_H_ */

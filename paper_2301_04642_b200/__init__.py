@@ -1,0 +1,259 @@
+"""paper_2301_04642_b200 -- B200-native recursive Fermi-operator expansion (RFOE, arXiv 2301.04642).
+
+Thin Python binding over the C-ABI library ``librfoe.so`` (``include/rfoe.h``): argument marshalling
+only -- every step of the path (Gershgorin bounds, affine map, symmetric squarings on the FP64 tensor
+cores with the fused update / mirror / reductions, device-side branch decisions, output pass) runs in
+the CUDA kernels under ``csrc/``.  PyTorch is used for device memory and streams, nothing else.
+There is no CPU fallback: importing works anywhere, but any call without the built library or without
+an sm_100 GPU raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+
+import numpy as np
+
+from . import build as _build
+
+__all__ = ["Rfoe", "RfoeError", "ExpandResult", "load_library", "SP2", "MCWEENY", "SP2_MIXED", "SP2_ACCEL",
+           "RULE_A", "RULE_B", "EXPORTS"]
+
+SP2, MCWEENY, SP2_MIXED, SP2_ACCEL = 0, 1, 2, 3
+RULE_A, RULE_B = 0, 1
+MAX_STEPS = 256
+
+(OPT_STOP_RULE, OPT_MAX_ITER, OPT_EPS_MIN, OPT_EPS_MAX, OPT_CHECK_SYMMETRY, OPT_MIXED_HEAD, OPT_MIXED_RELTR,
+ OPT_HOMO, OPT_LUMO) = range(9)
+
+OK, ERR_INVALID_ARG, ERR_ALLOC, ERR_CUDA, ERR_BAD_BOUNDS, ERR_NOT_SYMMETRIC, ERR_UNSUPPORTED, ERR_NOT_CONVERGED = range(8)
+
+# every symbol include/rfoe.h declares
+EXPORTS = ("rfoe_create", "rfoe_bounds", "rfoe_expand", "rfoe_expand_host", "rfoe_square", "rfoe_symm_product",
+           "rfoe_set_option", "rfoe_get_stats", "rfoe_destroy", "rfoe_strerror", "rfoe_version")
+
+
+class RfoeError(RuntimeError):
+    def __init__(self, status: int, msg: str, cuda_error: int = 0):
+        super().__init__(f"librfoe: {msg} (status {status}" + (f", cudaError {cuda_error})" if cuda_error else ")"))
+        self.status = status
+        self.cuda_error = cuda_error
+
+
+class _Stats(C.Structure):
+    _fields_ = [
+        ("status", C.c_int32), ("cuda_error", C.c_int32), ("variant", C.c_int32), ("stop_rule", C.c_int32),
+        ("iterations", C.c_int32), ("multiplications", C.c_int32), ("mcweeny_steps", C.c_int32),
+        ("fp32_steps", C.c_int32), ("converged", C.c_int32), ("square_launches", C.c_int32),
+        ("k", C.c_int64), ("nocc", C.c_int64), ("gpu_launches", C.c_int64),
+        ("tol", C.c_double), ("eps_min", C.c_double), ("eps_max", C.c_double), ("tr_PH", C.c_double),
+        ("device_ms", C.c_double), ("square_ms", C.c_double),
+        ("t", C.c_double * (MAX_STEPS + 1)), ("s", C.c_double * (MAX_STEPS + 1)),
+        ("e", C.c_double * MAX_STEPS), ("reltr", C.c_double * MAX_STEPS),
+        ("branch", C.c_char * (MAX_STEPS + 8)),
+    ]
+
+
+_lib = None
+
+
+def load_library(path: str | None = None):
+    """dlopen librfoe.so (building it first if the sources are newer) and declare the prototypes."""
+    global _lib
+    if _lib is not None and path is None:
+        return _lib
+    p = path or _build.LIB
+    if path is None and _build.stale():
+        _build.build()
+    if not os.path.exists(p):
+        raise RfoeError(ERR_UNSUPPORTED, f"{p} is missing: run `python -m paper_2301_04642_b200.build`")
+    L = C.CDLL(p)
+    vp, i64, dbl, dp = C.c_void_p, C.c_int64, C.c_double, C.POINTER(C.c_double)
+    L.rfoe_create.argtypes = [C.POINTER(vp), C.c_int, i64]
+    L.rfoe_bounds.argtypes = [vp, vp, i64, dp, dp, vp]
+    L.rfoe_expand.argtypes = [vp, vp, i64, i64, C.c_int, dbl, vp, vp]
+    L.rfoe_expand_host.argtypes = [vp, vp, i64, i64, C.c_int, dbl, vp, vp]
+    L.rfoe_square.argtypes = [vp, vp, i64, dbl, dbl, dbl, vp, dp, C.POINTER(C.c_float), vp]
+    L.rfoe_symm_product.argtypes = [vp, vp, vp, i64, dbl, dbl, dbl, vp, dp, C.POINTER(C.c_float), vp]
+    L.rfoe_set_option.argtypes = [vp, C.c_int, dbl]
+    L.rfoe_get_stats.argtypes = [vp, C.POINTER(_Stats)]
+    L.rfoe_destroy.argtypes = [vp]
+    L.rfoe_strerror.argtypes = [C.c_int]
+    L.rfoe_strerror.restype = C.c_char_p
+    L.rfoe_version.argtypes = []
+    for name in EXPORTS:
+        if name != "rfoe_strerror":
+            getattr(L, name).restype = C.c_int
+    if path is None:
+        _lib = L
+    return L
+
+
+@dataclass
+class ExpandResult:
+    P: object              # torch tensor (device) or numpy array (host entry point)
+    status: int
+    converged: bool
+    iterations: int
+    multiplications: int
+    mcweeny_steps: int
+    fp32_steps: int
+    branch: str
+    eps_min: float
+    eps_max: float
+    tr_PH: float
+    device_ms: float
+    square_ms: float
+    square_launches: int
+    gpu_launches: int
+    t: np.ndarray
+    s: np.ndarray
+    e: np.ndarray
+    reltr: np.ndarray
+
+
+def _stream_ptr(stream):
+    import torch
+
+    s = torch.cuda.current_stream() if stream is None else stream
+    return C.c_void_p(s.cuda_stream)
+
+
+def _check_dev(x, name):
+    import torch
+
+    if not (isinstance(x, torch.Tensor) and x.is_cuda and x.dtype == torch.float64 and x.dim() == 2
+            and x.shape[0] == x.shape[1] and x.is_contiguous()):
+        raise ValueError(f"{name}: contiguous square float64 CUDA tensor expected")
+
+
+class Rfoe:
+    """One librfoe handle (same names as the C ABI: bounds / expand / expand_host / square / symm_product)."""
+
+    def __init__(self, k_max: int, device: int = 0):
+        self._L = load_library()
+        self._h = C.c_void_p()
+        self.k_max = int(k_max)
+        self.device = int(device)
+        rc = self._L.rfoe_create(C.byref(self._h), self.device, self.k_max)
+        if rc != OK:
+            self._h = C.c_void_p()
+            raise RfoeError(rc, self._L.rfoe_strerror(rc).decode())
+
+    def close(self):
+        if getattr(self, "_h", None) and self._h.value:
+            self._L.rfoe_destroy(self._h)
+            self._h = C.c_void_p()
+
+    __del__ = close
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+    # ---- helpers
+    def _raise(self, rc):
+        st = self.stats_raw()
+        raise RfoeError(rc, self._L.rfoe_strerror(rc).decode(), st.cuda_error)
+
+    def stats_raw(self) -> _Stats:
+        st = _Stats()
+        self._L.rfoe_get_stats(self._h, C.byref(st))
+        return st
+
+    def set_option(self, key: int, value: float):
+        rc = self._L.rfoe_set_option(self._h, key, float(value))
+        if rc != OK:
+            raise RfoeError(rc, self._L.rfoe_strerror(rc).decode())
+
+    def configure(self, *, stop_rule=None, max_iter=None, bounds=None, check_symmetry=None, mixed_head=None,
+                  mixed_reltr=None, homo=None, lumo=None):
+        if stop_rule is not None: self.set_option(OPT_STOP_RULE, stop_rule)
+        if max_iter is not None: self.set_option(OPT_MAX_ITER, max_iter)
+        if bounds is not None:
+            lo, hi = (float("nan"), float("nan")) if bounds is False else bounds
+            self.set_option(OPT_EPS_MIN, lo)
+            self.set_option(OPT_EPS_MAX, hi)
+        if check_symmetry is not None: self.set_option(OPT_CHECK_SYMMETRY, 1.0 if check_symmetry else 0.0)
+        if mixed_head is not None: self.set_option(OPT_MIXED_HEAD, mixed_head)
+        if mixed_reltr is not None: self.set_option(OPT_MIXED_RELTR, mixed_reltr)
+        if homo is not None: self.set_option(OPT_HOMO, homo)
+        if lumo is not None: self.set_option(OPT_LUMO, lumo)
+        return self
+
+    def _result(self, P, rc) -> ExpandResult:
+        st = self.stats_raw()
+        n = st.iterations
+        return ExpandResult(
+            P=P, status=rc, converged=bool(st.converged), iterations=n, multiplications=st.multiplications,
+            mcweeny_steps=st.mcweeny_steps, fp32_steps=st.fp32_steps, branch=st.branch.decode()[:n],
+            eps_min=st.eps_min, eps_max=st.eps_max, tr_PH=st.tr_PH, device_ms=st.device_ms, square_ms=st.square_ms, square_launches=st.square_launches,
+            gpu_launches=st.gpu_launches, t=np.array(st.t[: n + 1]), s=np.array(st.s[: n + 1]),
+            e=np.array(st.e[:n]), reltr=np.array(st.reltr[:n]))
+
+    # ---- the C-ABI calls
+    def bounds(self, Hp, stream=None):
+        _check_dev(Hp, "Hp")
+        lo, hi = C.c_double(), C.c_double()
+        rc = self._L.rfoe_bounds(self._h, C.c_void_p(Hp.data_ptr()), Hp.shape[0], C.byref(lo), C.byref(hi), _stream_ptr(stream))
+        if rc != OK:
+            self._raise(rc)
+        return lo.value, hi.value
+
+    def expand(self, Hp, nocc: int, variant: int = SP2, tol: float = 1e-12, P=None, stream=None) -> ExpandResult:
+        import torch
+
+        _check_dev(Hp, "Hp")
+        if P is None:
+            P = torch.empty_like(Hp)
+        _check_dev(P, "P")
+        rc = self._L.rfoe_expand(self._h, C.c_void_p(Hp.data_ptr()), Hp.shape[0], int(nocc), int(variant), float(tol),
+                                 C.c_void_p(P.data_ptr()), _stream_ptr(stream))
+        if rc not in (OK, ERR_NOT_CONVERGED):
+            self._raise(rc)
+        return self._result(P, rc)
+
+    def expand_host(self, Hp: np.ndarray, nocc: int, variant: int = SP2, tol: float = 1e-12, P=None, stream=None) -> ExpandResult:
+        """Host buffers in, host buffers out (numpy arrays or pinned CPU torch tensors)."""
+        def ptr(a):
+            return a.ctypes.data if isinstance(a, np.ndarray) else a.data_ptr()
+        k = Hp.shape[0]
+        if P is None:
+            P = np.empty((k, k), dtype=np.float64)
+        rc = self._L.rfoe_expand_host(self._h, C.c_void_p(ptr(Hp)), k, int(nocc), int(variant), float(tol),
+                                      C.c_void_p(ptr(P)), _stream_ptr(stream))
+        if rc not in (OK, ERR_NOT_CONVERGED):
+            self._raise(rc)
+        return self._result(P, rc)
+
+    def square(self, X, c2=1.0, c1=0.0, c0=0.0, out=None, stream=None):
+        """out = c2 X X + c1 X + c0 I; returns (out, scalars[5], kernel_ms)."""
+        import torch
+
+        _check_dev(X, "X")
+        out = torch.empty_like(X) if out is None else out
+        sc = (C.c_double * 5)()
+        ms = C.c_float()
+        rc = self._L.rfoe_square(self._h, C.c_void_p(X.data_ptr()), X.shape[0], c2, c1, c0, C.c_void_p(out.data_ptr()),
+                                 sc, C.byref(ms), _stream_ptr(stream))
+        if rc != OK:
+            self._raise(rc)
+        return out, np.array(sc[:]), ms.value
+
+    def symm_product(self, A, B, c2=1.0, c1=0.0, c0=0.0, out=None, stream=None):
+        """out = c2 A B + c1 A + c0 I (upper triangle mirrored); returns (out, scalars[5], kernel_ms)."""
+        import torch
+
+        _check_dev(A, "A")
+        _check_dev(B, "B")
+        out = torch.empty_like(A) if out is None else out
+        sc = (C.c_double * 5)()
+        ms = C.c_float()
+        rc = self._L.rfoe_symm_product(self._h, C.c_void_p(A.data_ptr()), C.c_void_p(B.data_ptr()), A.shape[0], c2, c1, c0,
+                                       C.c_void_p(out.data_ptr()), sc, C.byref(ms), _stream_ptr(stream))
+        if rc != OK:
+            self._raise(rc)
+        return out, np.array(sc[:]), ms.value

@@ -1,0 +1,527 @@
+// librfoe -- C ABI (include/rfoe.h) over the sm_100a kernels.  Host logic only: argument checks,
+// workspace management, TMA descriptors, the launch sequence of one expansion and the one-word-per-step
+// read from mapped pinned memory.  Every arithmetic step of the path runs in the kernels.
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+#include <string.h>
+
+#include <new>
+#include <vector>
+
+#include "../../include/rfoe.h"
+#include "control.cuh"
+#include "hbm_kernels.cuh"
+#include "sym_square.cuh"
+
+using namespace rfoe;
+
+static_assert(RFOE_MAX_STEPS == CTRL_MAX_STEPS, "header / control history size mismatch");
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+struct HostPage {          // mapped pinned memory
+    volatile int word;     // next action, written by control_kernel
+    int sym_flag;
+    double bounds[2];
+    double scalars[8];
+    Ctrl ctrl;             // staging copy of the device control block
+};
+
+struct rfoe_handle_s {
+    int device = 0;
+    int sm_count = 148;
+    int64_t k_max = 0;
+    int ld_max = 0;
+    double* W[3] = {nullptr, nullptr, nullptr};
+    double* part[2] = {nullptr, nullptr};
+    double* rows[2] = {nullptr, nullptr};
+    double* d_bounds = nullptr;
+    double* d_scalars = nullptr;
+    int* d_flag = nullptr;
+    Ctrl* d_ctrl = nullptr;
+    int2* d_tiles = nullptr;
+    int tiles_m = 0;       // tile-grid size the tile map was built for
+    int n_tiles = 0;
+    HostPage* hp = nullptr;
+    int* d_word = nullptr; // device alias of hp->word
+    double* stage_H = nullptr;
+    double* stage_P = nullptr;
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    cudaEvent_t sq_ev[4 * RFOE_MAX_STEPS] = {};   // begin/end pairs around every squaring launch of an expansion
+    int sq_n = 0;
+    EncodeTiledFn encode = nullptr;
+    // options
+    int stop_rule = 0, max_iter = 100, check_sym = 1;
+    double eps_min = NAN, eps_max = NAN, mixed_head = 0.0, mixed_reltr = 5e-4, homo = NAN, lumo = NAN;
+    rfoe_stats_t stats;
+    int64_t launches = 0;
+};
+
+#define CK(call)                                                     \
+    do {                                                             \
+        cudaError_t e_ = (call);                                     \
+        if (e_ != cudaSuccess) {                                     \
+            h->stats.cuda_error = (int)e_;                           \
+            h->stats.status = RFOE_ERR_CUDA;                         \
+            return RFOE_ERR_CUDA;                                    \
+        }                                                            \
+    } while (0)
+
+static int round_up(int64_t v, int m) { return (int)((v + m - 1) / m * m); }
+
+static int hbm_grid(const rfoe_handle_s* h, int rows)
+{
+    int want = (rows + HBM_WARPS - 1) / HBM_WARPS;
+    int cap = h->sm_count * 8;
+    return want < cap ? (want < 1 ? 1 : want) : cap;
+}
+
+// Upper-triangle tile order: G x G super-blocks walked row-major, so that the ~148 CTAs resident at
+// any time share about 2G row panels and stream them through L2 together.
+static void build_tile_order(int m, std::vector<int2>& out)
+{
+    const int G = 12;
+    out.clear();
+    out.reserve((size_t)m * (m + 1) / 2);
+    for (int SI = 0; SI < m; SI += G)
+        for (int SJ = SI; SJ < m; SJ += G)
+            for (int i = SI; i < SI + G && i < m; ++i)
+                for (int j = (SJ > i ? SJ : i); j < SJ + G && j < m; ++j) out.push_back(make_int2(i, j));
+}
+
+static int ensure_tiles(rfoe_handle_s* h, int m, cudaStream_t st)
+{
+    if (h->tiles_m == m) return RFOE_OK;
+    std::vector<int2> order;
+    build_tile_order(m, order);
+    CK(cudaMemcpyAsync(h->d_tiles, order.data(), order.size() * sizeof(int2), cudaMemcpyHostToDevice, st));
+    CK(cudaStreamSynchronize(st));   // `order` is pageable and dies here
+    h->tiles_m = m;
+    h->n_tiles = (int)order.size();
+    return RFOE_OK;
+}
+
+static int make_map(rfoe_handle_s* h, CUtensorMap* map, double* base, int ld)
+{
+    cuuint64_t dims[2] = {(cuuint64_t)ld, (cuuint64_t)ld};
+    cuuint64_t strides[1] = {(cuuint64_t)ld * sizeof(double)};
+    cuuint32_t box[2] = {(cuuint32_t)SQ_BK, (cuuint32_t)SQ_BM};
+    cuuint32_t estr[2] = {1, 1};
+    CUresult r = h->encode(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, base, dims, strides, box, estr,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        h->stats.cuda_error = (int)cudaErrorInvalidValue;
+        return RFOE_ERR_CUDA;
+    }
+    return RFOE_OK;
+}
+
+template <bool TWO_OP>
+static cudaError_t launch_square(rfoe_handle_s* h, const CUtensorMap& a, const CUtensorMap& b, const double* E, double* Out,
+                                 int ld, int k, const StepCoef* coef, double* partials, cudaStream_t st)
+{
+    sym_square_kernel<TWO_OP><<<h->n_tiles, SQ_THREADS, SQ_SMEM_BYTES, st>>>(a, b, E, Out, ld, k, coef, h->d_tiles, partials);
+    h->launches++;
+    return cudaGetLastError();
+}
+
+// squaring launch bracketed by its own event pair (summed into stats.square_ms after the expansion)
+template <bool TWO_OP>
+static cudaError_t timed_square(rfoe_handle_s* h, const CUtensorMap& a, const CUtensorMap& b, const double* E, double* Out,
+                                int ld, int k, const StepCoef* coef, double* partials, cudaStream_t st)
+{
+    cudaError_t e = cudaEventRecord(h->sq_ev[2 * h->sq_n], st);
+    if (e != cudaSuccess) return e;
+    e = launch_square<TWO_OP>(h, a, b, E, Out, ld, k, coef, partials, st);
+    if (e != cudaSuccess) return e;
+    e = cudaEventRecord(h->sq_ev[2 * h->sq_n + 1], st);
+    h->sq_n++;
+    return e;
+}
+
+extern "C" const char* rfoe_strerror(int status)
+{
+    switch (status) {
+        case RFOE_OK: return "ok";
+        case RFOE_ERR_INVALID_ARG: return "invalid argument";
+        case RFOE_ERR_ALLOC: return "allocation failed";
+        case RFOE_ERR_CUDA: return "CUDA error";
+        case RFOE_ERR_BAD_BOUNDS: return "spectral bounds are empty or not finite";
+        case RFOE_ERR_NOT_SYMMETRIC: return "H^p is not bitwise symmetric";
+        case RFOE_ERR_UNSUPPORTED: return "unsupported variant, option or device";
+        case RFOE_ERR_NOT_CONVERGED: return "maximum number of recursion steps reached";
+        default: return "unknown status";
+    }
+}
+
+extern "C" int rfoe_version(void) { return 100; }
+
+extern "C" int rfoe_destroy(rfoe_handle_t h)
+{
+    if (!h) return RFOE_OK;
+    cudaSetDevice(h->device);
+    for (double* p : h->W) cudaFree(p);
+    for (double* p : h->part) cudaFree(p);
+    for (double* p : h->rows) cudaFree(p);
+    cudaFree(h->d_bounds); cudaFree(h->d_scalars); cudaFree(h->d_flag); cudaFree(h->d_ctrl); cudaFree(h->d_tiles);
+    cudaFree(h->stage_H); cudaFree(h->stage_P);
+    if (h->hp) cudaFreeHost(h->hp);
+    if (h->ev0) cudaEventDestroy(h->ev0);
+    if (h->ev1) cudaEventDestroy(h->ev1);
+    for (cudaEvent_t e : h->sq_ev) if (e) cudaEventDestroy(e);
+    delete h;
+    return RFOE_OK;
+}
+
+extern "C" int rfoe_create(rfoe_handle_t* out, int device, int64_t k_max)
+{
+    if (!out || k_max < 1 || k_max > (1 << 20)) return RFOE_ERR_INVALID_ARG;
+    *out = nullptr;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return RFOE_ERR_CUDA;
+    if (cudaSetDevice(device) != cudaSuccess) return RFOE_ERR_CUDA;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return RFOE_ERR_CUDA;
+    if (prop.major != 10) return RFOE_ERR_UNSUPPORTED;   // sm_100a cubin only; no fallback path
+    rfoe_handle_s* h = new (std::nothrow) rfoe_handle_s();
+    if (!h) return RFOE_ERR_ALLOC;
+    memset(&h->stats, 0, sizeof(h->stats));
+    h->device = device;
+    h->sm_count = prop.multiProcessorCount;
+    h->k_max = k_max;
+    h->ld_max = round_up(k_max, SQ_BM);
+    const size_t ld = (size_t)h->ld_max;
+    const size_t m = ld / SQ_BM, nt = m * (m + 1) / 2;
+    bool ok = true;
+    ok = ok && cudaMalloc(&h->W[0], ld * ld * sizeof(double)) == cudaSuccess;
+    ok = ok && cudaMalloc(&h->W[1], ld * ld * sizeof(double)) == cudaSuccess;
+    ok = ok && cudaMalloc(&h->part[0], nt * SQ_NPART * sizeof(double)) == cudaSuccess;
+    ok = ok && cudaMalloc(&h->part[1], nt * SQ_NPART * sizeof(double)) == cudaSuccess;
+    ok = ok && cudaMalloc(&h->rows[0], ld * sizeof(double)) == cudaSuccess;
+    ok = ok && cudaMalloc(&h->rows[1], ld * sizeof(double)) == cudaSuccess;
+    ok = ok && cudaMalloc(&h->d_bounds, 2 * sizeof(double)) == cudaSuccess;
+    ok = ok && cudaMalloc(&h->d_scalars, 8 * sizeof(double)) == cudaSuccess;
+    ok = ok && cudaMalloc(&h->d_flag, sizeof(int)) == cudaSuccess;
+    ok = ok && cudaMalloc(&h->d_ctrl, sizeof(Ctrl)) == cudaSuccess;
+    ok = ok && cudaMalloc(&h->d_tiles, nt * sizeof(int2)) == cudaSuccess;
+    ok = ok && cudaHostAlloc((void**)&h->hp, sizeof(HostPage), cudaHostAllocMapped) == cudaSuccess;
+    ok = ok && cudaHostGetDevicePointer((void**)&h->d_word, (void*)&h->hp->word, 0) == cudaSuccess;
+    ok = ok && cudaEventCreate(&h->ev0) == cudaSuccess && cudaEventCreate(&h->ev1) == cudaSuccess;
+    for (cudaEvent_t& e : h->sq_ev) ok = ok && cudaEventCreate(&e) == cudaSuccess;
+    if (!ok) { cudaGetLastError(); rfoe_destroy(h); return RFOE_ERR_ALLOC; }
+    cudaDriverEntryPointQueryResult qres;
+    void* fn = nullptr;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn) {
+        rfoe_destroy(h);
+        return RFOE_ERR_CUDA;
+    }
+    h->encode = (EncodeTiledFn)fn;
+    if (cudaFuncSetAttribute(sym_square_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SQ_SMEM_BYTES) != cudaSuccess ||
+        cudaFuncSetAttribute(sym_square_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SQ_SMEM_BYTES) != cudaSuccess) {
+        rfoe_destroy(h);
+        return RFOE_ERR_CUDA;
+    }
+    *out = h;
+    return RFOE_OK;
+}
+
+extern "C" int rfoe_set_option(rfoe_handle_t h, int key, double value)
+{
+    if (!h) return RFOE_ERR_INVALID_ARG;
+    switch (key) {
+        case RFOE_OPT_STOP_RULE:
+            if (value != 0.0 && value != 1.0) return RFOE_ERR_INVALID_ARG;
+            h->stop_rule = (int)value; return RFOE_OK;
+        case RFOE_OPT_MAX_ITER:
+            if (!(value >= 1.0 && value <= (double)RFOE_MAX_STEPS)) return RFOE_ERR_INVALID_ARG;
+            h->max_iter = (int)llround(value); return RFOE_OK;
+        case RFOE_OPT_EPS_MIN: h->eps_min = value; return RFOE_OK;
+        case RFOE_OPT_EPS_MAX: h->eps_max = value; return RFOE_OK;
+        case RFOE_OPT_CHECK_SYMMETRY: h->check_sym = (value != 0.0); return RFOE_OK;
+        case RFOE_OPT_MIXED_HEAD:
+            if (!(value >= 0.0)) return RFOE_ERR_INVALID_ARG;
+            h->mixed_head = value; return RFOE_OK;
+        case RFOE_OPT_MIXED_RELTR:
+            if (!(value >= 0.0)) return RFOE_ERR_INVALID_ARG;
+            h->mixed_reltr = value; return RFOE_OK;
+        case RFOE_OPT_HOMO: h->homo = value; return RFOE_OK;
+        case RFOE_OPT_LUMO: h->lumo = value; return RFOE_OK;
+        default: return RFOE_ERR_UNSUPPORTED;
+    }
+}
+
+extern "C" int rfoe_get_stats(rfoe_handle_t h, rfoe_stats_t* out)
+{
+    if (!h || !out) return RFOE_ERR_INVALID_ARG;
+    *out = h->stats;
+    return RFOE_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// A1: Gershgorin bounds into h->d_bounds (device) -- two launches
+static int run_bounds(rfoe_handle_s* h, const double* Hp, int k, cudaStream_t st)
+{
+    gershgorin_rows_kernel<<<hbm_grid(h, k), HBM_THREADS, 0, st>>>(Hp, k, h->rows[0], h->rows[1]);
+    h->launches++;
+    CK(cudaGetLastError());
+    bounds_reduce_kernel<<<1, 256, 0, st>>>(h->rows[0], h->rows[1], k, h->d_bounds);
+    h->launches++;
+    CK(cudaGetLastError());
+    return RFOE_OK;
+}
+
+static int check_common(rfoe_handle_s* h, const void* a, const void* b, int64_t k)
+{
+    if (!h) return RFOE_ERR_INVALID_ARG;
+    if (!a || !b || k < 1 || k > h->k_max) return RFOE_ERR_INVALID_ARG;
+    return RFOE_OK;
+}
+
+extern "C" int rfoe_bounds(rfoe_handle_t h, const double* Hp, int64_t k, double* eps_min, double* eps_max, rfoe_stream_t stream)
+{
+    if (!h || !Hp || !eps_min || !eps_max || k < 1 || k > h->k_max) return RFOE_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    h->launches = 0;
+    h->stats.cuda_error = 0;
+    CK(cudaSetDevice(h->device));
+    int rc = run_bounds(h, Hp, (int)k, st);
+    if (rc != RFOE_OK) return rc;
+    CK(cudaMemcpyAsync((void*)h->hp->bounds, h->d_bounds, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    *eps_min = h->hp->bounds[0];
+    *eps_max = h->hp->bounds[1];
+    h->stats.gpu_launches = h->launches;
+    h->stats.status = RFOE_OK;
+    return RFOE_OK;
+}
+
+static int ensure_third(rfoe_handle_s* h)
+{
+    if (h->W[2]) return RFOE_OK;
+    const size_t ld = (size_t)h->ld_max;
+    if (cudaMalloc(&h->W[2], ld * ld * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return RFOE_ERR_ALLOC; }
+    return RFOE_OK;
+}
+
+extern "C" int rfoe_expand(rfoe_handle_t h, const double* Hp, int64_t k64, int64_t nocc, int variant, double tol, double* P,
+                           rfoe_stream_t stream)
+{
+    int rc = check_common(h, Hp, P, k64);
+    if (rc != RFOE_OK) return rc;
+    rfoe_stats_t& S = h->stats;
+    memset(&S, 0, sizeof(S));
+    S.variant = variant; S.stop_rule = h->stop_rule; S.k = k64; S.nocc = nocc; S.tol = tol;
+    auto fail = [&](int code) { S.status = code; return code; };
+    if (!(nocc > 0 && nocc < k64) || !(tol >= 0.0) || !isfinite(tol)) return fail(RFOE_ERR_INVALID_ARG);
+    {   // overlap of Hp and P
+        const char* a = (const char*)Hp; const char* b = (const char*)P;
+        const size_t bytes = (size_t)k64 * k64 * sizeof(double);
+        if (a < b + bytes && b < a + bytes) return fail(RFOE_ERR_INVALID_ARG);
+    }
+    if (variant < RFOE_VARIANT_SP2 || variant > RFOE_VARIANT_SP2_ACCEL) return fail(RFOE_ERR_UNSUPPORTED);
+    if (variant == RFOE_VARIANT_SP2_MIXED) return fail(RFOE_ERR_UNSUPPORTED);   // FP32 path: see DESIGN.md (row A8)
+    if (variant == RFOE_VARIANT_SP2_ACCEL && !(isfinite(h->homo) && isfinite(h->lumo) && h->lumo > h->homo))
+        return fail(RFOE_ERR_INVALID_ARG);
+    const int k = (int)k64;
+    const int ld = round_up(k, SQ_BM);
+    const int m = ld / SQ_BM;
+    cudaStream_t st = (cudaStream_t)stream;
+    h->launches = 0;
+    CK(cudaSetDevice(h->device));
+    if (variant == RFOE_VARIANT_MCWEENY && (rc = ensure_third(h)) != RFOE_OK) return fail(rc);
+    if ((rc = ensure_tiles(h, m, st)) != RFOE_OK) return fail(rc);
+    CUtensorMap tm[3];
+    for (int i = 0; i < 3; ++i)
+        if (h->W[i] && (rc = make_map(h, &tm[i], h->W[i], ld)) != RFOE_OK) return fail(rc);
+
+    CK(cudaEventRecord(h->ev0, st));
+    // --- symmetry check, bounds, affine map, first decision -------------------------------------
+    h->hp->sym_flag = 0;
+    if (h->check_sym) {
+        CK(cudaMemsetAsync(h->d_flag, 0, sizeof(int), st));
+        const int nt32 = (k + 31) / 32;
+        long long blocks = (long long)nt32 * nt32;
+        if (blocks > h->sm_count * 16) blocks = h->sm_count * 16;
+        symmetry_check_kernel<<<(int)blocks, 256, 0, st>>>(Hp, k, h->d_flag);
+        h->launches++;
+        CK(cudaGetLastError());
+        CK(cudaMemcpyAsync(&h->hp->sym_flag, h->d_flag, sizeof(int), cudaMemcpyDeviceToHost, st));
+    }
+    const bool override_bounds = isfinite(h->eps_min) && isfinite(h->eps_max);
+    if (override_bounds) {
+        if (!(h->eps_max > h->eps_min)) return fail(RFOE_ERR_BAD_BOUNDS);
+        h->hp->bounds[0] = h->eps_min; h->hp->bounds[1] = h->eps_max;
+        CK(cudaMemcpyAsync(h->d_bounds, (void*)h->hp->bounds, 2 * sizeof(double), cudaMemcpyHostToDevice, st));
+    } else {
+        if ((rc = run_bounds(h, Hp, k, st)) != RFOE_OK) return fail(rc);
+        CK(cudaMemcpyAsync((void*)h->hp->bounds, h->d_bounds, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    }
+    // the check of the bounds needs them on the host before X0 is trusted: one sync (also covers sym_flag)
+    CK(cudaStreamSynchronize(st));
+    if (h->check_sym && h->hp->sym_flag) return fail(RFOE_ERR_NOT_SYMMETRIC);
+    const double emin = h->hp->bounds[0], emax = h->hp->bounds[1];
+    S.eps_min = emin; S.eps_max = emax;
+    if (!(isfinite(emin) && isfinite(emax) && emax > emin)) return fail(RFOE_ERR_BAD_BOUNDS);
+
+    Ctrl& C = h->hp->ctrl;
+    memset(&C, 0, sizeof(Ctrl));
+    C.variant = variant; C.stop_rule = h->stop_rule; C.max_iter = h->max_iter; C.kvalid = k;
+    C.nocc = (double)nocc; C.tol = tol;
+    C.mixed_head = h->mixed_head; C.mixed_reltr = h->mixed_reltr;
+    C.mixed_phase = (variant == RFOE_VARIANT_SP2_MIXED) ? (h->mixed_head > 0.0 ? 0 : 1) : 2;
+    C.reltr_prev = INFINITY;
+    C.emin = emin; C.emax = emax;
+    if (variant == RFOE_VARIANT_SP2_ACCEL) {
+        C.homo = h->homo; C.lumo = h->lumo;
+        C.beta = (emax - h->lumo) / (emax - emin);
+        C.bbar = (emax - h->homo) / (emax - emin);
+    }
+    CK(cudaMemcpyAsync(h->d_ctrl, &C, sizeof(Ctrl), cudaMemcpyHostToDevice, st));
+
+    affine_map_kernel<<<hbm_grid(h, ld), HBM_THREADS, 0, st>>>(Hp, k, ld, h->d_bounds, h->W[0], h->rows[0], h->rows[1]);
+    h->launches++;
+    CK(cudaGetLastError());
+    h->hp->word = -1;
+    control_kernel<<<1, 256, 0, st>>>(h->d_ctrl, 0, h->rows[0], h->rows[1], k, h->d_word);
+    h->launches++;
+    CK(cudaGetLastError());
+    CK(cudaStreamSynchronize(st));
+
+    // --- the recursion: one scalar (the action word) crosses to the host per step ----------------
+    int cur = 0;
+    int action = h->hp->word;
+    h->sq_n = 0;
+    while (action != ACT_STOP) {
+        const int nxt = cur ^ 1;
+        if (action == ACT_SP2) {
+            CK(timed_square<false>(h, tm[cur], tm[cur], h->W[cur], h->W[nxt], ld, k, &h->d_ctrl->coef, h->part[0], st));
+            control_kernel<<<1, 256, 0, st>>>(h->d_ctrl, 1, h->part[0], h->part[0], h->n_tiles, h->d_word);
+        } else if (action == ACT_MCWEENY) {
+            CK(timed_square<false>(h, tm[cur], tm[cur], h->W[cur], h->W[2], ld, k, &h->d_ctrl->coef, h->part[0], st));
+            CK(timed_square<true>(h, tm[2], tm[cur], h->W[2], h->W[nxt], ld, k, &h->d_ctrl->coef_aux, h->part[1], st));
+            control_kernel<<<1, 256, 0, st>>>(h->d_ctrl, 1, h->part[1], h->part[0], h->n_tiles, h->d_word);
+        } else {
+            return fail(RFOE_ERR_UNSUPPORTED);
+        }
+        h->launches++;
+        CK(cudaGetLastError());
+        CK(cudaStreamSynchronize(st));
+        action = h->hp->word;
+        cur = nxt;
+    }
+
+    // --- output pass: P and tr(P H) ---------------------------------------------------------------
+    copy_out_kernel<<<hbm_grid(h, k), HBM_THREADS, 0, st>>>(h->W[cur], k, ld, Hp, P, h->rows[0]);
+    h->launches++;
+    CK(cudaGetLastError());
+    sum_rows_kernel<<<1, 256, 0, st>>>(h->rows[0], k, &h->d_ctrl->tr_PH);
+    h->launches++;
+    CK(cudaGetLastError());
+    CK(cudaEventRecord(h->ev1, st));
+    CK(cudaMemcpyAsync(&C, h->d_ctrl, sizeof(Ctrl), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    float ms = 0.f;
+    CK(cudaEventElapsedTime(&ms, h->ev0, h->ev1));
+
+    S.iterations = C.step; S.multiplications = C.multiplications; S.mcweeny_steps = C.mcweeny_steps;
+    S.fp32_steps = C.fp32_steps; S.converged = C.converged; S.tr_PH = C.tr_PH; S.device_ms = ms;
+    S.gpu_launches = h->launches;
+    S.square_launches = h->sq_n;
+    for (int i = 0; i < h->sq_n; ++i) {
+        float sq = 0.f;
+        CK(cudaEventElapsedTime(&sq, h->sq_ev[2 * i], h->sq_ev[2 * i + 1]));
+        S.square_ms += sq;
+    }
+    const int n = C.step;
+    memcpy(S.t, C.ht, sizeof(double) * (n + 1));
+    memcpy(S.s, C.hs, sizeof(double) * (n + 1));
+    memcpy(S.e, C.he, sizeof(double) * n);
+    memcpy(S.reltr, C.hreltr, sizeof(double) * n);
+    memcpy(S.branch, C.branch, n);
+    S.branch[n] = 0;
+    S.status = C.converged ? RFOE_OK : RFOE_ERR_NOT_CONVERGED;
+    return S.status;
+}
+
+// ---------------------------------------------------------------------------------------------
+// single products (kernel-level entry points for tests and roofline timing)
+static int single_product(rfoe_handle_s* h, const double* A, const double* B, int64_t k64, double c2, double c1, double c0,
+                          double* Cout, double* scalars, float* kernel_ms, cudaStream_t st)
+{
+    if (!h || !A || !Cout || k64 < 1 || k64 > h->k_max) return RFOE_ERR_INVALID_ARG;
+    const bool two = (B != nullptr);
+    const int k = (int)k64, ld = round_up(k, SQ_BM), m = ld / SQ_BM;
+    int rc;
+    h->launches = 0;
+    h->stats.cuda_error = 0;
+    CK(cudaSetDevice(h->device));
+    if ((rc = ensure_third(h)) != RFOE_OK) return rc;
+    if ((rc = ensure_tiles(h, m, st)) != RFOE_OK) return rc;
+    CUtensorMap tm[3];
+    for (int i = 0; i < 3; ++i)
+        if ((rc = make_map(h, &tm[i], h->W[i], ld)) != RFOE_OK) return rc;
+    pad_copy_kernel<<<hbm_grid(h, ld), HBM_THREADS, 0, st>>>(A, k, ld, h->W[0]);
+    h->launches++;
+    if (two) {
+        pad_copy_kernel<<<hbm_grid(h, ld), HBM_THREADS, 0, st>>>(B, k, ld, h->W[1]);
+        h->launches++;
+    }
+    CK(cudaGetLastError());
+    Ctrl& C = h->hp->ctrl;
+    C.coef = StepCoef{c2, c1, c0};
+    CK(cudaMemcpyAsync(&h->d_ctrl->coef, &C.coef, sizeof(StepCoef), cudaMemcpyHostToDevice, st));
+    CK(cudaEventRecord(h->ev0, st));
+    if (two) CK(launch_square<true>(h, tm[0], tm[1], h->W[0], h->W[2], ld, k, &h->d_ctrl->coef, h->part[0], st));
+    else     CK(launch_square<false>(h, tm[0], tm[0], h->W[0], h->W[2], ld, k, &h->d_ctrl->coef, h->part[0], st));
+    CK(cudaEventRecord(h->ev1, st));
+    sum_partials_kernel<<<1, 256, 0, st>>>(h->part[0], h->n_tiles, h->d_scalars);
+    h->launches++;
+    copy_out_kernel<<<hbm_grid(h, k), HBM_THREADS, 0, st>>>(h->W[2], k, ld, nullptr, Cout, nullptr);
+    h->launches++;
+    CK(cudaGetLastError());
+    CK(cudaMemcpyAsync((void*)h->hp->scalars, h->d_scalars, 5 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    if (scalars) for (int i = 0; i < 5; ++i) scalars[i] = h->hp->scalars[i];
+    if (kernel_ms) CK(cudaEventElapsedTime(kernel_ms, h->ev0, h->ev1));
+    h->stats.gpu_launches = h->launches;
+    return RFOE_OK;
+}
+
+extern "C" int rfoe_square(rfoe_handle_t h, const double* X, int64_t k, double c2, double c1, double c0, double* Xout,
+                           double* scalars, float* kernel_ms, rfoe_stream_t stream)
+{
+    return single_product(h, X, nullptr, k, c2, c1, c0, Xout, scalars, kernel_ms, (cudaStream_t)stream);
+}
+
+extern "C" int rfoe_symm_product(rfoe_handle_t h, const double* A, const double* B, int64_t k, double c2, double c1, double c0,
+                                 double* Cout, double* scalars, float* kernel_ms, rfoe_stream_t stream)
+{
+    if (!B) return RFOE_ERR_INVALID_ARG;
+    return single_product(h, A, B, k, c2, c1, c0, Cout, scalars, kernel_ms, (cudaStream_t)stream);
+}
+
+// ---------------------------------------------------------------------------------------------
+// end-to-end entry point with host buffers
+extern "C" int rfoe_expand_host(rfoe_handle_t h, const double* Hp_host, int64_t k, int64_t nocc, int variant, double tol,
+                                double* P_host, rfoe_stream_t stream)
+{
+    int rc = check_common(h, Hp_host, P_host, k);
+    if (rc != RFOE_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    CK(cudaSetDevice(h->device));
+    const size_t cap = (size_t)h->k_max * h->k_max * sizeof(double);
+    if (!h->stage_H && cudaMalloc(&h->stage_H, cap) != cudaSuccess) { cudaGetLastError(); return RFOE_ERR_ALLOC; }
+    if (!h->stage_P && cudaMalloc(&h->stage_P, cap) != cudaSuccess) { cudaGetLastError(); return RFOE_ERR_ALLOC; }
+    const size_t bytes = (size_t)k * k * sizeof(double);
+    CK(cudaMemcpyAsync(h->stage_H, Hp_host, bytes, cudaMemcpyHostToDevice, st));
+    rc = rfoe_expand(h, h->stage_H, k, nocc, variant, tol, h->stage_P, stream);
+    if (rc != RFOE_OK && rc != RFOE_ERR_NOT_CONVERGED) return rc;
+    CK(cudaMemcpyAsync(P_host, h->stage_P, bytes, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    return rc;
+}

@@ -1,0 +1,221 @@
+// Symmetric squaring / symmetric product on the FP64 tensor cores (rows A4 + A5 of DESIGN.md).
+//
+// Computes, for upper-triangle tile pairs I <= J only,
+//     C_IJ = sum_l A(I, l) * B(J, l)^T            (A = B = X_n: the SYRK form of X_n * X_n;
+//                                                  A = X_n^2, B = X_n: the McWeeny product)
+// and fuses the whole recursion update into the epilogue:
+//     Out = c2 * C + c1 * E + c0 * I  written to (I,J) and mirrored to (J,I)
+//     per-tile partial sums of Tr Out, ||Out||_F^2, ||C - E||_F^2, Tr C, <C, E>
+// "matrix-matrix multiplication is the computationally dominant step".
+//
+// Layout: all matrices are ld x ld (ld = k rounded up to 128), zero outside k x k, row-major FP64.
+// Because X is bitwise symmetric, both operands are K-contiguous row panels (128 rows x 16 doubles
+// = 128-byte rows) fetched by TMA with the 128-byte swizzle into a 6-stage mbarrier ring; eight warps
+// (2 x 4, 64 x 32 outputs each) issue mma.m8n8k4.f64 (SASS DMMA.8x8x4) with accumulators in registers,
+// and lane 0 of warp 0 doubles as the TMA producer: it refills a stage as soon as a non-blocking
+// mbarrier test shows all eight warps have released it (2 warps per SMSP keep the 255-register budget).
+// Fragment row m of a 16-row group maps to tile row 2m + p (p = 0, 1): with the 128B swizzle this makes every 64-bit fragment load bank-conflict free.
+#pragma once
+#include "ptx_sm100.cuh"
+
+namespace rfoe {
+
+constexpr int SQ_BM = 128;               // tile rows = tile cols
+constexpr int SQ_BK = 16;                // doubles per K chunk = one 128-byte swizzle row
+constexpr int SQ_STAGES = 6;
+constexpr int SQ_CONSUMER_WARPS = 8;
+constexpr int SQ_THREADS = SQ_CONSUMER_WARPS * 32;   // no 9th warp: 3 warps on one SMSP would cap registers at 168
+constexpr int SQ_PANEL_BYTES = SQ_BM * SQ_BK * 8;                    // 16 KiB
+constexpr int SQ_SMEM_BYTES = SQ_STAGES * 2 * SQ_PANEL_BYTES + 1024; // + slack for 1024-byte alignment
+constexpr int SQ_NPART = 8;              // doubles per tile record in the partials array (5 used)
+
+struct StepCoef {
+    double c2, c1, c0;
+};
+
+template <bool TWO_OP>
+__global__ void __launch_bounds__(SQ_THREADS, 1)
+sym_square_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
+                  const double* __restrict__ E, double* __restrict__ Out, int ld, int kvalid,
+                  const StepCoef* __restrict__ coef, const int2* __restrict__ tile_map,
+                  double* __restrict__ partials)
+{
+    extern __shared__ uint8_t smem_raw[];
+    __shared__ __align__(8) uint64_t full_bar[SQ_STAGES];
+    __shared__ __align__(8) uint64_t empty_bar[SQ_STAGES];
+    __shared__ double red[SQ_CONSUMER_WARPS][5];
+
+    const int warp = threadIdx.x >> 5;
+    const int lane = threadIdx.x & 31;
+    const int2 tile = tile_map[blockIdx.x];
+    const int I = tile.x, J = tile.y;
+    const bool diag = (I == J);
+    const bool two_panels = TWO_OP || !diag;
+    const int KT = ld / SQ_BK;
+
+    const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    const uint32_t full0 = smem_u32(&full_bar[0]);
+    const uint32_t empty0 = smem_u32(&empty_bar[0]);
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < SQ_STAGES; ++s) {
+            mbar_init(full0 + 8 * s, 1);
+            mbar_init(empty0 + 8 * s, SQ_CONSUMER_WARPS);
+        }
+        mbar_fence_init();
+    }
+    if (threadIdx.x == 0) {
+        tma_prefetch_desc(&tmA);
+        if (TWO_OP) tma_prefetch_desc(&tmB);
+    }
+    __syncthreads();
+
+    // ===== TMA producer state (meaningful in lane 0 of warp 0 only) =====
+    const uint32_t stage_bytes = two_panels ? 2 * SQ_PANEL_BYTES : SQ_PANEL_BYTES;
+    int ld_kt = 0, ld_s = 0;
+    uint32_t ld_ph = 0;
+    auto issue_loads = [&](int upto) {
+        while (ld_kt < upto) {
+            if (ld_kt >= SQ_STAGES && !mbar_test(empty0 + 8 * ld_s, ld_ph ^ 1u)) break;
+            const uint32_t fb = full0 + 8 * ld_s;
+            mbar_expect_tx(fb, stage_bytes);
+            const uint32_t dstA = smem_base + ld_s * (2 * SQ_PANEL_BYTES);
+            tma_load_2d(dstA, &tmA, ld_kt * SQ_BK, I * SQ_BM, fb);
+            if (two_panels) tma_load_2d(dstA + SQ_PANEL_BYTES, TWO_OP ? &tmB : &tmA, ld_kt * SQ_BK, J * SQ_BM, fb);
+            ++ld_kt;
+            if (++ld_s == SQ_STAGES) { ld_s = 0; ld_ph ^= 1u; }
+        }
+    };
+    if (threadIdx.x == 0) issue_loads(min(KT, SQ_STAGES));
+    {
+        // ===== consumers =====
+        const int warp_m = warp >> 2;      // 0..1  -> 64 tile rows
+        const int warp_n = warp & 3;       // 0..3  -> 32 tile cols
+        const int r = lane >> 2;           // fragment row / col index 0..7
+        const int kk = lane & 3;           // k index inside the k4 step; also C column pair index
+        // swizzled byte offset inside a 128-byte panel row for (k4-step ks, parity p)
+        uint32_t off[4][2];
+#pragma unroll
+        for (int ks = 0; ks < 4; ++ks)
+#pragma unroll
+            for (int p = 0; p < 2; ++p)
+                off[ks][p] = ((uint32_t)(((2 * ks + (kk >> 1)) ^ ((2 * r + p) & 7)) << 4)) + (uint32_t)((kk & 1) * 8);
+        const uint32_t rowA = (uint32_t)(warp_m * 64 + 2 * r) * 128u;
+        const uint32_t rowB = (uint32_t)(warp_n * 32 + 2 * r) * 128u + (two_panels ? (uint32_t)SQ_PANEL_BYTES : 0u);
+
+        double acc[8][4][2];
+#pragma unroll
+        for (int mi = 0; mi < 8; ++mi)
+#pragma unroll
+            for (int ni = 0; ni < 4; ++ni) acc[mi][ni][0] = acc[mi][ni][1] = 0.0;
+
+        int s = 0;
+        uint32_t ph = 0;
+        for (int kt = 0; kt < KT; ++kt) {
+            if (threadIdx.x == 0) issue_loads(min(KT, kt + SQ_STAGES));
+            __syncwarp();
+            mbar_wait(full0 + 8 * s, ph);
+            const uint32_t st = smem_base + s * (2 * SQ_PANEL_BYTES);
+            const uint32_t aB = st + rowA, bB = st + rowB;
+#pragma unroll
+            for (int ks = 0; ks < 4; ++ks) {
+                double a[8], b[4];
+#pragma unroll
+                for (int mi = 0; mi < 8; ++mi)
+                    a[mi] = lds_f64(aB + (uint32_t)((mi >> 1) * 2048 + (mi & 1) * 128) + off[ks][mi & 1]);
+#pragma unroll
+                for (int ni = 0; ni < 4; ++ni)
+                    b[ni] = lds_f64(bB + (uint32_t)((ni >> 1) * 2048 + (ni & 1) * 128) + off[ks][ni & 1]);
+#pragma unroll
+                for (int mi = 0; mi < 8; ++mi)
+#pragma unroll
+                    for (int ni = 0; ni < 4; ++ni) dmma_8x8x4(acc[mi][ni][0], acc[mi][ni][1], a[mi], b[ni]);
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(empty0 + 8 * s);
+            if (++s == SQ_STAGES) { s = 0; ph ^= 1u; }
+        }
+
+        // ===== fused epilogue =====
+        const double c2 = coef->c2, c1 = coef->c1, c0 = coef->c0;
+        double p_tr = 0.0, p_ss = 0.0, p_err = 0.0, p_trc = 0.0, p_ce = 0.0;
+        const int row_base = I * SQ_BM + warp_m * 64 + 2 * r;       // + 16 g + p
+        const int col_base = J * SQ_BM + warp_n * 32 + 4 * kk;      // + 16 h + u
+#pragma unroll
+        for (int g = 0; g < 4; ++g) {
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                double o[2][4];
+                const int col = col_base + 16 * h;
+#pragma unroll
+                for (int p = 0; p < 2; ++p) {
+                    const int row = row_base + 16 * g + p;
+                    const int mi = 2 * g + p;
+                    const double cv[4] = {acc[mi][2 * h][0], acc[mi][2 * h + 1][0], acc[mi][2 * h][1], acc[mi][2 * h + 1][1]};
+                    const double2 e01 = *reinterpret_cast<const double2*>(E + (size_t)row * ld + col);
+                    const double2 e23 = *reinterpret_cast<const double2*>(E + (size_t)row * ld + col + 2);
+                    const double ev[4] = {e01.x, e01.y, e23.x, e23.y};
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        double v = fma(c2, cv[u], c1 * ev[u]);
+                        const double d = cv[u] - ev[u];
+                        double w = 1.0;   // off-diagonal tiles: x2 applied once at the end
+                        if (diag) {
+                            const int cc = col + u;
+                            w = (cc > row) ? 2.0 : ((cc == row) ? 1.0 : 0.0);
+                            if (cc == row) {
+                                if (row < kvalid) v += c0;
+                                p_tr += v;
+                                p_trc += cv[u];
+                            }
+                        }
+                        o[p][u] = v;
+                        p_ss = fma(w * v, v, p_ss);
+                        p_err = fma(w * d, d, p_err);
+                        p_ce = fma(w * cv[u], ev[u], p_ce);
+                    }
+                    if (!diag) {
+                        *reinterpret_cast<double2*>(Out + (size_t)row * ld + col) = make_double2(o[p][0], o[p][1]);
+                        *reinterpret_cast<double2*>(Out + (size_t)row * ld + col + 2) = make_double2(o[p][2], o[p][3]);
+                    } else {
+#pragma unroll
+                        for (int u = 0; u < 4; ++u)
+                            if (col + u >= row) Out[(size_t)row * ld + col + u] = o[p][u];
+                    }
+                }
+                // mirrored store: element (row, col+u) -> (col+u, row); rows 2r and 2r+1 are adjacent
+                const int row0 = row_base + 16 * g;
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    if (!diag) {
+                        *reinterpret_cast<double2*>(Out + (size_t)(col + u) * ld + row0) = make_double2(o[0][u], o[1][u]);
+                    } else {
+                        if (col + u > row0) Out[(size_t)(col + u) * ld + row0] = o[0][u];
+                        if (col + u > row0 + 1) Out[(size_t)(col + u) * ld + row0 + 1] = o[1][u];
+                    }
+                }
+            }
+        }
+        if (!diag) { p_ss *= 2.0; p_err *= 2.0; p_ce *= 2.0; }
+#pragma unroll
+        for (int m = 16; m >= 1; m >>= 1) {
+            p_tr += __shfl_xor_sync(0xffffffffu, p_tr, m);
+            p_ss += __shfl_xor_sync(0xffffffffu, p_ss, m);
+            p_err += __shfl_xor_sync(0xffffffffu, p_err, m);
+            p_trc += __shfl_xor_sync(0xffffffffu, p_trc, m);
+            p_ce += __shfl_xor_sync(0xffffffffu, p_ce, m);
+        }
+        if (lane == 0) {
+            red[warp][0] = p_tr; red[warp][1] = p_ss; red[warp][2] = p_err; red[warp][3] = p_trc; red[warp][4] = p_ce;
+        }
+    }
+    __syncthreads();
+    if (threadIdx.x < 5) {
+        double v = 0.0;
+#pragma unroll
+        for (int w = 0; w < SQ_CONSUMER_WARPS; ++w) v += red[w][threadIdx.x];
+        partials[(size_t)blockIdx.x * SQ_NPART + threadIdx.x] = v;
+    }
+}
+
+}  // namespace rfoe

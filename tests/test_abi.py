@@ -1,0 +1,67 @@
+"""CPU-side checks of the C-ABI boundary: the library builds/loads here (no GPU), exports every symbol
+include/rfoe.h declares, and fails loudly -- never falls back -- when no CUDA device is present."""
+import ctypes
+import os
+import re
+
+import pytest
+
+import paper_2301_04642_b200 as rfoe
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _declared_symbols():
+    txt = open(os.path.join(ROOT, "include", "rfoe.h")).read()
+    txt = re.sub(r"/\*.*?\*/", "", txt, flags=re.S)
+    return sorted(set(re.findall(r"\b(rfoe_[a-z_]+)\s*\(", txt)))
+
+
+def test_header_symbols_are_exported():
+    L = rfoe.load_library()
+    declared = _declared_symbols()
+    assert set(declared) == set(rfoe.EXPORTS)
+    for name in declared:
+        assert hasattr(L, name), name
+    assert L.rfoe_version() == 100
+    assert L.rfoe_strerror(0) == b"ok" and b"symmetric" in L.rfoe_strerror(5)
+
+
+def test_stats_struct_matches_header():
+    # sizeof(rfoe_stats_t) computed from the header's field list
+    n = rfoe.MAX_STEPS
+    expect = 10 * 4 + 3 * 8 + 6 * 8 + (n + 1) * 8 * 2 + n * 8 * 2 + (n + 8)
+    expect = (expect + 7) // 8 * 8
+    assert ctypes.sizeof(rfoe._Stats) == expect
+
+
+def test_argument_errors_without_gpu():
+    L = rfoe.load_library()
+    h = ctypes.c_void_p()
+    assert L.rfoe_create(None, 0, 16) == rfoe.ERR_INVALID_ARG
+    assert L.rfoe_create(ctypes.byref(h), 0, 0) == rfoe.ERR_INVALID_ARG
+    assert L.rfoe_destroy(None) == rfoe.OK
+    assert L.rfoe_set_option(None, 0, 0.0) == rfoe.ERR_INVALID_ARG
+
+
+def test_no_cpu_fallback():
+    import torch
+
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    with pytest.raises(rfoe.RfoeError) as ei:
+        rfoe.Rfoe(64)
+    assert ei.value.status == rfoe.ERR_CUDA
+
+
+def test_product_does_not_import_oracle():
+    pkg = os.path.join(ROOT, "paper_2301_04642_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert "oracle" not in src.replace("no CPU fallback", ""), f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".c")):
+            src = open(os.path.join(ROOT, "oracle", f)).read()
+            assert "import paper_2301_04642_b200" not in src and "csrc/" not in src.replace("paper_2301_04642_b200/csrc/", "")

@@ -1,0 +1,231 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle on the same seeded inputs.
+
+Tolerances (north_star, FP64 path): ||P_gpu - P_oracle||_F / sqrt(k) <= 1e-10, |tr(P H) difference| / |tr| <= 1e-11,
+identical iteration counts; branch strings identical wherever t_n - nocc is above rounding level (R10).
+Kernel-level products: the DMMA path and the oracle sum the same k products per element in different
+orders, so |C_gpu - C_oracle| <= 4 k eps max|x|^2.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+import rfoe_inputs
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+import paper_2301_04642_b200 as rfoe  # noqa: E402
+
+EPS = 2.0 ** -52
+
+
+@pytest.fixture(scope="module")
+def handle():
+    h = rfoe.Rfoe(2048)
+    yield h
+    h.close()
+
+
+def _dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _sym(k, seed, scale=1.0):
+    rng = np.random.default_rng(seed)
+    X = rng.standard_normal((k, k)) * scale
+    return np.ascontiguousarray(0.5 * (X + X.T))
+
+
+# ------------------------------------------------------------------ A1: Gershgorin
+@pytest.mark.parametrize("k", [1, 2, 7, 64, 129, 255, 1000, 2048])
+def test_bounds_parity(handle, k):
+    H = _sym(k, 10 + k)
+    lo, hi = handle.bounds(_dev(H))
+    olo, ohi = oracle.bounds(H)
+    tol = 4 * k * EPS * max(abs(olo), abs(ohi), 1.0)
+    assert abs(lo - olo) <= tol and abs(hi - ohi) <= tol
+
+
+# ------------------------------------------------------------------ A4 + A5: one squaring, all outputs
+@pytest.mark.parametrize("k", [1, 5, 64, 128, 130, 257, 384, 777])
+@pytest.mark.parametrize("coef", [(1.0, 0.0, 0.0), (-1.0, 2.0, 0.0), (1.21, -0.44, 0.04)])
+def test_square_parity(handle, k, coef):
+    X = _sym(k, 100 + k, scale=1.0 / math.sqrt(k))
+    c2, c1, c0 = coef
+    out, sc, ms = handle.square(_dev(X), c2, c1, c0)
+    out = out.cpu().numpy()
+    Y = oracle.square(X)
+    ref = c2 * Y + c1 * X + c0 * np.eye(k)
+    xmax = np.abs(X).max()
+    tol = 4 * k * EPS * xmax * xmax * (abs(c2) + 1) + 4 * EPS * np.abs(ref).max()
+    assert np.abs(out - ref).max() <= tol
+    assert np.array_equal(out, out.T)                                  # bitwise symmetric
+    rel = 1e-12
+    assert sc[0] == pytest.approx(np.trace(ref), rel=rel, abs=1e-13)
+    assert sc[1] == pytest.approx(np.sum(ref * ref), rel=rel)
+    assert sc[2] == pytest.approx(np.sum((Y - X) ** 2), rel=rel)
+    assert sc[3] == pytest.approx(np.trace(Y), rel=rel)
+    assert sc[3] == pytest.approx(np.sum(X * X), rel=rel)                # Tr(X^2) = ||X||_F^2
+    assert sc[4] == pytest.approx(np.sum(Y * X), rel=1e-10, abs=1e-12)
+    if coef == (1.0, 0.0, 0.0):
+        # exact when every product and partial sum is representable: small integers
+        Xi = np.random.default_rng(k).integers(-3, 4, size=(k, k)).astype(np.float64)
+        Xi = np.triu(Xi) + np.triu(Xi, 1).T
+        outi, _, _ = handle.square(_dev(Xi))
+        assert np.array_equal(outi.cpu().numpy(), oracle.square(Xi))
+
+
+@pytest.mark.parametrize("k", [3, 128, 200, 515])
+def test_symm_product_parity(handle, k):
+    X = _sym(k, 300 + k, scale=1.0 / math.sqrt(k))
+    Y = oracle.square(X)                                                 # commutes with X, symmetric
+    out, sc, _ = handle.symm_product(_dev(Y), _dev(X), -2.0, 3.0, 0.0)     # McWeeny: 3Y - 2YX
+    out = out.cpu().numpy()
+    Z = oracle.matmul(Y, X)
+    ref = np.triu(3.0 * Y - 2.0 * Z)
+    ref = ref + np.triu(ref, 1).T
+    tol = 8 * k * EPS * np.abs(Y).max() * np.abs(X).max() + 8 * EPS * np.abs(ref).max()
+    assert np.abs(out - ref).max() <= tol
+    assert np.array_equal(out, out.T)
+    assert sc[0] == pytest.approx(np.trace(ref), rel=1e-12)
+    assert sc[1] == pytest.approx(np.sum(ref * ref), rel=1e-12)
+
+
+# ------------------------------------------------------------------ whole expansions
+def _check_expansion(w, res, ref, *, ptol=1e-10, etol=1e-11):
+    k = w.k
+    P = res.P.cpu().numpy() if hasattr(res.P, "cpu") else res.P
+    assert res.converged == ref.converged
+    assert res.iterations == ref.iterations
+    decided = np.abs(ref.t[: ref.iterations] - w.nocc) > 1e-9 * max(1.0, k / 256)
+    assert all(a == b for a, b, d in zip(res.branch, ref.branch, decided) if d), (res.branch, ref.branch)
+    assert np.linalg.norm(P - ref.P) / math.sqrt(k) <= ptol
+    assert abs(res.tr_PH - ref.tr_PH) / abs(ref.tr_PH) <= etol
+    assert np.array_equal(P, P.T)
+    assert abs(res.eps_min - ref.emin) <= 1e-12 * abs(ref.emin) and abs(res.eps_max - ref.emax) <= 1e-12 * abs(ref.emax)
+    n = ref.iterations
+    assert np.allclose(res.t, ref.t, rtol=0, atol=1e-9 * k / 256)
+    assert np.allclose(res.s, ref.s, rtol=0, atol=1e-9 * k / 256)
+    assert np.allclose(res.e[: n - 1], ref.e[: n - 1], rtol=1e-6, atol=1e-11 * k / 256)
+    # north_star invariants on the GPU result, and the construction-exact projector (pin P2)
+    if ref.converged:
+        assert abs(np.trace(P) - w.nocc) <= 1e-9
+        assert np.linalg.norm(P @ P - P) <= 1e-10 * k / 256
+        H = w.H
+        assert np.linalg.norm(H @ P - P @ H) <= 1e-10 * k / 256
+        assert np.linalg.norm(P - w.exact_projector()) / math.sqrt(k) <= 1e-10
+
+
+def test_expand_config1(handle):
+    w = rfoe_inputs.make_workload(1)
+    ref = oracle.expand(w.H, w.nocc, tol=w.tol)
+    res = handle.expand(_dev(w.H), w.nocc, rfoe.SP2, w.tol)
+    assert res.status == rfoe.OK and res.iterations == 34
+    _check_expansion(w, res, ref)
+
+
+@pytest.mark.parametrize("c,k", [(1, 100), (2, 333), (3, 200), (4, 450), (5, 129)])
+def test_expand_ragged_sizes(handle, c, k):
+    w = rfoe_inputs.make_workload(c, k=k)
+    ref = oracle.expand(w.H, w.nocc, tol=w.tol)
+    res = handle.expand(_dev(w.H), w.nocc, rfoe.SP2, w.tol)
+    _check_expansion(w, res, ref)
+
+
+def test_expand_rule_b(handle):
+    w = rfoe_inputs.make_workload(2, k=300)
+    ref = oracle.expand(w.H, w.nocc, tol=5e-8, stop_rule=oracle.RULE_B)
+    handle.configure(stop_rule=rfoe.RULE_B)
+    try:
+        res = handle.expand(_dev(w.H), w.nocc, rfoe.SP2, 5e-8)
+    finally:
+        handle.configure(stop_rule=rfoe.RULE_A)
+    _check_expansion(w, res, ref, ptol=1e-9)
+    assert np.allclose(res.reltr, ref.reltr, rtol=1e-6, atol=1e-13)
+
+
+def test_expand_bounds_override_and_truncated(handle):
+    w = rfoe_inputs.make_workload(1, k=160)
+    lo, hi = float(w.lam.min()) - 0.01, float(w.lam.max()) + 0.01
+    handle.configure(bounds=(lo, hi))
+    try:
+        ref = oracle.expand(w.H, w.nocc, tol=w.tol, bounds_override=(lo, hi))
+        res = handle.expand(_dev(w.H), w.nocc, rfoe.SP2, w.tol)
+        _check_expansion(w, res, ref)
+        assert res.iterations < 30
+        # T-RFOE: truncated expansion G_m
+        handle.configure(max_iter=7)
+        ref = oracle.expand(w.H, w.nocc, tol=0.0, max_iter=7, bounds_override=(lo, hi))
+        res = handle.expand(_dev(w.H), w.nocc, rfoe.SP2, 0.0)
+        assert res.status == rfoe.ERR_NOT_CONVERGED and res.iterations == 7
+        _check_expansion(w, res, ref)
+    finally:
+        handle.configure(bounds=False, max_iter=100)
+
+
+def test_expand_mcweeny(handle):
+    w = rfoe_inputs.make_workload(2, k=260)
+    ref = oracle.expand(w.H, w.nocc, variant=oracle.MCWEENY, tol=w.tol)
+    res = handle.expand(_dev(w.H), w.nocc, rfoe.MCWEENY, w.tol)
+    assert res.mcweeny_steps == ref.mcweeny_steps >= 1 and res.multiplications == ref.multiplications
+    _check_expansion(w, res, ref)
+
+
+def test_expand_accelerated(handle):
+    w = rfoe_inputs.make_workload(3, k=256)
+    homo, lumo = float(w.lam[: w.nocc].max()), float(w.lam[w.nocc:].min())
+    ref = oracle.expand(w.H, w.nocc, variant=oracle.SP2_ACCEL, tol=w.tol, homo=homo, lumo=lumo)
+    handle.configure(homo=homo, lumo=lumo)
+    res = handle.expand(_dev(w.H), w.nocc, rfoe.SP2_ACCEL, w.tol)
+    _check_expansion(w, res, ref)
+    plain = handle.expand(_dev(w.H), w.nocc, rfoe.SP2, w.tol)
+    assert res.iterations < plain.iterations
+
+
+def test_expand_host_entry_point(handle):
+    w = rfoe_inputs.make_workload(1, k=192)
+    ref = oracle.expand(w.H, w.nocc, tol=w.tol)
+    res = handle.expand_host(w.H, w.nocc, rfoe.SP2, w.tol)
+    _check_expansion(w, res, ref)
+
+
+def test_expand_config2_full(handle):
+    w = rfoe_inputs.make_workload(2)
+    ref = oracle.expand(w.H, w.nocc, tol=w.tol)
+    res = handle.expand(_dev(w.H), w.nocc, rfoe.SP2, w.tol)
+    assert res.iterations == 42
+    _check_expansion(w, res, ref)
+
+
+# ------------------------------------------------------------------ errors and degenerate inputs
+def test_error_paths(handle):
+    w = rfoe_inputs.make_workload(1, k=64)
+    H = _dev(w.H)
+    with pytest.raises(rfoe.RfoeError) as ei:
+        handle.expand(H, 0, rfoe.SP2, 1e-12)
+    assert ei.value.status == rfoe.ERR_INVALID_ARG
+    with pytest.raises(rfoe.RfoeError) as ei:
+        handle.expand(H, 64, rfoe.SP2, 1e-12)
+    assert ei.value.status == rfoe.ERR_INVALID_ARG
+    with pytest.raises(rfoe.RfoeError) as ei:
+        handle.expand(H, 10, 17, 1e-12)
+    assert ei.value.status == rfoe.ERR_UNSUPPORTED
+    with pytest.raises(rfoe.RfoeError) as ei:
+        handle.expand(H, 10, rfoe.SP2, 1e-12, P=H)
+    assert ei.value.status == rfoe.ERR_INVALID_ARG
+    Hbad = H.clone()
+    Hbad[3, 5] += 1e-9
+    with pytest.raises(rfoe.RfoeError) as ei:
+        handle.expand(Hbad, 10, rfoe.SP2, 1e-12)
+    assert ei.value.status == rfoe.ERR_NOT_SYMMETRIC
+    with pytest.raises(rfoe.RfoeError) as ei:
+        handle.expand(torch.eye(8, dtype=torch.float64, device="cuda"), 3, rfoe.SP2, 1e-12)
+    assert ei.value.status == rfoe.ERR_BAD_BOUNDS
+    with pytest.raises(rfoe.RfoeError) as ei:
+        rfoe.Rfoe(64).expand(torch.zeros(65, 65, dtype=torch.float64, device="cuda"), 3)
+    assert ei.value.status == rfoe.ERR_INVALID_ARG
+    # the handle is still usable after errors
+    res = handle.expand(H, w.nocc, rfoe.SP2, w.tol)
+    assert res.converged
