@@ -94,7 +94,7 @@ def test_symm_product_parity(handle, k):
 
 
 # ------------------------------------------------------------------ whole expansions
-def _check_expansion(w, res, ref, *, ptol=1e-10, etol=1e-11):
+def _check_expansion(w, res, ref, *, ptol=1e-10, etol=1e-11, inv=1.0):
     k = w.k
     P = res.P.cpu().numpy() if hasattr(res.P, "cpu") else res.P
     assert res.converged == ref.converged
@@ -111,11 +111,12 @@ def _check_expansion(w, res, ref, *, ptol=1e-10, etol=1e-11):
     assert np.allclose(res.e[: n - 1], ref.e[: n - 1], rtol=1e-6, atol=1e-11 * k / 256)
     # north_star invariants on the GPU result, and the construction-exact projector (pin P2)
     if ref.converged:
-        assert abs(np.trace(P) - w.nocc) <= 1e-9
-        assert np.linalg.norm(P @ P - P) <= 1e-10 * k / 256
+        # (inv loosens them for stop rule B, which stops at RelTr 5e-8 -- before P is converged to rounding)
+        assert abs(np.trace(P) - w.nocc) <= 1e-9 * inv
+        assert np.linalg.norm(P @ P - P) <= 1e-10 * k / 256 * inv
         H = w.H
-        assert np.linalg.norm(H @ P - P @ H) <= 1e-10 * k / 256
-        assert np.linalg.norm(P - w.exact_projector()) / math.sqrt(k) <= 1e-10
+        assert np.linalg.norm(H @ P - P @ H) <= 1e-10 * k / 256 * inv
+        assert np.linalg.norm(P - w.exact_projector()) / math.sqrt(k) <= 1e-10 * inv
 
 
 def test_expand_config1(handle):
@@ -142,7 +143,7 @@ def test_expand_rule_b(handle):
         res = handle.expand(_dev(w.H), w.nocc, rfoe.SP2, 5e-8)
     finally:
         handle.configure(stop_rule=rfoe.RULE_A)
-    _check_expansion(w, res, ref, ptol=1e-9)
+    _check_expansion(w, res, ref, inv=1e4)
     assert np.allclose(res.reltr, ref.reltr, rtol=1e-6, atol=1e-13)
 
 
