@@ -58,10 +58,10 @@ gershgorin_rows_kernel(const double* __restrict__ H, int k, double* __restrict__
 }
 
 // A2 -- affine initial map (reading R2; the paper's "begins with X_0 = H"):
-// X0 = (emax I - H) / (emax - emin), true division.  X0 is written into the zero-padded ld x ld
-// work matrix (rows/cols >= k are set to zero); row_tr[i] = X0_ii, row_ss[i] = sum_j X0_ij^2.
+// X0 = (emax I - H) / (emax - emin), true division.  X0 is written into the zero-padded n x n
+// work matrix (row pitch ld) (rows/cols >= k are set to zero); row_tr[i] = X0_ii, row_ss[i] = sum_j X0_ij^2.
 __global__ void __launch_bounds__(HBM_THREADS)
-affine_map_kernel(const double* __restrict__ H, int k, int ld, const double* __restrict__ bounds,
+affine_map_kernel(const double* __restrict__ H, int k, int n, int ld, const double* __restrict__ bounds,
                   double* __restrict__ X, double* __restrict__ row_tr, double* __restrict__ row_ss)
 {
     const int lane = threadIdx.x & 31;
@@ -70,10 +70,10 @@ affine_map_kernel(const double* __restrict__ H, int k, int ld, const double* __r
     const double emin = bounds[0], emax = bounds[1];
     const double w = emax - emin;
     const bool vec = ((k & 1) == 0) && ((reinterpret_cast<uintptr_t>(H) & 15) == 0);
-    for (int i = wglobal; i < ld; i += wtotal) {
+    for (int i = wglobal; i < n; i += wtotal) {
         double* xrow = X + (size_t)i * ld;
         if (i >= k) {
-            for (int j = lane * 2; j < ld; j += 64) *reinterpret_cast<double2*>(xrow + j) = make_double2(0.0, 0.0);
+            for (int j = lane * 2; j < n; j += 64) *reinterpret_cast<double2*>(xrow + j) = make_double2(0.0, 0.0);
             continue;
         }
         const double* row = H + (size_t)i * k;
@@ -96,7 +96,7 @@ affine_map_kernel(const double* __restrict__ H, int k, int ld, const double* __r
                 xrow[j] = x;
             }
         }
-        for (int j = k + lane; j < ld; j += 32) xrow[j] = 0.0;
+        for (int j = k + lane; j < n; j += 32) xrow[j] = 0.0;
         ss = warp_sum(ss);
         if (lane == 0) {
             row_ss[i] = ss;
@@ -105,25 +105,25 @@ affine_map_kernel(const double* __restrict__ H, int k, int ld, const double* __r
     }
 }
 
-// pad copy: caller matrix (k x k, ld = k) -> zero-padded work matrix (ld x ld)
+// pad copy: caller matrix (k x k, ld = k) -> zero-padded work matrix (n x n, row pitch ld)
 __global__ void __launch_bounds__(HBM_THREADS)
-pad_copy_kernel(const double* __restrict__ src, int k, int ld, double* __restrict__ dst)
+pad_copy_kernel(const double* __restrict__ src, int k, int n, int ld, double* __restrict__ dst)
 {
     const int lane = threadIdx.x & 31;
     const int wglobal = blockIdx.x * HBM_WARPS + (threadIdx.x >> 5);
     const int wtotal = gridDim.x * HBM_WARPS;
-    for (int i = wglobal; i < ld; i += wtotal) {
+    for (int i = wglobal; i < n; i += wtotal) {
         double* drow = dst + (size_t)i * ld;
         if (i < k) {
             const double* srow = src + (size_t)i * k;
-            for (int j = lane; j < ld; j += 32) drow[j] = (j < k) ? srow[j] : 0.0;
+            for (int j = lane; j < n; j += 32) drow[j] = (j < k) ? srow[j] : 0.0;
         } else {
-            for (int j = lane; j < ld; j += 32) drow[j] = 0.0;
+            for (int j = lane; j < n; j += 32) drow[j] = 0.0;
         }
     }
 }
 
-// Output pass: P (k x k, ld = k) <- work matrix (ld x ld); row_ph[i] = sum_j P_ij H_ij (band energy
+// Output pass: P (k x k, ld = k) <- work matrix (row pitch ld); row_ph[i] = sum_j P_ij H_ij (band energy
 // tr(P H^p)).  H may be null (then only the copy is done).
 __global__ void __launch_bounds__(HBM_THREADS)
 copy_out_kernel(const double* __restrict__ W, int k, int ld, const double* __restrict__ H, double* __restrict__ P,

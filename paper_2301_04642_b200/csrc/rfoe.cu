@@ -105,9 +105,9 @@ static int ensure_tiles(rfoe_handle_s* h, int m, cudaStream_t st)
     return RFOE_OK;
 }
 
-static int make_map(rfoe_handle_s* h, CUtensorMap* map, double* base, int ld)
+static int make_map(rfoe_handle_s* h, CUtensorMap* map, double* base, int n, int ld)
 {
-    cuuint64_t dims[2] = {(cuuint64_t)ld, (cuuint64_t)ld};
+    cuuint64_t dims[2] = {(cuuint64_t)n, (cuuint64_t)n};
     cuuint64_t strides[1] = {(cuuint64_t)ld * sizeof(double)};
     cuuint32_t box[2] = {(cuuint32_t)SQ_BK, (cuuint32_t)SQ_BM};
     cuuint32_t estr[2] = {1, 1};
@@ -123,9 +123,9 @@ static int make_map(rfoe_handle_s* h, CUtensorMap* map, double* base, int ld)
 
 template <bool TWO_OP>
 static cudaError_t launch_square(rfoe_handle_s* h, const CUtensorMap& a, const CUtensorMap& b, const double* E, double* Out,
-                                 int ld, int k, const StepCoef* coef, double* partials, cudaStream_t st)
+                                 int n, int ld, int k, const StepCoef* coef, double* partials, cudaStream_t st)
 {
-    sym_square_kernel<TWO_OP><<<h->n_tiles, SQ_THREADS, SQ_SMEM_BYTES, st>>>(a, b, E, Out, ld, k, coef, h->d_tiles, partials);
+    sym_square_kernel<TWO_OP><<<h->n_tiles, SQ_THREADS, SQ_SMEM_BYTES, st>>>(a, b, E, Out, n, ld, k, coef, h->d_tiles, partials);
     h->launches++;
     return cudaGetLastError();
 }
@@ -133,11 +133,11 @@ static cudaError_t launch_square(rfoe_handle_s* h, const CUtensorMap& a, const C
 // squaring launch bracketed by its own event pair (summed into stats.square_ms after the expansion)
 template <bool TWO_OP>
 static cudaError_t timed_square(rfoe_handle_s* h, const CUtensorMap& a, const CUtensorMap& b, const double* E, double* Out,
-                                int ld, int k, const StepCoef* coef, double* partials, cudaStream_t st)
+                                int n, int ld, int k, const StepCoef* coef, double* partials, cudaStream_t st)
 {
     cudaError_t e = cudaEventRecord(h->sq_ev[2 * h->sq_n], st);
     if (e != cudaSuccess) return e;
-    e = launch_square<TWO_OP>(h, a, b, E, Out, ld, k, coef, partials, st);
+    e = launch_square<TWO_OP>(h, a, b, E, Out, n, ld, k, coef, partials, st);
     if (e != cudaSuccess) return e;
     e = cudaEventRecord(h->sq_ev[2 * h->sq_n + 1], st);
     h->sq_n++;
@@ -196,10 +196,11 @@ extern "C" int rfoe_create(rfoe_handle_t* out, int device, int64_t k_max)
     h->k_max = k_max;
     h->ld_max = round_up(k_max, SQ_BM);
     const size_t ld = (size_t)h->ld_max;
+    const size_t wbytes = ld * (ld + SQ_PAD) * sizeof(double);
     const size_t m = ld / SQ_BM, nt = m * (m + 1) / 2;
     bool ok = true;
-    ok = ok && cudaMalloc(&h->W[0], ld * ld * sizeof(double)) == cudaSuccess;
-    ok = ok && cudaMalloc(&h->W[1], ld * ld * sizeof(double)) == cudaSuccess;
+    ok = ok && cudaMalloc(&h->W[0], wbytes) == cudaSuccess;
+    ok = ok && cudaMalloc(&h->W[1], wbytes) == cudaSuccess;
     ok = ok && cudaMalloc(&h->part[0], nt * SQ_NPART * sizeof(double)) == cudaSuccess;
     ok = ok && cudaMalloc(&h->part[1], nt * SQ_NPART * sizeof(double)) == cudaSuccess;
     ok = ok && cudaMalloc(&h->rows[0], ld * sizeof(double)) == cudaSuccess;
@@ -304,7 +305,7 @@ static int ensure_third(rfoe_handle_s* h)
 {
     if (h->W[2]) return RFOE_OK;
     const size_t ld = (size_t)h->ld_max;
-    if (cudaMalloc(&h->W[2], ld * ld * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return RFOE_ERR_ALLOC; }
+    if (cudaMalloc(&h->W[2], ld * (ld + SQ_PAD) * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return RFOE_ERR_ALLOC; }
     return RFOE_OK;
 }
 
@@ -328,8 +329,9 @@ extern "C" int rfoe_expand(rfoe_handle_t h, const double* Hp, int64_t k64, int64
     if (variant == RFOE_VARIANT_SP2_ACCEL && !(isfinite(h->homo) && isfinite(h->lumo) && h->lumo > h->homo))
         return fail(RFOE_ERR_INVALID_ARG);
     const int k = (int)k64;
-    const int ld = round_up(k, SQ_BM);
-    const int m = ld / SQ_BM;
+    const int n = round_up(k, SQ_BM);      // padded extent of the work matrices
+    const int ld = n + SQ_PAD;             // their row pitch (never a power of two: see sym_square.cuh)
+    const int m = n / SQ_BM;
     cudaStream_t st = (cudaStream_t)stream;
     h->launches = 0;
     CK(cudaSetDevice(h->device));
@@ -337,7 +339,7 @@ extern "C" int rfoe_expand(rfoe_handle_t h, const double* Hp, int64_t k64, int64
     if ((rc = ensure_tiles(h, m, st)) != RFOE_OK) return fail(rc);
     CUtensorMap tm[3];
     for (int i = 0; i < 3; ++i)
-        if (h->W[i] && (rc = make_map(h, &tm[i], h->W[i], ld)) != RFOE_OK) return fail(rc);
+        if (h->W[i] && (rc = make_map(h, &tm[i], h->W[i], n, ld)) != RFOE_OK) return fail(rc);
 
     CK(cudaEventRecord(h->ev0, st));
     // --- symmetry check, bounds, affine map, first decision -------------------------------------
@@ -383,7 +385,7 @@ extern "C" int rfoe_expand(rfoe_handle_t h, const double* Hp, int64_t k64, int64
     }
     CK(cudaMemcpyAsync(h->d_ctrl, &C, sizeof(Ctrl), cudaMemcpyHostToDevice, st));
 
-    affine_map_kernel<<<hbm_grid(h, ld), HBM_THREADS, 0, st>>>(Hp, k, ld, h->d_bounds, h->W[0], h->rows[0], h->rows[1]);
+    affine_map_kernel<<<hbm_grid(h, n), HBM_THREADS, 0, st>>>(Hp, k, n, ld, h->d_bounds, h->W[0], h->rows[0], h->rows[1]);
     h->launches++;
     CK(cudaGetLastError());
     h->hp->word = -1;
@@ -399,11 +401,11 @@ extern "C" int rfoe_expand(rfoe_handle_t h, const double* Hp, int64_t k64, int64
     while (action != ACT_STOP) {
         const int nxt = cur ^ 1;
         if (action == ACT_SP2) {
-            CK(timed_square<false>(h, tm[cur], tm[cur], h->W[cur], h->W[nxt], ld, k, &h->d_ctrl->coef, h->part[0], st));
+            CK(timed_square<false>(h, tm[cur], tm[cur], h->W[cur], h->W[nxt], n, ld, k, &h->d_ctrl->coef, h->part[0], st));
             control_kernel<<<1, 256, 0, st>>>(h->d_ctrl, 1, h->part[0], h->part[0], h->n_tiles, h->d_word);
         } else if (action == ACT_MCWEENY) {
-            CK(timed_square<false>(h, tm[cur], tm[cur], h->W[cur], h->W[2], ld, k, &h->d_ctrl->coef, h->part[0], st));
-            CK(timed_square<true>(h, tm[2], tm[cur], h->W[2], h->W[nxt], ld, k, &h->d_ctrl->coef_aux, h->part[1], st));
+            CK(timed_square<false>(h, tm[cur], tm[cur], h->W[cur], h->W[2], n, ld, k, &h->d_ctrl->coef, h->part[0], st));
+            CK(timed_square<true>(h, tm[2], tm[cur], h->W[2], h->W[nxt], n, ld, k, &h->d_ctrl->coef_aux, h->part[1], st));
             control_kernel<<<1, 256, 0, st>>>(h->d_ctrl, 1, h->part[1], h->part[0], h->n_tiles, h->d_word);
         } else {
             return fail(RFOE_ERR_UNSUPPORTED);
@@ -437,13 +439,13 @@ extern "C" int rfoe_expand(rfoe_handle_t h, const double* Hp, int64_t k64, int64
         CK(cudaEventElapsedTime(&sq, h->sq_ev[2 * i], h->sq_ev[2 * i + 1]));
         S.square_ms += sq;
     }
-    const int n = C.step;
-    memcpy(S.t, C.ht, sizeof(double) * (n + 1));
-    memcpy(S.s, C.hs, sizeof(double) * (n + 1));
-    memcpy(S.e, C.he, sizeof(double) * n);
-    memcpy(S.reltr, C.hreltr, sizeof(double) * n);
-    memcpy(S.branch, C.branch, n);
-    S.branch[n] = 0;
+    const int ns = C.step;
+    memcpy(S.t, C.ht, sizeof(double) * (ns + 1));
+    memcpy(S.s, C.hs, sizeof(double) * (ns + 1));
+    memcpy(S.e, C.he, sizeof(double) * ns);
+    memcpy(S.reltr, C.hreltr, sizeof(double) * ns);
+    memcpy(S.branch, C.branch, ns);
+    S.branch[ns] = 0;
     S.status = C.converged ? RFOE_OK : RFOE_ERR_NOT_CONVERGED;
     return S.status;
 }
@@ -455,7 +457,7 @@ static int single_product(rfoe_handle_s* h, const double* A, const double* B, in
 {
     if (!h || !A || !Cout || k64 < 1 || k64 > h->k_max) return RFOE_ERR_INVALID_ARG;
     const bool two = (B != nullptr);
-    const int k = (int)k64, ld = round_up(k, SQ_BM), m = ld / SQ_BM;
+    const int k = (int)k64, n = round_up(k, SQ_BM), ld = n + SQ_PAD, m = n / SQ_BM;
     int rc;
     h->launches = 0;
     h->stats.cuda_error = 0;
@@ -464,11 +466,11 @@ static int single_product(rfoe_handle_s* h, const double* A, const double* B, in
     if ((rc = ensure_tiles(h, m, st)) != RFOE_OK) return rc;
     CUtensorMap tm[3];
     for (int i = 0; i < 3; ++i)
-        if ((rc = make_map(h, &tm[i], h->W[i], ld)) != RFOE_OK) return rc;
-    pad_copy_kernel<<<hbm_grid(h, ld), HBM_THREADS, 0, st>>>(A, k, ld, h->W[0]);
+        if ((rc = make_map(h, &tm[i], h->W[i], n, ld)) != RFOE_OK) return rc;
+    pad_copy_kernel<<<hbm_grid(h, n), HBM_THREADS, 0, st>>>(A, k, n, ld, h->W[0]);
     h->launches++;
     if (two) {
-        pad_copy_kernel<<<hbm_grid(h, ld), HBM_THREADS, 0, st>>>(B, k, ld, h->W[1]);
+        pad_copy_kernel<<<hbm_grid(h, n), HBM_THREADS, 0, st>>>(B, k, n, ld, h->W[1]);
         h->launches++;
     }
     CK(cudaGetLastError());
@@ -476,8 +478,8 @@ static int single_product(rfoe_handle_s* h, const double* A, const double* B, in
     C.coef = StepCoef{c2, c1, c0};
     CK(cudaMemcpyAsync(&h->d_ctrl->coef, &C.coef, sizeof(StepCoef), cudaMemcpyHostToDevice, st));
     CK(cudaEventRecord(h->ev0, st));
-    if (two) CK(launch_square<true>(h, tm[0], tm[1], h->W[0], h->W[2], ld, k, &h->d_ctrl->coef, h->part[0], st));
-    else     CK(launch_square<false>(h, tm[0], tm[0], h->W[0], h->W[2], ld, k, &h->d_ctrl->coef, h->part[0], st));
+    if (two) CK(launch_square<true>(h, tm[0], tm[1], h->W[0], h->W[2], n, ld, k, &h->d_ctrl->coef, h->part[0], st));
+    else     CK(launch_square<false>(h, tm[0], tm[0], h->W[0], h->W[2], n, ld, k, &h->d_ctrl->coef, h->part[0], st));
     CK(cudaEventRecord(h->ev1, st));
     sum_partials_kernel<<<1, 256, 0, st>>>(h->part[0], h->n_tiles, h->d_scalars);
     h->launches++;

@@ -8,7 +8,9 @@
 //     per-tile partial sums of Tr Out, ||Out||_F^2, ||C - E||_F^2, Tr C, <C, E>
 // "matrix-matrix multiplication is the computationally dominant step".
 //
-// Layout: all matrices are ld x ld (ld = k rounded up to 128), zero outside k x k, row-major FP64.
+// Layout: all matrices are n x n (n = k rounded up to 128), zero outside k x k, row-major FP64 with row
+// pitch ld = n + SQ_PAD doubles: a pitch of n*8 bytes is a power of two for k = 8192, 16384, ... and the 128
+// rows of every TMA box would then alias in L2 (measured: 6-9x DRAM re-reads, profiles/r01_sym_square_k16384.md).
 // Because X is bitwise symmetric, both operands are K-contiguous row panels (128 rows x 16 doubles
 // = 128-byte rows) fetched by TMA with the 128-byte swizzle into a 6-stage mbarrier ring; eight warps
 // (2 x 4, 64 x 32 outputs each) issue mma.m8n8k4.f64 (SASS DMMA.8x8x4) with accumulators in registers,
@@ -27,6 +29,7 @@ constexpr int SQ_CONSUMER_WARPS = 8;
 constexpr int SQ_THREADS = SQ_CONSUMER_WARPS * 32;   // no 9th warp: 3 warps on one SMSP would cap registers at 168
 constexpr int SQ_PANEL_BYTES = SQ_BM * SQ_BK * 8;                    // 16 KiB
 constexpr int SQ_SMEM_BYTES = SQ_STAGES * 2 * SQ_PANEL_BYTES + 1024; // + slack for 1024-byte alignment
+constexpr int SQ_PAD = 16;               // doubles added to the row pitch of the work matrices (see below)
 constexpr int SQ_NPART = 8;              // doubles per tile record in the partials array (5 used)
 
 struct StepCoef {
@@ -36,7 +39,7 @@ struct StepCoef {
 template <bool TWO_OP>
 __global__ void __launch_bounds__(SQ_THREADS, 1)
 sym_square_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
-                  const double* __restrict__ E, double* __restrict__ Out, int ld, int kvalid,
+                  const double* __restrict__ E, double* __restrict__ Out, int n, int ld, int kvalid,
                   const StepCoef* __restrict__ coef, const int2* __restrict__ tile_map,
                   double* __restrict__ partials)
 {
@@ -51,7 +54,7 @@ sym_square_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     const int I = tile.x, J = tile.y;
     const bool diag = (I == J);
     const bool two_panels = TWO_OP || !diag;
-    const int KT = ld / SQ_BK;
+    const int KT = n / SQ_BK;
 
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     const uint32_t full0 = smem_u32(&full_bar[0]);
@@ -109,31 +112,50 @@ sym_square_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
 #pragma unroll
             for (int ni = 0; ni < 4; ++ni) acc[mi][ni][0] = acc[mi][ni][1] = 0.0;
 
+        // Software pipeline over the flattened (kt, ks) sequence: the fragments of k4-step q+1 are loaded
+        // while the 32 DMMAs of step q issue, ACROSS stage boundaries too -- the full-barrier of stage
+        // kt+1 is waited for in the middle of stage kt, so no warp ever reaches a stage boundary with an
+        // empty DMMA queue (r01 profile: 5 % of the tensor pipe's cycles were lost exactly there).
+        auto load_frag = [&](double (&a)[8], double (&b)[4], uint32_t aB, uint32_t bB, const uint32_t (&o)[2]) {
+#pragma unroll
+            for (int mi = 0; mi < 8; ++mi) a[mi] = lds_f64(aB + (uint32_t)((mi >> 1) * 2048 + (mi & 1) * 128) + o[mi & 1]);
+#pragma unroll
+            for (int ni = 0; ni < 4; ++ni) b[ni] = lds_f64(bB + (uint32_t)((ni >> 1) * 2048 + (ni & 1) * 128) + o[ni & 1]);
+        };
+        auto mma_step = [&](const double (&a)[8], const double (&b)[4]) {
+#pragma unroll
+            for (int mi = 0; mi < 8; ++mi)
+#pragma unroll
+                for (int ni = 0; ni < 4; ++ni) dmma_8x8x4(acc[mi][ni][0], acc[mi][ni][1], a[mi], b[ni]);
+        };
+
         int s = 0;
         uint32_t ph = 0;
+        double a0[8], b0[4], a1[8], b1[4];
+        mbar_wait(full0, 0);
+        uint32_t st = smem_base;
+        load_frag(a0, b0, st + rowA, st + rowB, off[0]);
         for (int kt = 0; kt < KT; ++kt) {
             if (threadIdx.x == 0) issue_loads(min(KT, kt + SQ_STAGES));
             __syncwarp();
-            mbar_wait(full0 + 8 * s, ph);
-            const uint32_t st = smem_base + s * (2 * SQ_PANEL_BYTES);
             const uint32_t aB = st + rowA, bB = st + rowB;
-#pragma unroll
-            for (int ks = 0; ks < 4; ++ks) {
-                double a[8], b[4];
-#pragma unroll
-                for (int mi = 0; mi < 8; ++mi)
-                    a[mi] = lds_f64(aB + (uint32_t)((mi >> 1) * 2048 + (mi & 1) * 128) + off[ks][mi & 1]);
-#pragma unroll
-                for (int ni = 0; ni < 4; ++ni)
-                    b[ni] = lds_f64(bB + (uint32_t)((ni >> 1) * 2048 + (ni & 1) * 128) + off[ks][ni & 1]);
-#pragma unroll
-                for (int mi = 0; mi < 8; ++mi)
-#pragma unroll
-                    for (int ni = 0; ni < 4; ++ni) dmma_8x8x4(acc[mi][ni][0], acc[mi][ni][1], a[mi], b[ni]);
-            }
+            int s1 = s + 1;
+            uint32_t ph1 = ph;
+            if (s1 == SQ_STAGES) { s1 = 0; ph1 ^= 1u; }
+            const uint32_t stn = smem_base + s1 * (2 * SQ_PANEL_BYTES);
+            load_frag(a1, b1, aB, bB, off[1]);
+            mma_step(a0, b0);
+            load_frag(a0, b0, aB, bB, off[2]);
+            mma_step(a1, b1);
+            load_frag(a1, b1, aB, bB, off[3]);
+            if (kt + 1 < KT) mbar_wait(full0 + 8 * s1, ph1);
+            mma_step(a0, b0);
+            // first fragments of the next stage (after the last stage this reads stale smem; unused)
+            load_frag(a0, b0, stn + rowA, stn + rowB, off[0]);
+            mma_step(a1, b1);
             __syncwarp();
             if (lane == 0) mbar_arrive(empty0 + 8 * s);
-            if (++s == SQ_STAGES) { s = 0; ph ^= 1u; }
+            s = s1; ph = ph1; st = stn;
         }
 
         // ===== fused epilogue =====
