@@ -174,6 +174,22 @@ def run_reference(args) -> int:
 
 
 # ------------------------------------------------------------------------------------------ our arm
+def whole_job_rate(ms_local: float, flops_per_rank: float, device="cpu"):
+    """Replicas-only aggregation (DESIGN.md section 9): every rank did `flops_per_rank` of independent work;
+    the job's time is the MAX over ranks of the device-timed region, the job's work is the SUM.
+    Returns (ms_max, TFLOP/s of the whole job).  Works on any backend (gloo on CPU in the tests)."""
+    import torch
+    import torch.distributed as dist
+
+    ms = torch.tensor([ms_local], dtype=torch.float64, device=device)
+    fl = torch.tensor([flops_per_rank], dtype=torch.float64, device=device)
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(ms, op=dist.ReduceOp.MAX)
+        dist.all_reduce(fl, op=dist.ReduceOp.SUM)
+    ms_max = float(ms.item())
+    return ms_max, float(fl.item()) / (ms_max * 1e-3) / 1e12
+
+
 def run_ours(args) -> int:
     import torch
     import torch.distributed as dist
@@ -227,16 +243,13 @@ def run_ours(args) -> int:
     ev1.record(stream)
     barrier()
     clocks = sampler.stop()
-    ms = torch.tensor([ev0.elapsed_time(ev1)], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(ms, op=dist.ReduceOp.MAX)
-    ms_total = float(ms.item())
+    ms_local = ev0.elapsed_time(ev1)
     if not (res.converged and abs(float(torch.diagonal(P).sum().item()) - nocc) < 1e-6):
         raise SystemExit(f"bench.py: expansion did not converge to a projector (status {res.status})")
     iters = res.iterations
     fl_sq = executed_flops_per_squaring(k)
     fl_step = iters * fl_sq
-    value = world * args.steps * fl_step / (ms_total * 1e-3) / 1e12
+    ms_total, value = whole_job_rate(ms_local, args.steps * fl_step, dev)
 
     # ---- end-to-end arm: host buffers through rfoe_expand_host (H2D of H^p and D2H of P inside the timed region)
     Hh = torch.empty((k, k), dtype=torch.float64, pin_memory=True)
@@ -251,10 +264,7 @@ def run_ours(args) -> int:
         launches_e2e = r2.gpu_launches
     e1.record(stream)
     barrier()
-    ms2 = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(ms2, op=dist.ReduceOp.MAX)
-    e2e_value = world * args.steps * r2.iterations * fl_sq / (float(ms2.item()) * 1e-3) / 1e12
+    ms2, e2e_value = whole_job_rate(e0.elapsed_time(e1), args.steps * r2.iterations * fl_sq, dev)
     assert abs(float(Ph.diagonal().sum()) - nocc) < 1e-6
 
     if rank == 0:
@@ -278,7 +288,7 @@ def run_ours(args) -> int:
                          "flops_per_launch": fl_sq,
                          "peak_source": "derived: 148 SM x 64 DFMA/clk x 2 x 1.965 GHz (no FP64 entry in MEASURED_PEAKS.json)"},
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 8 * k * k, "d2h_bytes_per_step": 8 * k * k,
-                    "ms_per_step": float(ms2.item()) / args.steps},
+                    "ms_per_step": ms2 / args.steps},
             "gpu_launches": launches,
             "clocks": {"sm_mhz": clocks["sm_mhz"], "sm_max_mhz": clocks["sm_max_mhz"], "reasons": clocks["reasons"],
                        "power_w_max": clocks["power_w_max"], "samples": clocks["samples"]},
