@@ -180,3 +180,19 @@ def expand(H, nocc: int, *, variant: int = SP2, tol: float = 1e-12, stop_rule: i
         fp32_steps=run.fp32_steps, converged=bool(run.converged), branch=run.branch.decode()[:n],
         emin=run.emin, emax=run.emax, tr_PH=run.tr_PH,
         t=np.array(run.t[: n + 1]), s=np.array(run.s[: n + 1]), e=np.array(run.e[:n]), reltr=np.array(run.reltr[:n]))
+
+
+def square_entries(X, pairs):
+    """(X X)_ij for a list of (i, j), each by the definition Y_ij = sum_l X_il X_lj with l ascending, one
+    IEEE product and one IEEE sum at a time (pure-Python loop over Python floats).  Used where the full
+    naive product is out of reach (k >= 8192): sampled outputs computed one by one."""
+    X = np.asarray(X)
+    out = []
+    for i, j in pairs:
+        row = X[i, :].tolist()
+        col = X[:, j].tolist()
+        acc = 0.0
+        for a, b in zip(row, col):
+            acc = acc + a * b
+        out.append(acc)
+    return np.array(out)

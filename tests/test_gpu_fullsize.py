@@ -1,0 +1,112 @@
+"""GPU parity at BASELINE.json's full sizes, in the configuration bench.py times (rfoe_expand, SP2, rule A,
+Gershgorin bounds).  The naive oracle cannot run a whole expansion here (2 k^3 x 56 steps), so:
+  * the O(k^2) oracle steps run in full: Gershgorin bounds, affine map, Tr X0, ||X0||_F^2 (A1, A2);
+  * one squaring (A4 + A5) is checked on sampled outputs the oracle computes one by one (definition,
+    l ascending) in every tile class: diagonal tiles, off-diagonal tiles, mirrored entries, last tile;
+  * the whole expansion is checked through properties that hold at any size: the construction-exact
+    projector Q_occ Q_occ^T (pin P2), tr P = nocc, idempotency, bitwise symmetry, band energy =
+    sum of the occupied eigenvalues, and the scalar eigenvalue-space model (pin P5) for the iteration
+    count and the branch string.
+torch is used for the harness-side algebra only (building Q_occ Q_occ^T, norms)."""
+import math
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+import rfoe_inputs
+from tests import pins
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+import paper_2301_04642_b200 as rfoe  # noqa: E402
+
+EPS = 2.0 ** -52
+
+
+def _sample_pairs(k, rng, n_each=6):
+    m = (k + 127) // 128
+    pairs = []
+    for _ in range(n_each):
+        I, J = sorted(rng.integers(0, m, size=2).tolist())
+        i = min(k - 1, I * 128 + int(rng.integers(0, 128)))
+        j = min(k - 1, J * 128 + int(rng.integers(0, 128)))
+        pairs += [(i, j), (j, i)]                       # an entry and its mirror
+        d = min(k - 1, I * 128 + int(rng.integers(0, 128)))
+        pairs += [(d, d), (d, min(k - 1, d + 1))]       # inside a diagonal tile
+    pairs += [(0, 0), (k - 1, k - 1), (0, k - 1), (k - 1, 0), (k - 2, k - 1)]
+    return pairs
+
+
+def _run_fullsize(c):
+    w = rfoe_inputs.make_workload(c, device="cuda")
+    k, nocc = w.k, w.nocc
+    H = w.H
+    Hn = H.cpu().numpy()
+    with rfoe.Rfoe(k) as h:
+        # ---- A1/A2 against the full oracle (O(k^2))
+        lo, hi = h.bounds(H)
+        olo, ohi = oracle.bounds(Hn)
+        assert abs(lo - olo) <= 4 * k * EPS * abs(olo) and abs(hi - ohi) <= 4 * k * EPS * abs(ohi)
+        X0 = oracle.affine(Hn, olo, ohi)
+        t0, s0 = oracle.trace(X0), oracle.sumsq(X0)
+        # ---- A4/A5: one squaring of X0 at full size, sampled entries by the definition
+        Xd = torch.from_numpy(X0).cuda()
+        out, sc, ms = h.square(Xd, -1.0, 2.0, 0.0)                                     # the L branch: 2X - X^2
+        del Xd
+        pairs = _sample_pairs(k, np.random.default_rng(c))
+        y = oracle.square_entries(X0, pairs)
+        got = np.array([out[i, j].item() for i, j in pairs])
+        x = np.array([X0[i, j] for i, j in pairs])
+        xmax = float(np.abs(X0).max())
+        assert np.abs(got - (2.0 * x - y)).max() <= 8 * k * EPS * xmax * xmax + 4 * EPS * np.abs(x).max()
+        assert torch.equal(out, out.T)
+        assert sc[3] == pytest.approx(s0, rel=1e-12)                                   # Tr X^2 = ||X||_F^2
+        assert sc[0] == pytest.approx(2.0 * t0 - s0, rel=1e-12)
+        del out
+        # ---- the expansion bench.py times
+        res = h.expand(H, nocc, rfoe.SP2, w.tol)
+    assert res.status == rfoe.OK and res.converged
+    assert res.t[0] == pytest.approx(t0, rel=1e-13) and res.s[0] == pytest.approx(s0, rel=1e-12)
+    model = pins.scalar_sp2(w.lam, nocc, res.eps_min, res.eps_max, tol=w.tol)
+    assert res.iterations == model["iterations"]
+    decided = np.abs(model["t"][: res.iterations] - nocc) > 1e-9 * k / 256
+    assert all(a == b for a, b, d in zip(res.branch, model["branch"], decided) if d), (res.branch, model["branch"])
+    assert np.allclose(res.t, model["t"], rtol=0, atol=1e-8 * k / 256)
+    P = res.P
+    assert torch.equal(P, P.T)
+    assert abs(torch.diagonal(P).sum().item() - nocc) <= 1e-8
+    Qo = w.Q[:, :nocc]
+    Pex = Qo @ Qo.T
+    dP = torch.linalg.norm(P - Pex).item() / math.sqrt(k)
+    del Pex, Qo
+    assert dP <= 1e-10, dP
+    idem = torch.linalg.norm(P @ P - P).item()
+    assert idem <= 1e-10 * k / 256, idem
+    comm = torch.linalg.norm(H @ P - P @ H).item()
+    assert comm <= 1e-10 * k / 256, comm
+    assert abs(res.tr_PH - w.band_energy()) / abs(w.band_energy()) <= 1e-11
+    return dict(k=k, iterations=res.iterations, dP=dP, idem=idem, comm=comm, device_ms=res.device_ms,
+                square_ms=res.square_ms, branch=res.branch)
+
+
+def test_fullsize_config3():
+    r = _run_fullsize(3)
+    print(r)
+
+
+def test_fullsize_config4_headline():
+    r = _run_fullsize(4)
+    assert r["iterations"] == 56
+    print(r)
+
+
+@pytest.mark.slow
+def test_fullsize_config5():
+    r = _run_fullsize(5)
+    print(r)
+    os.makedirs("gpurun_out", exist_ok=True)
+    with open("gpurun_out/config5.txt", "w") as f:
+        f.write(repr(r) + "\n")
