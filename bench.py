@@ -40,8 +40,8 @@ TILE = 128
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 
 # dram__bytes_read.sum + dram__bytes_write.sum of one sym_square_kernel launch at k=16384, from the
-# `ncu --set full` capture summarised in profiles/ (None until that capture exists for the workload).
-NCU_TRAFFIC_BYTES = {}
+# `ncu --set full` capture summarised in profiles/ (None for sizes without a capture).
+NCU_TRAFFIC_BYTES = {16384: 34.673915e9 + 2.129676e9}   # profiles/r01b_sym_square_k16384.md
 
 
 def executed_flops_per_squaring(k: int) -> float:

@@ -79,13 +79,30 @@ affine_map_kernel(const double* __restrict__ H, int k, int n, int ld, const doub
         const double* row = H + (size_t)i * k;
         double ss = 0.0;
         if (vec) {
-            for (int j = lane * 2; j < k; j += 64) {
-                const double2 h = *reinterpret_cast<const double2*>(row + j);
-                double2 x;
+            // four independent 16-byte loads in flight per lane (512-byte runs per warp instruction)
+            auto map2 = [&](double2 h, int j, double2& x) {
                 x.x = ((j == i) ? (emax - h.x) : (-h.x)) / w;
                 x.y = ((j + 1 == i) ? (emax - h.y) : (-h.y)) / w;
                 ss = fma(x.x, x.x, ss);
                 ss = fma(x.y, x.y, ss);
+            };
+            int j = lane * 2;
+            for (; j + 192 < k; j += 256) {
+                const double2 h0 = *reinterpret_cast<const double2*>(row + j);
+                const double2 h1 = *reinterpret_cast<const double2*>(row + j + 64);
+                const double2 h2 = *reinterpret_cast<const double2*>(row + j + 128);
+                const double2 h3 = *reinterpret_cast<const double2*>(row + j + 192);
+                double2 x0, x1, x2, x3;
+                map2(h0, j, x0); map2(h1, j + 64, x1); map2(h2, j + 128, x2); map2(h3, j + 192, x3);
+                *reinterpret_cast<double2*>(xrow + j) = x0;
+                *reinterpret_cast<double2*>(xrow + j + 64) = x1;
+                *reinterpret_cast<double2*>(xrow + j + 128) = x2;
+                *reinterpret_cast<double2*>(xrow + j + 192) = x3;
+            }
+            for (; j < k; j += 64) {
+                const double2 h = *reinterpret_cast<const double2*>(row + j);
+                double2 x;
+                map2(h, j, x);
                 *reinterpret_cast<double2*>(xrow + j) = x;
             }
         } else {
@@ -160,27 +177,30 @@ copy_out_kernel(const double* __restrict__ W, int k, int ld, const double* __res
     }
 }
 
-// Bitwise symmetry check of a k x k matrix: 32 x 32 tiles of the upper triangle, both tiles read
-// row-contiguously and compared through shared memory.  *flag is set to 1 on any mismatch.
+// Bitwise symmetry check of a k x k matrix: 64 x 64 tiles of the upper triangle, both tiles read
+// row-contiguously (512-byte runs) and compared through shared memory.  *flag is set to 1 on any mismatch.
+constexpr int SYM_T = 64;
 __global__ void __launch_bounds__(256)
 symmetry_check_kernel(const double* __restrict__ H, int k, int* __restrict__ flag)
 {
-    __shared__ unsigned long long ta[32][33];
-    const int nt = (k + 31) / 32;
+    __shared__ unsigned long long ta[SYM_T][SYM_T + 1];
+    const int nt = (k + SYM_T - 1) / SYM_T;
     const unsigned long long* Hb = reinterpret_cast<const unsigned long long*>(H);
-    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    const int tx = threadIdx.x & (SYM_T - 1), ty = threadIdx.x / SYM_T;   // 64 x 4
     for (long long t = blockIdx.x; t < (long long)nt * nt; t += gridDim.x) {
         const int bi = (int)(t / nt), bj = (int)(t % nt);
         if (bj < bi) continue;
         __syncthreads();
-        for (int y = ty; y < 32; y += 8) {
-            const int i = bi * 32 + y, j = bj * 32 + tx;
+#pragma unroll 4
+        for (int y = ty; y < SYM_T; y += 4) {
+            const int i = bi * SYM_T + y, j = bj * SYM_T + tx;
             ta[y][tx] = (i < k && j < k) ? Hb[(size_t)i * k + j] : 0ull;
         }
         __syncthreads();
         int bad = 0;
-        for (int y = ty; y < 32; y += 8) {
-            const int i = bj * 32 + y, j = bi * 32 + tx;   // element (i, j) of the mirrored tile
+#pragma unroll 4
+        for (int y = ty; y < SYM_T; y += 4) {
+            const int i = bj * SYM_T + y, j = bi * SYM_T + tx;   // element (i, j) of the mirrored tile
             if (i < k && j < k) bad |= (Hb[(size_t)i * k + j] != ta[tx][y]);
         }
         if (bad) atomicExch(flag, 1);

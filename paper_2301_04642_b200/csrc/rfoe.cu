@@ -346,8 +346,8 @@ extern "C" int rfoe_expand(rfoe_handle_t h, const double* Hp, int64_t k64, int64
     h->hp->sym_flag = 0;
     if (h->check_sym) {
         CK(cudaMemsetAsync(h->d_flag, 0, sizeof(int), st));
-        const int nt32 = (k + 31) / 32;
-        long long blocks = (long long)nt32 * nt32;
+        const int nts = (k + SYM_T - 1) / SYM_T;
+        long long blocks = (long long)nts * nts;
         if (blocks > h->sm_count * 16) blocks = h->sm_count * 16;
         symmetry_check_kernel<<<(int)blocks, 256, 0, st>>>(Hp, k, h->d_flag);
         h->launches++;
