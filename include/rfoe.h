@@ -45,8 +45,8 @@ typedef enum {
  *  SP2        Z-RFOE with second-order projection polynomials           PAPER.md:35-39 (sec. II.B.1)
  *  MCWEENY    SP2 until (Tr X - Tr X^2) < 3/16 and |Tr X - N_occ| < 1/2, then X <- 3X^2 - 2X^3
  *             (purification, cited only: PAPER.md:23; reading R11 in DESIGN.md)
- *  SP2_MIXED  FP32 squarings far from convergence, FP64 afterwards, switch tied to RelTr
- *                                                                       PAPER.md:66, 92
+ *  SP2_MIXED  reduced-precision (3xTF32, FP32 accumulate) squarings far from convergence, FP64 afterwards,
+ *             switch tied to RelTr; optional FP64 head (RFOE_OPT_MIXED_HEAD)
  *  SP2_ACCEL  A-Z-RFOE: shifted-and-scaled SP2 polynomials from HOMO/LUMO estimates
  *                                                                       PAPER.md:43 (sec. II.B.2)
  * T-RFOE (Eq. 2) is SP2 with RFOE_OPT_MAX_ITER = m and tol = 0: the truncated
@@ -97,7 +97,7 @@ typedef struct {
 
 /* Create a handle on CUDA device `device` able to expand matrices up to k_max x k_max.
  * Allocates (device) three zero-padded work matrices of ceil(k_max/128)*128 squared doubles (the third
- * lazily, on the first McWeeny or mixed call), per-tile reduction scratch and one pinned host page.
+ * lazily, on the first McWeeny call; two FP32 matrices lazily on the first mixed call), per-tile reduction scratch and one pinned host page.
  * Errors: INVALID_ARG (h null, k_max < 1), CUDA (no device / wrong device), UNSUPPORTED (not sm_100),
  * ALLOC. */
 int rfoe_create(rfoe_handle_t* h, int device, int64_t k_max);
@@ -128,6 +128,13 @@ int rfoe_expand_host(rfoe_handle_t h, const double* Hp_host, int64_t k, int64_t 
  * kernel_ms (HOST, may be null): CUDA-event time of the squaring kernel alone (padding copies excluded). */
 int rfoe_square(rfoe_handle_t h, const double* X, int64_t k, double c2, double c1, double c0, double* Xout,
                 double* scalars, float* kernel_ms, rfoe_stream_t stream);
+
+/* The same step with the reduced-precision product of the mixed variant: X is split into
+ * tf32 parts X = Xh + Xl and X X is taken as Xh Xh + Xh Xl + Xl Xh on the tcgen05 tensor cores with FP32
+ * accumulation (about FP32 accuracy); the update, mirror and the five scalars are FP64 as in rfoe_square.
+ * kernel_ms covers the split pass and the product kernel. */
+int rfoe_square_reduced(rfoe_handle_t h, const double* X, int64_t k, double c2, double c1, double c0, double* Xout,
+                        double* scalars, float* kernel_ms, rfoe_stream_t stream);
 
 /* Symmetric product for commuting symmetric A, B (k x k, device): Cout = c2 * (A B) + c1 * A + c0 * I, upper
  * triangle computed and mirrored (the McWeeny step uses it with A = X^2, B = X).  scalars as in rfoe_square

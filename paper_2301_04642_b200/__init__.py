@@ -30,7 +30,8 @@ MAX_STEPS = 256
 OK, ERR_INVALID_ARG, ERR_ALLOC, ERR_CUDA, ERR_BAD_BOUNDS, ERR_NOT_SYMMETRIC, ERR_UNSUPPORTED, ERR_NOT_CONVERGED = range(8)
 
 # every symbol include/rfoe.h declares
-EXPORTS = ("rfoe_create", "rfoe_bounds", "rfoe_expand", "rfoe_expand_host", "rfoe_square", "rfoe_symm_product",
+EXPORTS = ("rfoe_create", "rfoe_bounds", "rfoe_expand", "rfoe_expand_host", "rfoe_square", "rfoe_square_reduced",
+           "rfoe_symm_product",
            "rfoe_set_option", "rfoe_get_stats", "rfoe_destroy", "rfoe_strerror", "rfoe_version")
 
 
@@ -75,6 +76,7 @@ def load_library(path: str | None = None):
     L.rfoe_expand.argtypes = [vp, vp, i64, i64, C.c_int, dbl, vp, vp]
     L.rfoe_expand_host.argtypes = [vp, vp, i64, i64, C.c_int, dbl, vp, vp]
     L.rfoe_square.argtypes = [vp, vp, i64, dbl, dbl, dbl, vp, dp, C.POINTER(C.c_float), vp]
+    L.rfoe_square_reduced.argtypes = [vp, vp, i64, dbl, dbl, dbl, vp, dp, C.POINTER(C.c_float), vp]
     L.rfoe_symm_product.argtypes = [vp, vp, vp, i64, dbl, dbl, dbl, vp, dp, C.POINTER(C.c_float), vp]
     L.rfoe_set_option.argtypes = [vp, C.c_int, dbl]
     L.rfoe_get_stats.argtypes = [vp, C.POINTER(_Stats)]
@@ -142,9 +144,10 @@ class Rfoe:
             raise RfoeError(rc, self._L.rfoe_strerror(rc).decode())
 
     def close(self):
-        if getattr(self, "_h", None) and self._h.value:
-            self._L.rfoe_destroy(self._h)
-            self._h = C.c_void_p()
+        h = getattr(self, "_h", None)
+        if h is not None and h.value:
+            self._h = None
+            self._L.rfoe_destroy(h)
 
     __del__ = close
 
@@ -229,15 +232,16 @@ class Rfoe:
             self._raise(rc)
         return self._result(P, rc)
 
-    def square(self, X, c2=1.0, c1=0.0, c0=0.0, out=None, stream=None):
-        """out = c2 X X + c1 X + c0 I; returns (out, scalars[5], kernel_ms)."""
+    def square(self, X, c2=1.0, c1=0.0, c0=0.0, out=None, stream=None, reduced=False):
+        """out = c2 X X + c1 X + c0 I; returns (out, scalars[5], kernel_ms).  reduced=True: rfoe_square_reduced."""
         import torch
 
         _check_dev(X, "X")
         out = torch.empty_like(X) if out is None else out
         sc = (C.c_double * 5)()
         ms = C.c_float()
-        rc = self._L.rfoe_square(self._h, C.c_void_p(X.data_ptr()), X.shape[0], c2, c1, c0, C.c_void_p(out.data_ptr()),
+        fn = self._L.rfoe_square_reduced if reduced else self._L.rfoe_square
+        rc = fn(self._h, C.c_void_p(X.data_ptr()), X.shape[0], c2, c1, c0, C.c_void_p(out.data_ptr()),
                                  sc, C.byref(ms), _stream_ptr(stream))
         if rc != OK:
             self._raise(rc)

@@ -178,6 +178,15 @@ sum_rows_kernel(const double* __restrict__ rows, int n, double* __restrict__ dst
     if (threadIdx.x == 0) *dst = v;
 }
 
+// Tr X of a pitched work matrix (rfoe_square_reduced needs it for the shift)
+__global__ void __launch_bounds__(256)
+diag_sum_kernel(const double* __restrict__ X, int k, int ld, double* __restrict__ dst)
+{
+    __shared__ double sh[256];
+    const double v = block_sum_strided(X, k, ld + 1, sh);
+    if (threadIdx.x == 0) *dst = v;
+}
+
 // 5 scalars of one squaring launch (rfoe_square / rfoe_symm_product)
 __global__ void __launch_bounds__(256)
 sum_partials_kernel(const double* __restrict__ part, int n_rec, double* __restrict__ dst5)

@@ -14,6 +14,7 @@
 #include "control.cuh"
 #include "hbm_kernels.cuh"
 #include "sym_square.cuh"
+#include "sym_square_tf32.cuh"
 
 using namespace rfoe;
 
@@ -37,6 +38,7 @@ struct rfoe_handle_s {
     int64_t k_max = 0;
     int ld_max = 0;
     double* W[3] = {nullptr, nullptr, nullptr};
+    float* F[2] = {nullptr, nullptr};   // tf32 hi / lo copies of X_n for the reduced-precision squaring (lazy)
     double* part[2] = {nullptr, nullptr};
     double* rows[2] = {nullptr, nullptr};
     double* d_bounds = nullptr;
@@ -121,6 +123,43 @@ static int make_map(rfoe_handle_s* h, CUtensorMap* map, double* base, int n, int
     return RFOE_OK;
 }
 
+static int make_map32(rfoe_handle_s* h, CUtensorMap* map, float* base, int n, int ld32)
+{
+    cuuint64_t dims[2] = {(cuuint64_t)n, (cuuint64_t)n};
+    cuuint64_t strides[1] = {(cuuint64_t)ld32 * sizeof(float)};
+    cuuint32_t box[2] = {(cuuint32_t)TQ_BK, (cuuint32_t)TQ_BM};
+    cuuint32_t estr[2] = {1, 1};
+    CUresult r = h->encode(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, base, dims, strides, box, estr,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        h->stats.cuda_error = (int)cudaErrorInvalidValue;
+        return RFOE_ERR_CUDA;
+    }
+    return RFOE_OK;
+}
+
+static int ensure_tf32(rfoe_handle_s* h)
+{
+    const size_t ld = (size_t)h->ld_max;
+    for (float*& p : h->F)
+        if (!p && cudaMalloc(&p, ld * (ld + TQ_PAD) * sizeof(float)) != cudaSuccess) { cudaGetLastError(); return RFOE_ERR_ALLOC; }
+    return RFOE_OK;
+}
+
+// reduced-precision step: split X (FP64, in Xin) into tf32 hi / lo, then the tcgen05 squaring with the FP64 epilogue
+static cudaError_t launch_square_tf32(rfoe_handle_s* h, const CUtensorMap& hi, const CUtensorMap& lo, const double* Xin,
+                                      double* Out, int n, int ld, int k, const double* trace, const StepCoef* coef,
+                                      double* partials, cudaStream_t st)
+{
+    split_tf32_kernel<<<hbm_grid(h, n), 256, 0, st>>>(Xin, n, ld, k, trace, h->F[0], h->F[1], n + TQ_PAD);
+    h->launches++;
+    sym_square_tf32_kernel<<<h->n_tiles, TQ_THREADS, TQ_SMEM_BYTES, st>>>(hi, lo, Xin, Out, n, ld, k, trace, coef, h->d_tiles,
+                                                                         partials);
+    h->launches++;
+    return cudaGetLastError();
+}
+
 template <bool TWO_OP>
 static cudaError_t launch_square(rfoe_handle_s* h, const CUtensorMap& a, const CUtensorMap& b, const double* E, double* Out,
                                  int n, int ld, int k, const StepCoef* coef, double* partials, cudaStream_t st)
@@ -166,6 +205,7 @@ extern "C" int rfoe_destroy(rfoe_handle_t h)
     if (!h) return RFOE_OK;
     cudaSetDevice(h->device);
     for (double* p : h->W) cudaFree(p);
+    for (float* p : h->F) cudaFree(p);
     for (double* p : h->part) cudaFree(p);
     for (double* p : h->rows) cudaFree(p);
     cudaFree(h->d_bounds); cudaFree(h->d_scalars); cudaFree(h->d_flag); cudaFree(h->d_ctrl); cudaFree(h->d_tiles);
@@ -223,7 +263,8 @@ extern "C" int rfoe_create(rfoe_handle_t* out, int device, int64_t k_max)
     }
     h->encode = (EncodeTiledFn)fn;
     if (cudaFuncSetAttribute(sym_square_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SQ_SMEM_BYTES) != cudaSuccess ||
-        cudaFuncSetAttribute(sym_square_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SQ_SMEM_BYTES) != cudaSuccess) {
+        cudaFuncSetAttribute(sym_square_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SQ_SMEM_BYTES) != cudaSuccess ||
+        cudaFuncSetAttribute(sym_square_tf32_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TQ_SMEM_BYTES) != cudaSuccess) {
         rfoe_destroy(h);
         return RFOE_ERR_CUDA;
     }
@@ -325,7 +366,6 @@ extern "C" int rfoe_expand(rfoe_handle_t h, const double* Hp, int64_t k64, int64
         if (a < b + bytes && b < a + bytes) return fail(RFOE_ERR_INVALID_ARG);
     }
     if (variant < RFOE_VARIANT_SP2 || variant > RFOE_VARIANT_SP2_ACCEL) return fail(RFOE_ERR_UNSUPPORTED);
-    if (variant == RFOE_VARIANT_SP2_MIXED) return fail(RFOE_ERR_UNSUPPORTED);   // FP32 path: see DESIGN.md (row A8)
     if (variant == RFOE_VARIANT_SP2_ACCEL && !(isfinite(h->homo) && isfinite(h->lumo) && h->lumo > h->homo))
         return fail(RFOE_ERR_INVALID_ARG);
     const int k = (int)k64;
@@ -336,10 +376,15 @@ extern "C" int rfoe_expand(rfoe_handle_t h, const double* Hp, int64_t k64, int64
     h->launches = 0;
     CK(cudaSetDevice(h->device));
     if (variant == RFOE_VARIANT_MCWEENY && (rc = ensure_third(h)) != RFOE_OK) return fail(rc);
+    if (variant == RFOE_VARIANT_SP2_MIXED && (rc = ensure_tf32(h)) != RFOE_OK) return fail(rc);
     if ((rc = ensure_tiles(h, m, st)) != RFOE_OK) return fail(rc);
     CUtensorMap tm[3];
     for (int i = 0; i < 3; ++i)
         if (h->W[i] && (rc = make_map(h, &tm[i], h->W[i], n, ld)) != RFOE_OK) return fail(rc);
+    CUtensorMap tmF[2];
+    if (variant == RFOE_VARIANT_SP2_MIXED)
+        for (int i = 0; i < 2; ++i)
+            if ((rc = make_map32(h, &tmF[i], h->F[i], n, n + TQ_PAD)) != RFOE_OK) return fail(rc);
 
     CK(cudaEventRecord(h->ev0, st));
     // --- symmetry check, bounds, affine map, first decision -------------------------------------
@@ -403,6 +448,12 @@ extern "C" int rfoe_expand(rfoe_handle_t h, const double* Hp, int64_t k64, int64
         if (action == ACT_SP2) {
             CK(timed_square<false>(h, tm[cur], tm[cur], h->W[cur], h->W[nxt], n, ld, k, &h->d_ctrl->coef, h->part[0], st));
             control_kernel<<<1, 256, 0, st>>>(h->d_ctrl, 1, h->part[0], h->part[0], h->n_tiles, h->d_word);
+        } else if (action == ACT_SP2_FP32) {
+            CK(cudaEventRecord(h->sq_ev[2 * h->sq_n], st));
+            CK(launch_square_tf32(h, tmF[0], tmF[1], h->W[cur], h->W[nxt], n, ld, k, &h->d_ctrl->t, &h->d_ctrl->coef, h->part[0], st));
+            CK(cudaEventRecord(h->sq_ev[2 * h->sq_n + 1], st));
+            h->sq_n++;
+            control_kernel<<<1, 256, 0, st>>>(h->d_ctrl, 1, h->part[0], h->part[0], h->n_tiles, h->d_word);
         } else if (action == ACT_MCWEENY) {
             CK(timed_square<false>(h, tm[cur], tm[cur], h->W[cur], h->W[2], n, ld, k, &h->d_ctrl->coef, h->part[0], st));
             CK(timed_square<true>(h, tm[2], tm[cur], h->W[2], h->W[nxt], n, ld, k, &h->d_ctrl->coef_aux, h->part[1], st));
@@ -453,7 +504,7 @@ extern "C" int rfoe_expand(rfoe_handle_t h, const double* Hp, int64_t k64, int64
 // ---------------------------------------------------------------------------------------------
 // single products (kernel-level entry points for tests and roofline timing)
 static int single_product(rfoe_handle_s* h, const double* A, const double* B, int64_t k64, double c2, double c1, double c0,
-                          double* Cout, double* scalars, float* kernel_ms, cudaStream_t st)
+                          double* Cout, double* scalars, float* kernel_ms, cudaStream_t st, bool reduced = false)
 {
     if (!h || !A || !Cout || k64 < 1 || k64 > h->k_max) return RFOE_ERR_INVALID_ARG;
     const bool two = (B != nullptr);
@@ -464,9 +515,14 @@ static int single_product(rfoe_handle_s* h, const double* A, const double* B, in
     CK(cudaSetDevice(h->device));
     if ((rc = ensure_third(h)) != RFOE_OK) return rc;
     if ((rc = ensure_tiles(h, m, st)) != RFOE_OK) return rc;
-    CUtensorMap tm[3];
+    CUtensorMap tm[3], tmF[2];
     for (int i = 0; i < 3; ++i)
         if ((rc = make_map(h, &tm[i], h->W[i], n, ld)) != RFOE_OK) return rc;
+    if (reduced) {
+        if ((rc = ensure_tf32(h)) != RFOE_OK) return rc;
+        for (int i = 0; i < 2; ++i)
+            if ((rc = make_map32(h, &tmF[i], h->F[i], n, n + TQ_PAD)) != RFOE_OK) return rc;
+    }
     pad_copy_kernel<<<hbm_grid(h, n), HBM_THREADS, 0, st>>>(A, k, n, ld, h->W[0]);
     h->launches++;
     if (two) {
@@ -478,7 +534,12 @@ static int single_product(rfoe_handle_s* h, const double* A, const double* B, in
     C.coef = StepCoef{c2, c1, c0};
     CK(cudaMemcpyAsync(&h->d_ctrl->coef, &C.coef, sizeof(StepCoef), cudaMemcpyHostToDevice, st));
     CK(cudaEventRecord(h->ev0, st));
-    if (two) CK(launch_square<true>(h, tm[0], tm[1], h->W[0], h->W[2], n, ld, k, &h->d_ctrl->coef, h->part[0], st));
+    if (reduced) {
+        diag_sum_kernel<<<1, 256, 0, st>>>(h->W[0], k, ld, h->d_scalars + 7);      // Tr X for the shift d = Tr X / k
+        h->launches++;
+        CK(launch_square_tf32(h, tmF[0], tmF[1], h->W[0], h->W[2], n, ld, k, h->d_scalars + 7, &h->d_ctrl->coef, h->part[0], st));
+    }
+    else if (two) CK(launch_square<true>(h, tm[0], tm[1], h->W[0], h->W[2], n, ld, k, &h->d_ctrl->coef, h->part[0], st));
     else     CK(launch_square<false>(h, tm[0], tm[0], h->W[0], h->W[2], n, ld, k, &h->d_ctrl->coef, h->part[0], st));
     CK(cudaEventRecord(h->ev1, st));
     sum_partials_kernel<<<1, 256, 0, st>>>(h->part[0], h->n_tiles, h->d_scalars);
@@ -498,6 +559,12 @@ extern "C" int rfoe_square(rfoe_handle_t h, const double* X, int64_t k, double c
                            double* scalars, float* kernel_ms, rfoe_stream_t stream)
 {
     return single_product(h, X, nullptr, k, c2, c1, c0, Xout, scalars, kernel_ms, (cudaStream_t)stream);
+}
+
+extern "C" int rfoe_square_reduced(rfoe_handle_t h, const double* X, int64_t k, double c2, double c1, double c0, double* Xout,
+                                   double* scalars, float* kernel_ms, rfoe_stream_t stream)
+{
+    return single_product(h, X, nullptr, k, c2, c1, c0, Xout, scalars, kernel_ms, (cudaStream_t)stream, true);
 }
 
 extern "C" int rfoe_symm_product(rfoe_handle_t h, const double* A, const double* B, int64_t k, double c2, double c1, double c0,

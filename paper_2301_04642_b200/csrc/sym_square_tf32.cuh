@@ -1,0 +1,269 @@
+// Reduced-precision symmetric squaring on the 5th-generation tensor cores (row A8 of DESIGN.md):
+// the paper's mixed-precision RFOE runs the squarings far from convergence in FP32.
+// Here an "FP32 step" is a 3xTF32 product: X = Xh + Xl with Xh = tf32(X), Xl = tf32(X - Xh), and
+//     C = Xh Xh^T  +  (Xh Xl^T + Xl Xh^T)          (Xl Xl^T, 2^-22 relative, is dropped)
+// computed by tcgen05.mma.kind::tf32 with TWO FP32 accumulators in tensor memory (the exact-product
+// head term and the small cross terms are accumulated separately and added in FP64 in the epilogue).
+// Two measures keep the tensor cores' FP32 accumulation (which TRUNCATES: measured, a systematic bias of
+// ~(k/8) 2^-24 on coherent sums such as the diagonal of X^2, enough to push eigenvalues past 1 and make SP2
+// diverge) at plain-FP32 accuracy:
+//   * shift: with d = Tr X / k the product is taken of Z = X - d I (zero-mean diagonal, small entries) and
+//     X^2 = Z^2 + 2 d X - d^2 I is completed exactly in FP64 in the epilogue;
+//   * chunking: the head term is accumulated in tensor memory over 256 k values only, then drained by the
+//     (otherwise idle) epilogue warps into FP32 register sums with round-to-nearest adds, double-buffered.
+// The master copy of X stays FP64: the epilogue is the same as the FP64 kernel's -- Out = c2 C + c1 X
+// + c0 I written to (I,J) and mirrored, five FP64 partial sums per tile -- so the recursion, its
+// scalars and its control flow are unchanged; only the product is reduced precision.
+//
+// Roles (192 threads): warp 0 = TMA producer, warp 1 = TMEM allocator + single-thread MMA issuer,
+// warps 2..5 = epilogue (each reads its own 32 TMEM lanes = 32 tile rows).
+#pragma once
+#include "ptx_sm100.cuh"
+#include "sym_square.cuh"
+
+namespace rfoe {
+
+constexpr int TQ_BM = 128;                 // tile rows = cols (UMMA M = N = 128, cta_group::1)
+constexpr int TQ_BK = 32;                  // floats per K chunk = one 128-byte swizzle row
+constexpr int TQ_UK = 8;                   // K of one tcgen05.mma.kind::tf32
+constexpr int TQ_STAGES = 3;
+constexpr int TQ_THREADS = 192;
+constexpr int TQ_PANEL_BYTES = TQ_BM * TQ_BK * 4;                 // 16 KiB
+constexpr int TQ_STAGE_BYTES = 4 * TQ_PANEL_BYTES;               // A_hi, A_lo, B_hi, B_lo
+constexpr int TQ_SMEM_BYTES = TQ_STAGES * TQ_STAGE_BYTES + 1024; // + slack for 1024-byte alignment
+constexpr int TQ_CHUNK_KT = 8;             // K chunks (of 32) per tensor-memory accumulation run: 256 k values
+constexpr int TQ_TMEM_COLS = 512;          // head accumulator x 2 (double-buffered) + cross-term accumulator
+constexpr int TQ_PAD = 32;                 // floats added to the row pitch of the hi / lo matrices
+
+// HBM-bound: split the FP64 work matrix (n x n, pitch ld) into tf32-rounded hi and lo FP32 matrices
+// (n x n, pitch ld32) of Z = X - d I, d = *trace / kvalid (rows >= kvalid stay zero).
+// hi = tf32(fl32(z)), lo = tf32(fl32(z - hi)) with z - hi exact in FP64.
+__global__ void __launch_bounds__(256)
+split_tf32_kernel(const double* __restrict__ X, int n, int ld, int kvalid, const double* __restrict__ trace,
+                  float* __restrict__ Hi, float* __restrict__ Lo, int ld32)
+{
+    const double d = *trace / (double)kvalid;
+    const int lane = threadIdx.x & 31;
+    const int wglobal = blockIdx.x * 8 + (threadIdx.x >> 5);
+    const int wtotal = gridDim.x * 8;
+    for (int i = wglobal; i < n; i += wtotal) {
+        const double2* row = reinterpret_cast<const double2*>(X + (size_t)i * ld);
+        float2* hrow = reinterpret_cast<float2*>(Hi + (size_t)i * ld32);
+        float2* lrow = reinterpret_cast<float2*>(Lo + (size_t)i * ld32);
+#pragma unroll 4
+        for (int j = lane; j < n / 2; j += 32) {
+            double2 x = row[j];
+            if (2 * j == i && i < kvalid) x.x -= d;
+            if (2 * j + 1 == i && i < kvalid) x.y -= d;
+            float2 h, l;
+            h.x = to_tf32((float)x.x);
+            h.y = to_tf32((float)x.y);
+            l.x = to_tf32((float)(x.x - (double)h.x));
+            l.y = to_tf32((float)(x.y - (double)h.y));
+            hrow[j] = h;
+            lrow[j] = l;
+        }
+    }
+}
+
+__global__ void __launch_bounds__(TQ_THREADS, 1)
+sym_square_tf32_kernel(const __grid_constant__ CUtensorMap tmHi, const __grid_constant__ CUtensorMap tmLo,
+                       const double* __restrict__ E, double* __restrict__ Out, int n, int ld, int kvalid,
+                       const double* __restrict__ trace, const StepCoef* __restrict__ coef,
+                       const int2* __restrict__ tile_map, double* __restrict__ partials)
+{
+    extern __shared__ uint8_t smem_raw[];
+    __shared__ __align__(8) uint64_t full_bar[TQ_STAGES];
+    __shared__ __align__(8) uint64_t empty_bar[TQ_STAGES];
+    __shared__ __align__(8) uint64_t hfull_bar[2];    // head accumulator b holds a finished chunk
+    __shared__ __align__(8) uint64_t hempty_bar[2];   // head accumulator b has been drained
+    __shared__ uint32_t tmem_base_sh;
+    __shared__ double red[4][5];
+
+    const int warp = threadIdx.x >> 5;
+    const int lane = threadIdx.x & 31;
+    const int2 tile = tile_map[blockIdx.x];
+    const int I = tile.x, J = tile.y;
+    const bool diag = (I == J);
+    const int KT = n / TQ_BK;
+
+    const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    const uint32_t full0 = smem_u32(&full_bar[0]);
+    const uint32_t empty0 = smem_u32(&empty_bar[0]);
+    const uint32_t hfull0 = smem_u32(&hfull_bar[0]);
+    const uint32_t hempty0 = smem_u32(&hempty_bar[0]);
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < TQ_STAGES; ++s) {
+            mbar_init(full0 + 8 * s, 1);
+            mbar_init(empty0 + 8 * s, 1);
+        }
+        for (int b = 0; b < 2; ++b) {
+            mbar_init(hfull0 + 8 * b, 1);
+            mbar_init(hempty0 + 8 * b, 4);     // lane 0 of each of the four epilogue warps
+        }
+        mbar_fence_init();
+        tma_prefetch_desc(&tmHi);
+        tma_prefetch_desc(&tmLo);
+    }
+    if (warp == 1) tmem_alloc<TQ_TMEM_COLS>(smem_u32(&tmem_base_sh));
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = tmem_base_sh;
+
+    if (warp == 0) {
+        // ===== TMA producer (one thread) =====
+        if (lane == 0) {
+            int s = 0;
+            uint32_t ph = 0;
+            const uint32_t bytes = diag ? 2 * TQ_PANEL_BYTES : 4 * TQ_PANEL_BYTES;
+            for (int kt = 0; kt < KT; ++kt) {
+                mbar_wait_bounded(empty0 + 8 * s, ph ^ 1u);
+                const uint32_t fb = full0 + 8 * s;
+                const uint32_t dst = smem_base + s * TQ_STAGE_BYTES;
+                mbar_expect_tx(fb, bytes);
+                tma_load_2d(dst, &tmHi, kt * TQ_BK, I * TQ_BM, fb);
+                tma_load_2d(dst + TQ_PANEL_BYTES, &tmLo, kt * TQ_BK, I * TQ_BM, fb);
+                if (!diag) {
+                    tma_load_2d(dst + 2 * TQ_PANEL_BYTES, &tmHi, kt * TQ_BK, J * TQ_BM, fb);
+                    tma_load_2d(dst + 3 * TQ_PANEL_BYTES, &tmLo, kt * TQ_BK, J * TQ_BM, fb);
+                }
+                if (++s == TQ_STAGES) { s = 0; ph ^= 1u; }
+            }
+        }
+    } else if (warp == 1) {
+        // ===== MMA issuer (one thread): 3 tcgen05.mma per 8-wide k step =====
+        if (lane == 0) {
+            constexpr uint32_t idesc = umma_idesc_tf32(TQ_BM, TQ_BM);
+            int s = 0;
+            uint32_t ph = 0;
+            for (int kt = 0; kt < KT; ++kt) {
+                const int kc = kt % TQ_CHUNK_KT;             // position inside the chunk
+                const int hb = (kt / TQ_CHUNK_KT) & 1;       // head accumulator of this chunk
+                if (kc == 0 && kt >= 2 * TQ_CHUNK_KT) {      // buffer reused: wait until its previous chunk is drained
+                    mbar_wait_bounded(hempty0 + 8 * hb, (uint32_t)((kt / (2 * TQ_CHUNK_KT)) - 1) & 1u);
+                    tc_fence_after();
+                }
+                mbar_wait_bounded(full0 + 8 * s, ph);
+                tc_fence_after();
+                const uint32_t a_hi = smem_base + s * TQ_STAGE_BYTES;
+                const uint32_t a_lo = a_hi + TQ_PANEL_BYTES;
+                const uint64_t dAh = umma_desc_k128(a_hi), dAl = umma_desc_k128(a_lo);
+                const uint64_t dBh = diag ? dAh : umma_desc_k128(a_hi + 2 * TQ_PANEL_BYTES);
+                const uint64_t dBl = diag ? dAl : umma_desc_k128(a_hi + 3 * TQ_PANEL_BYTES);
+                const uint32_t t_head = tmem + hb * TQ_BM, t_cross = tmem + 2 * TQ_BM;
+#pragma unroll
+                for (int ks = 0; ks < TQ_BK / TQ_UK; ++ks) {
+                    const uint64_t o = (uint64_t)(ks * TQ_UK * 4 >> 4);      // 32 bytes per k step, in 16-byte units
+                    umma_tf32(t_head, dAh + o, dBh + o, idesc, (kc | ks) != 0);   // head: Zh Zh^T (products exact in FP32)
+                    umma_tf32(t_cross, dAh + o, dBl + o, idesc, (kt | ks) != 0);  // cross terms: tiny, one long accumulation
+                    umma_tf32(t_cross, dAl + o, dBh + o, idesc, 1u);
+                }
+                umma_commit(empty0 + 8 * s);      // frees the stage when these MMAs have read it
+                if (kc == TQ_CHUNK_KT - 1 || kt == KT - 1) umma_commit(hfull0 + 8 * hb);   // chunk complete
+                if (++s == TQ_STAGES) { s = 0; ph ^= 1u; }
+            }
+        }
+    } else {
+        // ===== epilogue warps: TMEM -> registers -> fused FP64 update, mirror, partial sums =====
+        const int q = warp & 3;                   // TMEM lane quarter this warp may access
+        const int row = I * TQ_BM + q * 32 + lane;
+        const uint32_t trow = tmem + ((uint32_t)(q * 32) << 16);
+        // ---- drain the head accumulator chunk by chunk into FP32 register sums (round-to-nearest adds)
+        float hsum[TQ_BM];
+        const int NC = (KT + TQ_CHUNK_KT - 1) / TQ_CHUNK_KT;
+#pragma unroll 1
+        for (int ch = 0; ch < NC; ++ch) {
+            const int hb = ch & 1;
+            mbar_wait_bounded(hfull0 + 8 * hb, (uint32_t)(ch >> 1) & 1u);
+            tc_fence_after();
+#pragma unroll
+            for (int cb = 0; cb < TQ_BM; cb += 16) {
+                float v[16];
+                tmem_ld16(trow + hb * TQ_BM + cb, v);
+#pragma unroll
+                for (int u = 0; u < 16; ++u) hsum[cb + u] = (ch == 0) ? v[u] : __fadd_rn(hsum[cb + u], v[u]);
+            }
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(hempty0 + 8 * hb);
+        }
+        // ---- the last chunk's commit also covers every cross-term MMA: finish in FP64
+        const double d = *trace / (double)kvalid;
+        const double c2 = coef->c2, c1 = coef->c1, c0 = coef->c0;
+        double p_tr = 0.0, p_ss = 0.0, p_err = 0.0, p_trc = 0.0, p_ce = 0.0;
+        const double* erow = E + (size_t)row * ld + (size_t)J * TQ_BM;
+        double* orow = Out + (size_t)row * ld + (size_t)J * TQ_BM;
+#pragma unroll
+        for (int cb = 0; cb < TQ_BM; cb += 16) {
+            float xx[16];
+            tmem_ld16(trow + 2 * TQ_BM + cb, xx);
+            double ev[16], o[16];
+#pragma unroll
+            for (int u = 0; u < 16; u += 2) {
+                const double2 e2 = *reinterpret_cast<const double2*>(erow + cb + u);
+                ev[u] = e2.x; ev[u + 1] = e2.y;
+            }
+            const int col = J * TQ_BM + cb;
+#pragma unroll
+            for (int u = 0; u < 16; ++u) {
+                // X^2 = Z^2 + 2 d X - d^2 I   (Z = X - d I on rows < kvalid)
+                double cv = fma(2.0 * d, ev[u], (double)hsum[cb + u] + (double)xx[u]);
+                double v;
+                const double d0 = cv - ev[u];
+                double w = 1.0;                   // off-diagonal tiles: x2 applied once at the end
+                if (diag) {
+                    const int cc = col + u;
+                    w = (cc > row) ? 2.0 : ((cc == row) ? 1.0 : 0.0);
+                    if (cc == row && row < kvalid) cv -= d * d;
+                    v = fma(c2, cv, c1 * ev[u]);
+                    if (cc == row) {
+                        if (row < kvalid) v += c0;
+                        p_tr += v;
+                        p_trc += cv;
+                    }
+                } else {
+                    v = fma(c2, cv, c1 * ev[u]);
+                }
+                const double dd = diag ? (cv - ev[u]) : d0;
+                o[u] = v;
+                p_ss = fma(w * v, v, p_ss);
+                p_err = fma(w * dd, dd, p_err);
+                p_ce = fma(w * cv, ev[u], p_ce);
+            }
+            if (!diag) {
+#pragma unroll
+                for (int u = 0; u < 16; u += 2) *reinterpret_cast<double2*>(orow + cb + u) = make_double2(o[u], o[u + 1]);
+#pragma unroll
+                for (int u = 0; u < 16; ++u) Out[(size_t)(col + u) * ld + row] = o[u];   // mirror: lanes = consecutive rows
+            } else {
+#pragma unroll
+                for (int u = 0; u < 16; ++u) {
+                    if (col + u >= row) orow[cb + u] = o[u];
+                    if (col + u > row) Out[(size_t)(col + u) * ld + row] = o[u];
+                }
+            }
+        }
+        if (!diag) { p_ss *= 2.0; p_err *= 2.0; p_ce *= 2.0; }
+#pragma unroll
+        for (int m = 16; m >= 1; m >>= 1) {
+            p_tr += __shfl_xor_sync(0xffffffffu, p_tr, m);
+            p_ss += __shfl_xor_sync(0xffffffffu, p_ss, m);
+            p_err += __shfl_xor_sync(0xffffffffu, p_err, m);
+            p_trc += __shfl_xor_sync(0xffffffffu, p_trc, m);
+            p_ce += __shfl_xor_sync(0xffffffffu, p_ce, m);
+        }
+        if (lane == 0) {
+            red[q][0] = p_tr; red[q][1] = p_ss; red[q][2] = p_err; red[q][3] = p_trc; red[q][4] = p_ce;
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 1) tmem_dealloc<TQ_TMEM_COLS>(tmem);
+    if (threadIdx.x < 5)
+        partials[(size_t)blockIdx.x * SQ_NPART + threadIdx.x] =
+            (red[0][threadIdx.x] + red[1][threadIdx.x]) + (red[2][threadIdx.x] + red[3][threadIdx.x]);
+}
+
+}  // namespace rfoe

@@ -230,3 +230,63 @@ def test_error_paths(handle):
     # the handle is still usable after errors
     res = handle.expand(H, w.nocc, rfoe.SP2, w.tol)
     assert res.converged
+
+
+# ------------------------------------------------------------------ A8: reduced-precision path (reported separately)
+@pytest.mark.parametrize("k", [1, 5, 128, 130, 257, 777])
+def test_square_reduced_error_bound(handle, k):
+    """3xTF32 product with FP32 tensor-core accumulation against the FP64 oracle product.  Bound:
+    dropped Zl Zl term and tf32 rounding of Zl: 3 * 2^-22 per product; FP32 accumulation in tensor memory, one
+    truncation per 8-wide MMA block plus the in-block tree, over chunks of 256: (k/8 + 8) * 2^-23 bounds it,
+    all relative to sum_l |z_il||z_lj| with Z = X - (Tr X / k) I."""
+    X = _sym(k, 100 + k, scale=1.0 / math.sqrt(k))
+    out, sc, ms = handle.square(_dev(X), -1.0, 2.0, 0.0, reduced=True)
+    out = out.cpu().numpy()
+    Y = oracle.square(X)
+    Z = X - np.trace(X) / k * np.eye(k)
+    S = np.abs(Z) @ np.abs(Z)
+    bound = (3 * 2.0 ** -22 + (k / 8 + 8) * 2.0 ** -23) * S + 4 * EPS * np.abs(2 * X - Y)
+    assert np.all(np.abs(out - (2.0 * X - Y)) <= bound)
+    assert np.array_equal(out, out.T)
+    assert sc[0] == pytest.approx(np.trace(out), rel=1e-12, abs=1e-13)       # scalars describe the matrix written
+    assert sc[1] == pytest.approx(np.sum(out * out), rel=1e-12)
+    assert sc[3] == pytest.approx(np.trace(Y), rel=1e-4)
+
+
+@pytest.mark.parametrize("c,k", [(3, 256), (3, 640), (2, 333), (4, 450)])
+def test_expand_mixed(handle, c, k):
+    """Mixed variant with the FP64 head (R-MIX): north_star's reduced-precision tolerances 1e-6 / 1e-8 and
+    identical iteration counts against the oracle's FP32 steps; FP32 steps occupy the same positions."""
+    w = rfoe_inputs.make_workload(c, k=k)
+    head = w.nocc / 512.0      # FP32 phase starts late enough for the ORACLE's own FP32 noise to stay below 1e-6
+    ref = oracle.expand(w.H, w.nocc, variant=oracle.SP2_MIXED, tol=w.tol, mixed_head=head, mixed_reltr=5e-4)
+    handle.configure(mixed_head=head, mixed_reltr=5e-4)
+    res = handle.expand(_dev(w.H), w.nocc, rfoe.SP2_MIXED, w.tol)
+    P = res.P.cpu().numpy()
+    assert res.converged and ref.converged
+    assert res.iterations == ref.iterations
+    assert res.fp32_steps == ref.fp32_steps >= 2
+    assert [ch.islower() for ch in res.branch] == [ch.islower() for ch in ref.branch]
+    dP = np.linalg.norm(P - ref.P) / math.sqrt(k)
+    dE = abs(res.tr_PH - ref.tr_PH) / abs(ref.tr_PH)
+    print(f"mixed c={c} k={k}: fp32 steps {res.fp32_steps}/{res.iterations} dP={dP:.2e} dE={dE:.2e} "
+          f"errP_exact={np.linalg.norm(P - w.exact_projector()) / math.sqrt(k):.2e}")
+    assert dP <= 1e-6 and dE <= 1e-8
+    assert np.array_equal(P, P.T)
+    assert abs(np.trace(P) - w.nocc) <= 1e-9
+    assert np.linalg.norm(P @ P - P) <= 1e-10 * max(1.0, k / 256)
+
+
+def test_expand_mixed_paper_schedule(handle):
+    """Paper's own schedule (FP32 from the first step until RelTr <= 5e-4): converges to a
+    projector with tr P = nocc; accuracy is FP32-limited (paper: eps1 ~ 1e-7 on its matrix), reported, not 1e-6."""
+    w = rfoe_inputs.make_workload(3, k=512)
+    handle.configure(mixed_head=0.0, mixed_reltr=5e-4)
+    res = handle.expand(_dev(w.H), w.nocc, rfoe.SP2_MIXED, w.tol)
+    ref = oracle.expand(w.H, w.nocc, variant=oracle.SP2_MIXED, tol=w.tol, mixed_head=0.0, mixed_reltr=5e-4)
+    P = res.P.cpu().numpy()
+    assert res.converged and res.iterations == ref.iterations and res.fp32_steps == ref.fp32_steps
+    assert abs(np.trace(P) - w.nocc) <= 1e-9
+    err = np.linalg.norm(P - w.exact_projector()) / math.sqrt(w.k)
+    assert err <= 2e-4
+    assert abs(res.tr_PH - w.band_energy()) / abs(w.band_energy()) <= 1e-7
