@@ -110,3 +110,41 @@ def test_fullsize_config5():
     os.makedirs("gpurun_out", exist_ok=True)
     with open("gpurun_out/config5.txt", "w") as f:
         f.write(repr(r) + "\n")
+
+
+def _run_fullsize_mixed(c):
+    """Reduced-precision path (A8) at full size with the paper's schedule (FP32 steps from the start until
+    RelTr <= 5e-4).  The oracle's FP32 loop cannot run here; properties that hold at any
+    size: north_star's reduced-precision tolerances against the construction-exact projector (1e-6) and the
+    exact band energy (1e-8), the FP64 path's iteration count and branch string, tr P = nocc, idempotency."""
+    w = rfoe_inputs.make_workload(c, device="cuda")
+    k, nocc = w.k, w.nocc
+    Qo = w.Q[:, :nocc]
+    Pex = Qo @ Qo.T
+    del Qo
+    with rfoe.Rfoe(k) as h:
+        r64 = h.expand(w.H, nocc, rfoe.SP2, w.tol)
+        its64, br64, ms64 = r64.iterations, r64.branch, r64.device_ms
+        del r64
+        h.configure(mixed_head=0.0, mixed_reltr=5e-4)
+        res = h.expand(w.H, nocc, rfoe.SP2_MIXED, w.tol)
+    assert res.status == rfoe.OK and res.converged
+    assert res.iterations == its64 and res.branch.upper() == br64
+    assert res.fp32_steps >= res.iterations // 2 and res.branch[: res.fp32_steps].islower()
+    P = res.P
+    assert torch.equal(P, P.T)
+    assert abs(torch.diagonal(P).sum().item() - nocc) <= 1e-8
+    dP = torch.linalg.norm(P - Pex).item() / math.sqrt(k)
+    dE = abs(res.tr_PH - w.band_energy()) / abs(w.band_energy())
+    idem = torch.linalg.norm(P @ P - P).item()
+    assert dP <= 1e-6 and dE <= 1e-8 and idem <= 1e-10 * k / 256, (dP, dE, idem)
+    return dict(k=k, iterations=res.iterations, fp32_steps=res.fp32_steps, dP=dP, dE=dE, idem=idem,
+                device_ms=res.device_ms, fp64_device_ms=ms64, branch=res.branch)
+
+
+def test_fullsize_config3_mixed():
+    print(_run_fullsize_mixed(3))
+
+
+def test_fullsize_config4_mixed():
+    print(_run_fullsize_mixed(4))
