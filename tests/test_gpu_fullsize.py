@@ -148,3 +148,46 @@ def test_fullsize_config3_mixed():
 
 def test_fullsize_config4_mixed():
     print(_run_fullsize_mixed(4))
+
+
+def test_paper_workload_k8192():
+    """NEXT-3: the paper's own synthetic H^p (reading R12), N_occ = 0.9 k, RelTr 5e-8 (stop rule B,
+    PAPER.md:92), k = 8192 (the smallest size the paper runs).  D_ref comes from an explicit
+    eigendecomposition, as in the paper (ELPA there, torch.linalg.eigh here -- harness only); error metrics
+    eps1 = ||D - D_ref||_F / ||D_ref||_F and eps2 = |Tr(D H) - Tr(D_ref H)| / |Tr(D_ref H)|.
+    Paper: "around 50" Z-RFOE and "around 30" A-Z-RFOE iterations, eps1 ~ 1e-10, eps2 ~ 1e-9 (FP64),
+    eps1 ~ 1e-7, eps2 ~ 1e-9 (mixed)."""
+    k = 8192
+    Hn = rfoe_inputs.paper_matrix(k)
+    H = torch.from_numpy(Hn).cuda()
+    nocc = round(0.9 * k)
+    lam, V = torch.linalg.eigh(H)
+    Vo = V[:, :nocc]
+    Dref = Vo @ Vo.T
+    del V, Vo
+    homo, lumo, eband = lam[nocc - 1].item(), lam[nocc].item(), lam[:nocc].sum().item()
+    nref = torch.linalg.norm(Dref).item()
+    assert nref == pytest.approx(math.sqrt(nocc), rel=1e-9)                      # R14: ||D_ref||_F = sqrt(N_occ)
+
+    def eps(r):
+        return torch.linalg.norm(r.P - Dref).item() / nref, abs(r.tr_PH - eband) / abs(eband)
+
+    out = {}
+    with rfoe.Rfoe(k) as h:
+        h.configure(stop_rule=rfoe.RULE_B)
+        z = h.expand(H, nocc, rfoe.SP2, 5e-8)
+        out["Z-RFOE"] = (z.iterations, *eps(z), z.device_ms)
+        model = pins.scalar_sp2(lam.cpu().numpy(), nocc, z.eps_min, z.eps_max, tol=5e-8, rule="B")
+        assert z.converged and z.iterations == model["iterations"] and 45 <= z.iterations <= 60
+        assert out["Z-RFOE"][1] <= 1e-5 and out["Z-RFOE"][2] <= 1e-6              # limited by the RelTr stop, not by rounding
+        h.configure(homo=homo, lumo=lumo)
+        a = h.expand(H, nocc, rfoe.SP2_ACCEL, 5e-8)
+        out["A-Z-RFOE"] = (a.iterations, *eps(a), a.device_ms)
+        assert a.converged and 26 <= a.iterations <= 34
+        assert out["A-Z-RFOE"][1] <= 1e-9 and out["A-Z-RFOE"][2] <= 1e-9
+        h.configure(mixed_head=0.0, mixed_reltr=5e-4)
+        m = h.expand(H, nocc, rfoe.SP2_MIXED, 5e-8)
+        out["Z-RFOE mixed"] = (m.iterations, *eps(m), m.device_ms)
+        assert m.converged and m.iterations == z.iterations and m.fp32_steps >= 20
+        assert out["Z-RFOE mixed"][1] <= 1e-5 and out["Z-RFOE mixed"][2] <= 1e-6
+    print({k_: tuple(float(f"{v:.3g}") for v in vs) for k_, vs in out.items()})
