@@ -290,3 +290,22 @@ def test_expand_mixed_paper_schedule(handle):
     err = np.linalg.norm(P - w.exact_projector()) / math.sqrt(w.k)
     assert err <= 2e-4
     assert abs(res.tr_PH - w.band_energy()) / abs(w.band_energy()) <= 1e-7
+
+
+def test_expand_mixed_truncated(handle):
+    """Mixed T-RFOE: the truncated expansion G_m with reduced-precision steps; fractional
+    occupancies, so the comparison with the oracle's FP32 loop is entry-wise at FP32 level, scalars likewise."""
+    w = rfoe_inputs.make_workload(1, k=192)
+    lo, hi = float(w.lam.min()) - 0.01, float(w.lam.max()) + 0.01
+    handle.configure(bounds=(lo, hi), max_iter=9, mixed_head=0.0, mixed_reltr=0.0)
+    try:
+        ref = oracle.expand(w.H, w.nocc, variant=oracle.SP2_MIXED, tol=0.0, max_iter=9, bounds_override=(lo, hi),
+                            mixed_head=0.0, mixed_reltr=0.0)
+        res = handle.expand(_dev(w.H), w.nocc, rfoe.SP2_MIXED, 0.0)
+    finally:
+        handle.configure(bounds=False, max_iter=100, mixed_reltr=5e-4)
+    assert res.status == rfoe.ERR_NOT_CONVERGED and res.iterations == ref.iterations == 9
+    assert res.fp32_steps == ref.fp32_steps == 9 and res.branch == ref.branch
+    P = res.P.cpu().numpy()
+    assert np.abs(P - ref.P).max() <= 2e-5
+    assert np.allclose(res.t, ref.t, rtol=0, atol=1e-3) and np.array_equal(P, P.T)
