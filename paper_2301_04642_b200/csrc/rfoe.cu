@@ -46,6 +46,8 @@ struct rfoe_handle_s {
     int* d_flag = nullptr;
     Ctrl* d_ctrl = nullptr;
     int2* d_tiles = nullptr;
+    int2* d_pairs = nullptr;   // reduced-precision kernel: (I, J0) of every 2-CTA cluster (tiles (I,J0), (I,J0+1))
+    int n_pairs = 0;
     int tiles_m = 0;       // tile-grid size the tile map was built for
     int n_tiles = 0;
     HostPage* hp = nullptr;
@@ -98,12 +100,16 @@ static void build_tile_order(int m, std::vector<int2>& out)
 static int ensure_tiles(rfoe_handle_s* h, int m, cudaStream_t st)
 {
     if (h->tiles_m == m) return RFOE_OK;
-    std::vector<int2> order;
+    std::vector<int2> order, pairs;
     build_tile_order(m, order);
+    for (const int2& t : order)      // row pairs in the same L2-friendly order: tiles (i, j), (i, j+1) with j - i even
+        if (((t.y - t.x) & 1) == 0) pairs.push_back(t);
     CK(cudaMemcpyAsync(h->d_tiles, order.data(), order.size() * sizeof(int2), cudaMemcpyHostToDevice, st));
-    CK(cudaStreamSynchronize(st));   // `order` is pageable and dies here
+    CK(cudaMemcpyAsync(h->d_pairs, pairs.data(), pairs.size() * sizeof(int2), cudaMemcpyHostToDevice, st));
+    CK(cudaStreamSynchronize(st));   // the vectors are pageable and die here
     h->tiles_m = m;
     h->n_tiles = (int)order.size();
+    h->n_pairs = (int)pairs.size();
     return RFOE_OK;
 }
 
@@ -127,7 +133,7 @@ static int make_map32(rfoe_handle_s* h, CUtensorMap* map, float* base, int n, in
 {
     cuuint64_t dims[2] = {(cuuint64_t)n, (cuuint64_t)n};
     cuuint64_t strides[1] = {(cuuint64_t)ld32 * sizeof(float)};
-    cuuint32_t box[2] = {(cuuint32_t)TQ_BK, (cuuint32_t)TQ_BM};
+    cuuint32_t box[2] = {(cuuint32_t)TQ_BK, (cuuint32_t)(TQ_BM / 2)};   // half panels: 64 rows x 128 bytes
     cuuint32_t estr[2] = {1, 1};
     CUresult r = h->encode(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, base, dims, strides, box, estr,
                            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
@@ -154,10 +160,21 @@ static cudaError_t launch_square_tf32(rfoe_handle_s* h, const CUtensorMap& hi, c
 {
     split_tf32_kernel<<<hbm_grid(h, n), 256, 0, st>>>(Xin, n, ld, k, trace, h->F[0], h->F[1], n + TQ_PAD);
     h->launches++;
-    sym_square_tf32_kernel<<<h->n_tiles, TQ_THREADS, TQ_SMEM_BYTES, st>>>(hi, lo, Xin, Out, n, ld, k, trace, coef, h->d_tiles,
-                                                                         partials);
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(2 * h->n_pairs);
+    cfg.blockDim = dim3(TQ_THREADS);
+    cfg.dynamicSmemBytes = TQ_SMEM_BYTES;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = 2;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
     h->launches++;
-    return cudaGetLastError();
+    return cudaLaunchKernelEx(&cfg, sym_square_tf32_kernel, hi, lo, Xin, Out, n, ld, k, trace, coef, (const int2*)h->d_pairs,
+                              n / TQ_BM, partials);
 }
 
 template <bool TWO_OP>
@@ -209,6 +226,7 @@ extern "C" int rfoe_destroy(rfoe_handle_t h)
     for (double* p : h->part) cudaFree(p);
     for (double* p : h->rows) cudaFree(p);
     cudaFree(h->d_bounds); cudaFree(h->d_scalars); cudaFree(h->d_flag); cudaFree(h->d_ctrl); cudaFree(h->d_tiles);
+    cudaFree(h->d_pairs);
     cudaFree(h->stage_H); cudaFree(h->stage_P);
     if (h->hp) cudaFreeHost(h->hp);
     if (h->ev0) cudaEventDestroy(h->ev0);
@@ -241,8 +259,8 @@ extern "C" int rfoe_create(rfoe_handle_t* out, int device, int64_t k_max)
     bool ok = true;
     ok = ok && cudaMalloc(&h->W[0], wbytes) == cudaSuccess;
     ok = ok && cudaMalloc(&h->W[1], wbytes) == cudaSuccess;
-    ok = ok && cudaMalloc(&h->part[0], nt * SQ_NPART * sizeof(double)) == cudaSuccess;
-    ok = ok && cudaMalloc(&h->part[1], nt * SQ_NPART * sizeof(double)) == cudaSuccess;
+    ok = ok && cudaMalloc(&h->part[0], (nt + m) * SQ_NPART * sizeof(double)) == cudaSuccess;   // + phantom records
+    ok = ok && cudaMalloc(&h->part[1], (nt + m) * SQ_NPART * sizeof(double)) == cudaSuccess;
     ok = ok && cudaMalloc(&h->rows[0], ld * sizeof(double)) == cudaSuccess;
     ok = ok && cudaMalloc(&h->rows[1], ld * sizeof(double)) == cudaSuccess;
     ok = ok && cudaMalloc(&h->d_bounds, 2 * sizeof(double)) == cudaSuccess;
@@ -250,6 +268,7 @@ extern "C" int rfoe_create(rfoe_handle_t* out, int device, int64_t k_max)
     ok = ok && cudaMalloc(&h->d_flag, sizeof(int)) == cudaSuccess;
     ok = ok && cudaMalloc(&h->d_ctrl, sizeof(Ctrl)) == cudaSuccess;
     ok = ok && cudaMalloc(&h->d_tiles, nt * sizeof(int2)) == cudaSuccess;
+    ok = ok && cudaMalloc(&h->d_pairs, nt * sizeof(int2)) == cudaSuccess;
     ok = ok && cudaHostAlloc((void**)&h->hp, sizeof(HostPage), cudaHostAllocMapped) == cudaSuccess;
     ok = ok && cudaHostGetDevicePointer((void**)&h->d_word, (void*)&h->hp->word, 0) == cudaSuccess;
     ok = ok && cudaEventCreate(&h->ev0) == cudaSuccess && cudaEventCreate(&h->ev1) == cudaSuccess;
@@ -453,7 +472,7 @@ extern "C" int rfoe_expand(rfoe_handle_t h, const double* Hp, int64_t k64, int64
             CK(launch_square_tf32(h, tmF[0], tmF[1], h->W[cur], h->W[nxt], n, ld, k, &h->d_ctrl->t, &h->d_ctrl->coef, h->part[0], st));
             CK(cudaEventRecord(h->sq_ev[2 * h->sq_n + 1], st));
             h->sq_n++;
-            control_kernel<<<1, 256, 0, st>>>(h->d_ctrl, 1, h->part[0], h->part[0], h->n_tiles, h->d_word);
+            control_kernel<<<1, 256, 0, st>>>(h->d_ctrl, 1, h->part[0], h->part[0], 2 * h->n_pairs, h->d_word);
         } else if (action == ACT_MCWEENY) {
             CK(timed_square<false>(h, tm[cur], tm[cur], h->W[cur], h->W[2], n, ld, k, &h->d_ctrl->coef, h->part[0], st));
             CK(timed_square<true>(h, tm[2], tm[cur], h->W[2], h->W[nxt], n, ld, k, &h->d_ctrl->coef_aux, h->part[1], st));
@@ -542,7 +561,7 @@ static int single_product(rfoe_handle_s* h, const double* A, const double* B, in
     else if (two) CK(launch_square<true>(h, tm[0], tm[1], h->W[0], h->W[2], n, ld, k, &h->d_ctrl->coef, h->part[0], st));
     else     CK(launch_square<false>(h, tm[0], tm[0], h->W[0], h->W[2], n, ld, k, &h->d_ctrl->coef, h->part[0], st));
     CK(cudaEventRecord(h->ev1, st));
-    sum_partials_kernel<<<1, 256, 0, st>>>(h->part[0], h->n_tiles, h->d_scalars);
+    sum_partials_kernel<<<1, 256, 0, st>>>(h->part[0], reduced ? 2 * h->n_pairs : h->n_tiles, h->d_scalars);
     h->launches++;
     copy_out_kernel<<<hbm_grid(h, k), HBM_THREADS, 0, st>>>(h->W[2], k, ld, nullptr, Cout, nullptr);
     h->launches++;

@@ -17,6 +17,12 @@
 //
 // Roles (192 threads): warp 0 = TMA producer, warp 1 = TMEM allocator + single-thread MMA issuer,
 // warps 2..5 = epilogue (each reads its own 32 TMEM lanes = 32 tile rows).
+// Clusters of two CTAs own the tiles (I, J0) and (I, J0+1): they share the row panels Zh(I), Zl(I), each
+// CTA fetches half of them and TMA-multicasts it to both (25 % fewer L2 requests per CTA; the kernel is
+// bound by L2->SM bytes per flop, profiles/r01c).  A stage is refilled only after BOTH CTAs' MMAs have
+// read it (multicast tcgen05.commit on both empty barriers).  A row with an odd number of tiles ends in a
+// phantom tile (J0+1 = m): that CTA loads zeros (TMA out-of-bounds fill), serves its half of the shared
+// panels and writes nothing but a zero partial record.
 #pragma once
 #include "ptx_sm100.cuh"
 #include "sym_square.cuh"
@@ -33,6 +39,7 @@ constexpr int TQ_STAGE_BYTES = 4 * TQ_PANEL_BYTES;               // A_hi, A_lo, 
 constexpr int TQ_SMEM_BYTES = TQ_STAGES * TQ_STAGE_BYTES + 1024; // + slack for 1024-byte alignment
 constexpr int TQ_CHUNK_KT = 8;             // K chunks (of 32) per tensor-memory accumulation run: 256 k values
 constexpr int TQ_TMEM_COLS = 512;          // head accumulator x 2 (double-buffered) + cross-term accumulator
+constexpr int TQ_HALF_BYTES = TQ_PANEL_BYTES / 2;                // 64 rows of a panel
 constexpr int TQ_PAD = 32;                 // floats added to the row pitch of the hi / lo matrices
 
 // HBM-bound: split the FP64 work matrix (n x n, pitch ld) into tf32-rounded hi and lo FP32 matrices
@@ -70,7 +77,7 @@ __global__ void __launch_bounds__(TQ_THREADS, 1)
 sym_square_tf32_kernel(const __grid_constant__ CUtensorMap tmHi, const __grid_constant__ CUtensorMap tmLo,
                        const double* __restrict__ E, double* __restrict__ Out, int n, int ld, int kvalid,
                        const double* __restrict__ trace, const StepCoef* __restrict__ coef,
-                       const int2* __restrict__ tile_map, double* __restrict__ partials)
+                       const int2* __restrict__ pair_map, int m_tiles, double* __restrict__ partials)
 {
     extern __shared__ uint8_t smem_raw[];
     __shared__ __align__(8) uint64_t full_bar[TQ_STAGES];
@@ -82,8 +89,10 @@ sym_square_tf32_kernel(const __grid_constant__ CUtensorMap tmHi, const __grid_co
 
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
-    const int2 tile = tile_map[blockIdx.x];
-    const int I = tile.x, J = tile.y;
+    const uint32_t crank = cluster_ctarank();               // 0 or 1
+    const int2 pair = pair_map[blockIdx.x >> 1];
+    const int I = pair.x, J = pair.y + (int)crank;
+    const bool phantom = (J >= m_tiles);
     const bool diag = (I == J);
     const int KT = n / TQ_BK;
 
@@ -96,7 +105,7 @@ sym_square_tf32_kernel(const __grid_constant__ CUtensorMap tmHi, const __grid_co
     if (threadIdx.x == 0) {
         for (int s = 0; s < TQ_STAGES; ++s) {
             mbar_init(full0 + 8 * s, 1);
-            mbar_init(empty0 + 8 * s, 1);
+            mbar_init(empty0 + 8 * s, 2);      // this CTA's MMA commit + the peer's
         }
         for (int b = 0; b < 2; ++b) {
             mbar_init(hfull0 + 8 * b, 1);
@@ -108,7 +117,7 @@ sym_square_tf32_kernel(const __grid_constant__ CUtensorMap tmHi, const __grid_co
     }
     if (warp == 1) tmem_alloc<TQ_TMEM_COLS>(smem_u32(&tmem_base_sh));
     tc_fence_before();
-    __syncthreads();
+    cluster_sync_all();                         // barriers of both CTAs initialised before any multicast lands
     tc_fence_after();
     const uint32_t tmem = tmem_base_sh;
 
@@ -117,18 +126,20 @@ sym_square_tf32_kernel(const __grid_constant__ CUtensorMap tmHi, const __grid_co
         if (lane == 0) {
             int s = 0;
             uint32_t ph = 0;
-            const uint32_t bytes = diag ? 2 * TQ_PANEL_BYTES : 4 * TQ_PANEL_BYTES;
             for (int kt = 0; kt < KT; ++kt) {
-                mbar_wait_bounded(empty0 + 8 * s, ph ^ 1u);
+                mbar_wait_bounded(empty0 + 8 * s, ph ^ 1u);              // both CTAs have consumed this stage
                 const uint32_t fb = full0 + 8 * s;
                 const uint32_t dst = smem_base + s * TQ_STAGE_BYTES;
-                mbar_expect_tx(fb, bytes);
-                tma_load_2d(dst, &tmHi, kt * TQ_BK, I * TQ_BM, fb);
-                tma_load_2d(dst + TQ_PANEL_BYTES, &tmLo, kt * TQ_BK, I * TQ_BM, fb);
-                if (!diag) {
-                    tma_load_2d(dst + 2 * TQ_PANEL_BYTES, &tmHi, kt * TQ_BK, J * TQ_BM, fb);
-                    tma_load_2d(dst + 3 * TQ_PANEL_BYTES, &tmLo, kt * TQ_BK, J * TQ_BM, fb);
-                }
+                mbar_expect_tx(fb, TQ_STAGE_BYTES);                     // 2 x 8 KiB from me + 2 x 8 KiB from the peer + 32 KiB own
+                const int c0 = kt * TQ_BK;
+                // my half of the shared row panels, to both CTAs
+                tma_load_2d_mc(dst + crank * TQ_HALF_BYTES, &tmHi, c0, I * TQ_BM + (int)crank * 64, fb, (uint16_t)3);
+                tma_load_2d_mc(dst + TQ_PANEL_BYTES + crank * TQ_HALF_BYTES, &tmLo, c0, I * TQ_BM + (int)crank * 64, fb, (uint16_t)3);
+                // my own column panels (rows of tile column J; beyond the matrix for a phantom tile -> zeros)
+                tma_load_2d(dst + 2 * TQ_PANEL_BYTES, &tmHi, c0, J * TQ_BM, fb);
+                tma_load_2d(dst + 2 * TQ_PANEL_BYTES + TQ_HALF_BYTES, &tmHi, c0, J * TQ_BM + 64, fb);
+                tma_load_2d(dst + 3 * TQ_PANEL_BYTES, &tmLo, c0, J * TQ_BM, fb);
+                tma_load_2d(dst + 3 * TQ_PANEL_BYTES + TQ_HALF_BYTES, &tmLo, c0, J * TQ_BM + 64, fb);
                 if (++s == TQ_STAGES) { s = 0; ph ^= 1u; }
             }
         }
@@ -150,8 +161,8 @@ sym_square_tf32_kernel(const __grid_constant__ CUtensorMap tmHi, const __grid_co
                 const uint32_t a_hi = smem_base + s * TQ_STAGE_BYTES;
                 const uint32_t a_lo = a_hi + TQ_PANEL_BYTES;
                 const uint64_t dAh = umma_desc_k128(a_hi), dAl = umma_desc_k128(a_lo);
-                const uint64_t dBh = diag ? dAh : umma_desc_k128(a_hi + 2 * TQ_PANEL_BYTES);
-                const uint64_t dBl = diag ? dAl : umma_desc_k128(a_hi + 3 * TQ_PANEL_BYTES);
+                const uint64_t dBh = umma_desc_k128(a_hi + 2 * TQ_PANEL_BYTES);
+                const uint64_t dBl = umma_desc_k128(a_hi + 3 * TQ_PANEL_BYTES);
                 const uint32_t t_head = tmem + hb * TQ_BM, t_cross = tmem + 2 * TQ_BM;
 #pragma unroll
                 for (int ks = 0; ks < TQ_BK / TQ_UK; ++ks) {
@@ -160,7 +171,7 @@ sym_square_tf32_kernel(const __grid_constant__ CUtensorMap tmHi, const __grid_co
                     umma_tf32(t_cross, dAh + o, dBl + o, idesc, (kt | ks) != 0);  // cross terms: tiny, one long accumulation
                     umma_tf32(t_cross, dAl + o, dBh + o, idesc, 1u);
                 }
-                umma_commit(empty0 + 8 * s);      // frees the stage when these MMAs have read it
+                umma_commit_mc(empty0 + 8 * s, (uint16_t)3);   // frees the stage in BOTH CTAs' producers' view
                 if (kc == TQ_CHUNK_KT - 1 || kt == KT - 1) umma_commit(hfull0 + 8 * hb);   // chunk complete
                 if (++s == TQ_STAGES) { s = 0; ph ^= 1u; }
             }
@@ -190,6 +201,9 @@ sym_square_tf32_kernel(const __grid_constant__ CUtensorMap tmHi, const __grid_co
             if (lane == 0) mbar_arrive(hempty0 + 8 * hb);
         }
         // ---- the last chunk's commit also covers every cross-term MMA: finish in FP64
+        if (phantom) {
+            if (lane == 0) { red[q][0] = red[q][1] = red[q][2] = red[q][3] = red[q][4] = 0.0; }
+        } else {
         const double d = *trace / (double)kvalid;
         const double c2 = coef->c2, c1 = coef->c1, c0 = coef->c0;
         double p_tr = 0.0, p_ss = 0.0, p_err = 0.0, p_trc = 0.0, p_ce = 0.0;
@@ -257,9 +271,11 @@ sym_square_tf32_kernel(const __grid_constant__ CUtensorMap tmHi, const __grid_co
         if (lane == 0) {
             red[q][0] = p_tr; red[q][1] = p_ss; red[q][2] = p_err; red[q][3] = p_trc; red[q][4] = p_ce;
         }
+        }
     }
+    __syncwarp();
     tc_fence_before();
-    __syncthreads();
+    cluster_sync_all();                         // the peer's commits / multicasts into this CTA are over
     if (warp == 1) tmem_dealloc<TQ_TMEM_COLS>(tmem);
     if (threadIdx.x < 5)
         partials[(size_t)blockIdx.x * SQ_NPART + threadIdx.x] =
