@@ -9,7 +9,7 @@
  *
  * What it follows (PAPER.md line : section):
  *   - X_{n+1} = X_n +/- (X_n - X_n^2), i.e. X^2 or 2X - X^2, sign chosen so that the trace
- *     converges to N_occ                                   PAPER.md:35-39 (sec. II.B.1, Eq. 1)
+ *     of X_{n+1} lands nearer N_occ                                 PAPER.md:35-39 (sec. II.B.1, Eq. 1)
  *   - Tr(X) by diagonal traversal, Tr(X^2) = ||X||_F^2      PAPER.md:72    (sec. III.B)
  *   - RelTr = trace change relative to the previous iterate PAPER.md:64, 92 (sec. III.A, IV)
  *   - mixed precision: FP32 steps far from convergence,
@@ -244,7 +244,18 @@ int rfoe_oracle_expand(const double* H, int64_t k, int64_t nocc, oracle_run_t* r
     double reltr_prev = INFINITY;
 
     for (int n = 0; n < run->max_iter; ++n) {
-        const int sq = (t > (double)nocc);           /* S iff Tr X_n > N_occ; tie -> L (R4, R5) */
+        /* "The +/- sign is chosen to adjust the trace of X_{n+1} ... such that it converges to N_occ"
+         * (PAPER.md:39): take the branch whose RESULTING trace is nearer N_occ; tie -> L (R4, R5).
+         * Tr X^2 = s and Tr(2X - X^2) = 2t - s are known before the product.  For a spectrum
+         * inside [0,1] (t - s >= 0) this is exactly "S iff t > N_occ"; it differs only when rounding noise has
+         * pushed eigenvalues outside [0,1], where it picks the branch that maps them back. */
+        double trS = s, trL = 2.0 * t - s;
+        if (run->variant == ORC_SP2_ACCEL) {
+            const double aS = 2.0 / (2.0 - beta), aL = 2.0 / (1.0 + bbar);
+            trS = aS * aS * s + 2.0 * aS * (1.0 - aS) * t + (1.0 - aS) * (1.0 - aS) * (double)k;
+            trL = 2.0 * aL * t - aL * aL * s;
+        }
+        const int sq = (fabs(trS - (double)nocc) < fabs(trL - (double)nocc));
         if (mixed_phase == 0 && (t - s) < run->mixed_head) mixed_phase = 1;
         if (mixed_phase == 1 && reltr_prev <= run->mixed_reltr) mixed_phase = 2;
         const int fp32 = (mixed_phase == 1);

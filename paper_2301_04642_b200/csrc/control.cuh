@@ -85,7 +85,17 @@ bounds_reduce_kernel(const double* __restrict__ row_lo, const double* __restrict
 __device__ inline void decide_next(Ctrl* c)
 {
     const double t = c->t, s = c->s;
-    const bool sq = (t > c->nocc);                      // S iff Tr X_n > N_occ, tie -> L (R4, R5)
+    // "The +/- sign is chosen to adjust the trace of X_{n+1} ... such that it converges to N_occ":
+    // the branch whose RESULTING trace is nearer N_occ, tie -> L (R4, R5).  Both candidate traces follow from
+    // t = Tr X_n and s = Tr X_n^2 before the product.  Inside [0,1] this is "S iff t > N_occ"; it differs only
+    // when rounding noise has pushed eigenvalues outside [0,1], where it picks the branch that maps them back.
+    double trS = s, trL = 2.0 * t - s;
+    if (c->variant == VAR_ACCEL) {
+        const double aS = 2.0 / (2.0 - c->beta), aL = 2.0 / (1.0 + c->bbar);
+        trS = aS * aS * s + 2.0 * aS * (1.0 - aS) * t + (1.0 - aS) * (1.0 - aS) * (double)c->kvalid;
+        trL = 2.0 * aL * t - aL * aL * s;
+    }
+    const bool sq = fabs(trS - c->nocc) < fabs(trL - c->nocc);
     int action = ACT_SP2;
     if (c->variant == VAR_MCWEENY) {
         if (!c->mcweeny_phase && (t - s) < 3.0 / 16.0 && fabs(t - c->nocc) < 0.5) c->mcweeny_phase = 1;   // R11

@@ -228,12 +228,4 @@ __device__ __forceinline__ void umma_commit_mc(uint32_t bar, uint16_t mask)
                  : "memory");
 }
 
-// prefetch one TMA box into L2 only (no shared memory, no barrier)
-__device__ __forceinline__ void tma_prefetch_l2_2d(const CUtensorMap* map, int c0, int c1)
-{
-    asm volatile("cp.async.bulk.prefetch.tensor.2d.L2.global.tile [%0, {%1, %2}];" ::"l"(reinterpret_cast<uint64_t>(map)), "r"(c0),
-                 "r"(c1)
-                 : "memory");
-}
-
 }  // namespace rfoe

@@ -53,7 +53,7 @@ def jacobi_projector(H, nocc: int):
 
 def scalar_sp2(lam, nocc: int, emin: float, emax: float, *, tol: float, rule: str = "A", max_iter: int = 100):
     """Eigenvalue-space SP2 (pin P5): x_i <- (emax - lam_i)/(emax - emin), then x <- x^2 if
-    sum(x) > nocc else 2x - x^2.  Returns dict(branch, iterations, t, s, e)."""
+    the resulting trace is nearer nocc than that of 2x - x^2 (else the latter).  Returns dict(branch, iterations, t, s, e)."""
     x = (emax - np.asarray(lam, dtype=np.float64)) / (emax - emin)
     t_hist, s_hist, e_hist, branch = [float(np.sum(x))], [float(np.sum(x * x))], [], ""
     it = 0
@@ -61,7 +61,8 @@ def scalar_sp2(lam, nocc: int, emin: float, emax: float, *, tol: float, rule: st
         t = float(np.sum(x))
         x2 = x * x
         e = float(np.sqrt(np.sum((x2 - x) ** 2)))
-        if t > nocc:
+        # the sign that brings the trace of X_{n+1} nearer N_occ (tie -> L)
+        if abs(float(np.sum(x2)) - nocc) < abs(float(np.sum(2.0 * x - x2)) - nocc):
             x = x2
             branch += "S"
         else:
@@ -89,13 +90,14 @@ def scalar_sp2_accel(lam, nocc: int, emin: float, emax: float, homo: float, lumo
     for _ in range(max_iter):
         t = float(np.sum(x))
         e = float(np.sqrt(np.sum((x * x - x) ** 2)))
-        if t > nocc:
-            a = 2.0 / (2.0 - beta)
-            f = lambda v: ((1.0 - a) + a * v) ** 2
+        aS, aL = 2.0 / (2.0 - beta), 2.0 / (1.0 + bbar)
+        fS = lambda v, a=aS: ((1.0 - a) + a * v) ** 2
+        fL = lambda v, a=aL: 2.0 * (a * v) - (a * v) ** 2
+        if abs(float(np.sum(fS(x))) - nocc) < abs(float(np.sum(fL(x))) - nocc):
+            f = fS
             branch += "S"
         else:
-            a = 2.0 / (1.0 + bbar)
-            f = lambda v: 2.0 * (a * v) - (a * v) ** 2
+            f = fL
             branch += "L"
         x, beta, bbar = f(x), f(beta), f(bbar)
         it += 1
