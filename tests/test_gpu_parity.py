@@ -12,6 +12,7 @@ import pytest
 
 import oracle
 import rfoe_inputs
+from tests import pins
 
 torch = pytest.importorskip("torch")
 pytestmark = pytest.mark.gpu
@@ -309,3 +310,43 @@ def test_expand_mixed_truncated(handle):
     P = res.P.cpu().numpy()
     assert np.abs(P - ref.P).max() <= 2e-5
     assert np.allclose(res.t, ref.t, rtol=0, atol=1e-3) and np.array_equal(P, P.T)
+
+
+# ------------------------------------------------------------------ tiny and degenerate problems
+@pytest.mark.parametrize("k,nocc", [(2, 1), (3, 1), (3, 2), (5, 4)])
+def test_expand_tiny(handle, k, nocc):
+    rng = np.random.default_rng(900 + 10 * k + nocc)
+    A = rng.standard_normal((k, k))
+    H = np.ascontiguousarray(0.5 * (A + A.T)) + np.diag(np.arange(k, dtype=np.float64))
+    ref = oracle.expand(H, nocc, tol=1e-12)
+    res = handle.expand(_dev(H), nocc, rfoe.SP2, 1e-12)
+    assert res.converged and ref.converged and res.iterations == ref.iterations
+    P = res.P.cpu().numpy()
+    Pref, _ = pins.jacobi_projector(H, nocc)
+    assert np.abs(P - ref.P).max() <= 1e-13 and np.abs(P - Pref).max() <= 1e-12
+    assert abs(np.trace(P) - nocc) <= 1e-12
+
+
+def test_expand_degenerate_fermi_level(handle):
+    """No gap at the Fermi level: the eigenvalue pair straddling N_occ is degenerate, theta(mu I - H) is not a
+    projector of rank N_occ and the recursion cannot converge -- both sides must say so in the same way
+    (max_iter steps, NOT_CONVERGED, last iterate returned, the degenerate pair left at fractional occupation)."""
+    k, nocc = 64, 20
+    rng = np.random.default_rng(77)
+    Q, _ = np.linalg.qr(rng.standard_normal((k, k)))
+    lam = np.sort(rng.uniform(-1.0, 1.0, size=k))
+    lam[nocc] = lam[nocc - 1]                                  # HOMO == LUMO
+    H = (Q * lam[None, :]) @ Q.T
+    H = np.ascontiguousarray(0.5 * (H + H.T))
+    handle.configure(max_iter=60)
+    try:
+        ref = oracle.expand(H, nocc, tol=1e-12, max_iter=60)
+        res = handle.expand(_dev(H), nocc, rfoe.SP2, 1e-12)
+    finally:
+        handle.configure(max_iter=100)
+    assert not ref.converged and not res.converged and res.status == rfoe.ERR_NOT_CONVERGED
+    assert res.iterations == ref.iterations == 60
+    P = res.P.cpu().numpy()
+    occ = np.sort(np.linalg.eigvalsh(P))
+    assert np.sum((occ > 0.01) & (occ < 0.99)) >= 1            # fractional occupation survives
+    assert np.allclose(res.t[:20], ref.t[:20], rtol=0, atol=1e-8)   # the trace-steered map is chaotic here: compare the head only
