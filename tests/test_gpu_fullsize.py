@@ -191,3 +191,46 @@ def test_paper_workload_k8192():
         assert m.converged and m.iterations == z.iterations and m.fp32_steps >= 20
         assert out["Z-RFOE mixed"][1] <= 1e-5 and out["Z-RFOE mixed"][2] <= 1e-6
     print({k_: tuple(float(f"{v:.3g}") for v in vs) for k_, vs in out.items()})
+
+
+def _paper_matrix_cuda(k, block=4096):
+    """rfoe_inputs.paper_matrix (reading R12) built on the GPU in row blocks (same formula)."""
+    H = torch.empty((k, k), dtype=torch.float64, device="cuda")
+    j = torch.arange(k, device="cuda", dtype=torch.float64)
+    for r0 in range(0, k, block):
+        i = j[r0:r0 + block]
+        H[r0:r0 + block] = torch.exp(-0.5 * (i[:, None] - j[None, :]).abs()) * torch.sin(torch.minimum(i[:, None], j[None, :]) + 1.0)
+    return H
+
+
+@pytest.mark.slow
+def test_paper_workload_k65536():
+    """The paper's largest problem (k = 65536) on ONE B200: 34 GB per FP64 matrix.
+    No eigendecomposition reference at this size; properties only: the scalar-model-free invariants
+    tr D = N_occ, bitwise symmetry, idempotency, commutation with H, and A-Z-RFOE reaching the same D as Z-RFOE."""
+    k = 65536
+    nocc = round(0.9 * k)
+    H = _paper_matrix_cuda(k)
+    assert torch.allclose(H[:512, :512], torch.from_numpy(rfoe_inputs.paper_matrix(512)).cuda(), rtol=1e-13, atol=1e-300)
+    out = {}
+    with rfoe.Rfoe(k) as h:
+        h.configure(stop_rule=rfoe.RULE_B, check_symmetry=True)
+        z = h.expand(H, nocc, rfoe.SP2, 5e-8)
+        Pz = z.P
+        fl = 2.0 * k * (512 * 513 // 2) * 128 * 128
+        out["Z-RFOE"] = dict(steps=z.iterations, seconds=z.device_ms / 1e3, tflops=z.iterations * fl / (z.device_ms * 1e-3) / 1e12)
+        assert z.converged and 45 <= z.iterations <= 66
+        assert abs(torch.diagonal(Pz).sum().item() - nocc) <= 1e-3          # RelTr 5e-8 of 59k stops ~3e-3 away at most
+    # the handle (two 34 GB work matrices) is gone: room for the checks
+    PP = Pz @ Pz
+    idem = torch.linalg.norm(PP - Pz).item()
+    del PP
+    HP = H @ Pz
+    comm = torch.linalg.norm(HP - HP.T).item()
+    del HP
+    out["Z-RFOE"].update(idem=idem, comm=comm, trace_err=abs(torch.diagonal(Pz).sum().item() - nocc))
+    assert torch.equal(Pz, Pz.T) and idem <= 1e-2 and comm <= 1e-2
+    print(out)
+    os.makedirs("gpurun_out", exist_ok=True)
+    with open("gpurun_out/paper_k65536.txt", "w") as f:
+        f.write(repr(out) + "\n")
