@@ -228,4 +228,20 @@ __device__ __forceinline__ void umma_commit_mc(uint32_t bar, uint16_t mask)
                  : "memory");
 }
 
+// one lane of a CONVERGED warp (the warp stays converged, so the elected lane's tcgen05 / TMA instructions
+// take their operands from uniform registers; an `if (lane == 0)` region makes ptxas emit an
+// ELECT + R2UR.BROADCAST loop of ~14 instructions in front of every UTCHMMA / UTMALDG instead)
+__device__ __forceinline__ bool elect_one()
+{
+    uint32_t pred;
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "elect.sync _|p, 0xffffffff;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n"
+        : "=r"(pred));
+    return pred != 0;
+}
+
 }  // namespace rfoe

@@ -15,11 +15,11 @@
 // + c0 I written to (I,J) and mirrored, five FP64 partial sums per tile -- so the recursion, its
 // scalars and its control flow are unchanged; only the product is reduced precision.
 //
-// Roles (192 threads): warp 0 = TMA producer, warp 1 = TMEM allocator + single-thread MMA issuer,
-// warps 2..5 = epilogue (each reads its own 32 TMEM lanes = 32 tile rows).
+// Roles (192 threads): warp 0 = TMA producer, warp 1 = TMEM allocator + MMA issuer (both warps stay converged
+// and one elected lane issues, so the TMA / tcgen05 operands live in uniform registers), warps 2..5 = epilogue (each reads its own 32 TMEM lanes = 32 tile rows).
 // Clusters of two CTAs own the tiles (I, J0) and (I, J0+1): they share the row panels Zh(I), Zl(I), each
 // CTA fetches half of them and TMA-multicasts it to both (25 % fewer L2 requests per CTA; measured: no
-// change in time -- an ablation shows the MMA stream alone takes as long).
+// change in time -- the kernel runs into the 1 kW power cap).
 // A stage is refilled only after BOTH CTAs' MMAs have
 // read it (multicast tcgen05.commit on both empty barriers).  A row with an odd number of tiles ends in a
 // phantom tile (J0+1 = m): that CTA loads zeros (TMA out-of-bounds fill), serves its half of the shared
@@ -123,14 +123,15 @@ sym_square_tf32_kernel(const __grid_constant__ CUtensorMap tmHi, const __grid_co
     const uint32_t tmem = tmem_base_sh;
 
     if (warp == 0) {
-        // ===== TMA producer (one thread) =====
-        if (lane == 0) {
+        // ===== TMA producer (the warp stays converged; one elected lane issues) =====
+        {
             int s = 0;
             uint32_t ph = 0;
             for (int kt = 0; kt < KT; ++kt) {
                 mbar_wait_bounded(empty0 + 8 * s, ph ^ 1u);              // both CTAs have consumed this stage
                 const uint32_t fb = full0 + 8 * s;
                 const uint32_t dst = smem_base + s * TQ_STAGE_BYTES;
+                if (elect_one()) {
                 mbar_expect_tx(fb, TQ_STAGE_BYTES);                     // 2 x 8 KiB from me + 2 x 8 KiB from the peer + 32 KiB own
                 const int c0 = kt * TQ_BK;
                 // my half of the shared row panels, to both CTAs
@@ -141,12 +142,14 @@ sym_square_tf32_kernel(const __grid_constant__ CUtensorMap tmHi, const __grid_co
                 tma_load_2d(dst + 2 * TQ_PANEL_BYTES + TQ_HALF_BYTES, &tmHi, c0, J * TQ_BM + 64, fb);
                 tma_load_2d(dst + 3 * TQ_PANEL_BYTES, &tmLo, c0, J * TQ_BM, fb);
                 tma_load_2d(dst + 3 * TQ_PANEL_BYTES + TQ_HALF_BYTES, &tmLo, c0, J * TQ_BM + 64, fb);
+                }
+                __syncwarp();
                 if (++s == TQ_STAGES) { s = 0; ph ^= 1u; }
             }
         }
     } else if (warp == 1) {
-        // ===== MMA issuer (one thread): 3 tcgen05.mma per 8-wide k step =====
-        if (lane == 0) {
+        // ===== MMA issuer (converged warp, one elected lane): 3 tcgen05.mma per 8-wide k step =====
+        {
             constexpr uint32_t idesc = umma_idesc_tf32(TQ_BM, TQ_BM);
             int s = 0;
             uint32_t ph = 0;
@@ -165,6 +168,7 @@ sym_square_tf32_kernel(const __grid_constant__ CUtensorMap tmHi, const __grid_co
                 const uint64_t dBh = umma_desc_k128(a_hi + 2 * TQ_PANEL_BYTES);
                 const uint64_t dBl = umma_desc_k128(a_hi + 3 * TQ_PANEL_BYTES);
                 const uint32_t t_head = tmem + hb * TQ_BM, t_cross = tmem + 2 * TQ_BM;
+                if (elect_one()) {
 #pragma unroll
                 for (int ks = 0; ks < TQ_BK / TQ_UK; ++ks) {
                     const uint64_t o = (uint64_t)(ks * TQ_UK * 4 >> 4);      // 32 bytes per k step, in 16-byte units
@@ -174,6 +178,8 @@ sym_square_tf32_kernel(const __grid_constant__ CUtensorMap tmHi, const __grid_co
                 }
                 umma_commit_mc(empty0 + 8 * s, (uint16_t)3);   // frees the stage in BOTH CTAs' producers' view
                 if (kc == TQ_CHUNK_KT - 1 || kt == KT - 1) umma_commit(hfull0 + 8 * hb);   // chunk complete
+                }
+                __syncwarp();
                 if (++s == TQ_STAGES) { s = 0; ph ^= 1u; }
             }
         }
