@@ -73,7 +73,9 @@ sym_square_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     }
     __syncthreads();
 
-    // ===== TMA producer state (meaningful in lane 0 of warp 0 only) =====
+    // ===== TMA producer state (warp 0; the warp stays converged and one elected lane issues, so the TMA
+    //       operands live in uniform registers -- an `if (threadIdx.x == 0)` region costs an ELECT /
+    //       R2UR.BROADCAST loop in front of every UTMALDG) =====
     const uint32_t stage_bytes = two_panels ? 2 * SQ_PANEL_BYTES : SQ_PANEL_BYTES;
     int ld_kt = 0, ld_s = 0;
     uint32_t ld_ph = 0;
@@ -81,15 +83,18 @@ sym_square_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
         while (ld_kt < upto) {
             if (ld_kt >= SQ_STAGES && !mbar_test(empty0 + 8 * ld_s, ld_ph ^ 1u)) break;
             const uint32_t fb = full0 + 8 * ld_s;
-            mbar_expect_tx(fb, stage_bytes);
             const uint32_t dstA = smem_base + ld_s * (2 * SQ_PANEL_BYTES);
-            tma_load_2d(dstA, &tmA, ld_kt * SQ_BK, I * SQ_BM, fb);
-            if (two_panels) tma_load_2d(dstA + SQ_PANEL_BYTES, TWO_OP ? &tmB : &tmA, ld_kt * SQ_BK, J * SQ_BM, fb);
+            if (elect_one()) {
+                mbar_expect_tx(fb, stage_bytes);
+                tma_load_2d(dstA, &tmA, ld_kt * SQ_BK, I * SQ_BM, fb);
+                if (two_panels) tma_load_2d(dstA + SQ_PANEL_BYTES, TWO_OP ? &tmB : &tmA, ld_kt * SQ_BK, J * SQ_BM, fb);
+            }
+            __syncwarp();
             ++ld_kt;
             if (++ld_s == SQ_STAGES) { ld_s = 0; ld_ph ^= 1u; }
         }
     };
-    if (threadIdx.x == 0) issue_loads(min(KT, SQ_STAGES));
+    if (warp == 0) issue_loads(min(KT, SQ_STAGES));
     {
         // ===== consumers =====
         const int warp_m = warp >> 2;      // 0..1  -> 64 tile rows
@@ -136,8 +141,7 @@ sym_square_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
         uint32_t st = smem_base;
         load_frag(a0, b0, st + rowA, st + rowB, off[0]);
         for (int kt = 0; kt < KT; ++kt) {
-            if (threadIdx.x == 0) issue_loads(min(KT, kt + SQ_STAGES));
-            __syncwarp();
+            if (warp == 0) issue_loads(min(KT, kt + SQ_STAGES));
             const uint32_t aB = st + rowA, bB = st + rowB;
             int s1 = s + 1;
             uint32_t ph1 = ph;
