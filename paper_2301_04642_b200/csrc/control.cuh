@@ -61,10 +61,14 @@ bounds_reduce_kernel(const double* __restrict__ row_lo, const double* __restrict
 {
     __shared__ double slo[256], shi[256];
     double lo = INFINITY, hi = -INFINITY;
+    int bad = 0;                       // fmin / fmax drop NaNs: a non-finite H^p must not yield finite bounds
     for (int i = threadIdx.x; i < k; i += 256) {
-        lo = fmin(lo, row_lo[i]);
-        hi = fmax(hi, row_hi[i]);
+        const double a = row_lo[i], b = row_hi[i];
+        bad |= (a != a) | (b != b);
+        lo = fmin(lo, a);
+        hi = fmax(hi, b);
     }
+    bad = __syncthreads_or(bad);
     slo[threadIdx.x] = lo;
     shi[threadIdx.x] = hi;
     __syncthreads();
@@ -76,8 +80,8 @@ bounds_reduce_kernel(const double* __restrict__ row_lo, const double* __restrict
         __syncthreads();
     }
     if (threadIdx.x == 0) {
-        bounds[0] = slo[0];
-        bounds[1] = shi[0];
+        bounds[0] = bad ? NAN : slo[0];
+        bounds[1] = bad ? NAN : shi[0];
     }
 }
 

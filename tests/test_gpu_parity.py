@@ -228,6 +228,18 @@ def test_error_paths(handle):
     with pytest.raises(rfoe.RfoeError) as ei:
         rfoe.Rfoe(64).expand(torch.zeros(65, 65, dtype=torch.float64, device="cuda"), 3)
     assert ei.value.status == rfoe.ERR_INVALID_ARG
+    # empty input
+    empty = torch.empty((0, 0), dtype=torch.float64, device="cuda")
+    for call in (lambda: handle.expand(empty, 1, rfoe.SP2, 1e-12), lambda: handle.bounds(empty), lambda: handle.square(empty)):
+        with pytest.raises(rfoe.RfoeError) as ei:
+            call()
+        assert ei.value.status == rfoe.ERR_INVALID_ARG
+    # non-finite input: the bounds are not finite
+    Hnan = H.clone()
+    Hnan[2, 2] = float("nan")
+    with pytest.raises(rfoe.RfoeError) as ei:
+        handle.expand(Hnan, 10, rfoe.SP2, 1e-12)
+    assert ei.value.status == rfoe.ERR_BAD_BOUNDS        # (the bitwise symmetry check passes: same NaN pattern)
     # the handle is still usable after errors
     res = handle.expand(H, w.nocc, rfoe.SP2, w.tol)
     assert res.converged
