@@ -362,3 +362,16 @@ def test_expand_degenerate_fermi_level(handle):
     occ = np.sort(np.linalg.eigvalsh(P))
     assert np.sum((occ > 0.01) & (occ < 0.99)) >= 1            # fractional occupation survives
     assert np.allclose(res.t[:20], ref.t[:20], rtol=0, atol=1e-8)   # the trace-steered map is chaotic here: compare the head only
+
+
+def test_run_to_run_bitwise(handle):
+    """No FP atomics, fixed-order reductions: two runs give the same bits (P, traces, branch string), for the
+    FP64 path and for the reduced-precision path."""
+    w = rfoe_inputs.make_workload(4, k=515)
+    H = _dev(w.H)
+    for variant in (rfoe.SP2, rfoe.SP2_MIXED):
+        a = handle.expand(H, w.nocc, variant, w.tol)
+        Pa, ta, sa, ba = a.P.clone(), a.t.copy(), a.s.copy(), a.branch
+        b = handle.expand(H, w.nocc, variant, w.tol)
+        assert torch.equal(Pa, b.P) and np.array_equal(ta, b.t) and np.array_equal(sa, b.s) and ba == b.branch
+        assert a.tr_PH == b.tr_PH
