@@ -73,6 +73,10 @@ def lib():
             f = getattr(L, name)
             f.argtypes = [dp, dp, C.c_int64, dp]
             f.restype = None
+        for name in ("rfoe_oracle_project", "rfoe_oracle_project_full", "rfoe_oracle_apply", "rfoe_oracle_density"):
+            f = getattr(L, name)
+            f.argtypes = [dp, dp, C.c_int64, C.c_int64, C.c_int64, dp]
+            f.restype = None
         L.rfoe_oracle_is_symmetric.argtypes = [dp, C.c_int64]
         L.rfoe_oracle_is_symmetric.restype = C.c_int
         L.rfoe_oracle_expand.argtypes = [dp, C.c_int64, C.c_int64, C.POINTER(_Run), dp]
@@ -196,3 +200,41 @@ def square_entries(X, pairs):
             acc = acc + a * b
         out.append(acc)
     return np.array(out)
+
+
+def _rect(a) -> np.ndarray:
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    if a.ndim != 2:
+        raise ValueError("k x M FP64 matrix expected")
+    return a
+
+
+def project(Psi, HPsi, full: bool = False) -> np.ndarray:
+    """Rayleigh-Ritz step: H^p = Psi H Psi^T from Psi (k x M, one state per row) and HPsi
+    (row j = H applied to state j).  Upper triangle by the definition, mirrored; ``full`` = all k^2 sums."""
+    Psi, HPsi = _rect(Psi), _rect(HPsi)
+    k, M = Psi.shape
+    assert HPsi.shape == (k, M)
+    Hp = np.empty((k, k))
+    (lib().rfoe_oracle_project_full if full else lib().rfoe_oracle_project)(_p(Psi), _p(HPsi), k, M, M, _p(Hp))
+    return Hp
+
+
+def apply(P, Psi) -> np.ndarray:
+    """Y = P Psi (the subspace density matrix applied to the basis), j ascending."""
+    P, Psi = _sq(P), _rect(Psi)
+    k, M = Psi.shape
+    assert P.shape == (k, k)
+    Y = np.empty((k, M))
+    lib().rfoe_oracle_apply(_p(P), _p(Psi), k, M, M, _p(Y))
+    return Y
+
+
+def density(Psi, Y) -> np.ndarray:
+    """rho_m = sum_i Psi_im Y_im = diag(Psi^T P Psi), i ascending."""
+    Psi, Y = _rect(Psi), _rect(Y)
+    k, M = Psi.shape
+    assert Y.shape == (k, M)
+    rho = np.empty(M)
+    lib().rfoe_oracle_density(_p(Psi), _p(Y), k, M, M, _p(rho))
+    return rho

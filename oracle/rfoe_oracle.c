@@ -31,6 +31,8 @@
  * inputs; construction-exact projector Q_occ Q_occ^T; diagonal-H closed form (scalar recursion);
  * per-step invariants; scalar eigenvalue-space model for branch strings and iteration counts;
  * the paper's printed iteration counts on the paper's matrix.
+ * Rayleigh-Ritz / apply / density (NEXT-4): pinned by an invariant-subspace construction against an
+ * explicit eigendecomposition (numpy eigh and the Jacobi projector), sum rho = N_occ, and closed forms.
  * Not pinned: the exact bit patterns of X_n (the paper prints no worked example) -- "parity
  * unpinned" for bits, covered by tolerances.
  */
@@ -173,6 +175,65 @@ static void matmul_ilj(const double* A, const double* B, int64_t k, double* Y, i
 
 void rfoe_oracle_square(const double* X, int64_t k, double* Y) { matmul_ilj(X, X, k, Y, 1); }
 void rfoe_oracle_matmul(const double* A, const double* B, int64_t k, double* Y) { matmul_ilj(A, B, k, Y, 0); }
+
+/* ---- steps either side of the expansion (reading R-RR) --------------
+ * The paper's setting: "the discretized Kohn-Sham Hamiltonian matrix H of size M x M is
+ * orthogonally projected onto a carefully constructed subspace ... (Rayleigh-Ritz step), and subsequently,
+ * the resulting smaller dense projected Hamiltonian H^p of dimension k (<< M) is" handed to RFOE, which
+ * "approximate[s] the density matrix in the subspace".  The paper prints neither step; they are written
+ * here by their plain definitions for a basis stored one state per row (Psi: k x M, row pitch ld):
+ *   project : H^p = Psi H Psi^T, given HPsi = (H Psi^T)^T (k x M, row j = H applied to state j):
+ *             H^p_ij = sum_{m ascending} Psi_im * HPsi_jm for i <= j, then mirrored -- for symmetric H the
+ *             exact H^p is symmetric, and rfoe_expand needs it bitwise symmetric, so the upper triangle is
+ *             the definition (rfoe_oracle_project_full computes all k^2 sums for the pin that says so).
+ *   apply   : Y = P Psi,  Y_im = sum_{j ascending} P_ij * Psi_jm      (the subspace density matrix applied
+ *             to the basis; Psi^T Y is the density matrix in the full M-dimensional space)
+ *   density : rho_m = sum_{i ascending} Psi_im * Y_im = (Psi^T P Psi)_mm (its diagonal: the electron
+ *             density on the M degrees of freedom, per spin).  sum_m rho_m = Tr P = N_occ for orthonormal Psi. */
+void rfoe_oracle_project_full(const double* Psi, const double* HPsi, int64_t k, int64_t M, int64_t ld, double* Hp)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < k; ++i)
+        for (int64_t j = 0; j < k; ++j) {
+            double acc = 0.0;
+            for (int64_t m = 0; m < M; ++m) acc = acc + Psi[i * ld + m] * HPsi[j * ld + m];
+            Hp[i * k + j] = acc;
+        }
+}
+
+void rfoe_oracle_project(const double* Psi, const double* HPsi, int64_t k, int64_t M, int64_t ld, double* Hp)
+{
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int64_t i = 0; i < k; ++i)
+        for (int64_t j = i; j < k; ++j) {
+            double acc = 0.0;
+            for (int64_t m = 0; m < M; ++m) acc = acc + Psi[i * ld + m] * HPsi[j * ld + m];
+            Hp[i * k + j] = acc;
+        }
+    for (int64_t i = 1; i < k; ++i)
+        for (int64_t j = 0; j < i; ++j) Hp[i * k + j] = Hp[j * k + i];
+}
+
+void rfoe_oracle_apply(const double* P, const double* Psi, int64_t k, int64_t M, int64_t ld, double* Y)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < k; ++i) {
+        double* y = Y + i * ld;
+        for (int64_t m = 0; m < M; ++m) y[m] = 0.0;
+        for (int64_t j = 0; j < k; ++j) {          /* j ascending for every Y_im */
+            const double p = P[i * k + j];
+            const double* q = Psi + j * ld;
+            for (int64_t m = 0; m < M; ++m) y[m] = y[m] + p * q[m];
+        }
+    }
+}
+
+void rfoe_oracle_density(const double* Psi, const double* Y, int64_t k, int64_t M, int64_t ld, double* rho)
+{
+    for (int64_t m = 0; m < M; ++m) rho[m] = 0.0;
+    for (int64_t i = 0; i < k; ++i)                /* i ascending for every rho_m */
+        for (int64_t m = 0; m < M; ++m) rho[m] = rho[m] + Psi[i * ld + m] * Y[i * ld + m];
+}
 
 /* FP32 step of the mixed variant: X rounded to float, float products, float accumulation */
 static void square_f32(const double* X, int64_t k, double* Y, float* xf, float* yf)

@@ -23,7 +23,8 @@ from dataclasses import dataclass, field
 
 import numpy as np
 
-__all__ = ["CONFIGS", "Workload", "spectrum", "make_workload", "from_spectrum", "paper_matrix", "sha256"]
+__all__ = ["CONFIGS", "Workload", "spectrum", "make_workload", "from_spectrum", "paper_matrix", "sha256",
+           "Subspace", "make_subspace", "invariant_subspace"]
 
 
 @dataclass(frozen=True)
@@ -171,3 +172,78 @@ def sha256(H) -> str:
     if not isinstance(H, np.ndarray):
         H = H.detach().cpu().numpy()
     return hashlib.sha256(np.ascontiguousarray(H).tobytes()).hexdigest()
+
+
+# ---- inputs of the steps either side of the expansion (Rayleigh-Ritz before, P applied to the basis after) ----
+@dataclass
+class Subspace:
+    """A subspace basis and the action of H on it, one state per row (k x M, row-major, pitch M).
+    ``Psi`` has orthonormal rows; ``HPsi`` row j is H applied to state j; ``Psi @ HPsi.T`` equals the
+    projected Hamiltonian ``w.H`` of the underlying workload up to rounding.  numpy arrays or CUDA tensors."""
+    k: int
+    M: int
+    Psi: object
+    HPsi: object
+    w: Workload
+    H_full: object = None      # the M x M matrix, only for the tiny explicit construction
+
+
+def make_subspace(c: int, k: int, M: int, *, resid: float = 0.1, device: str = "cpu") -> Subspace:
+    """Synthetic Rayleigh-Ritz input with the structure of the paper's setting (a basis of
+    k states over M >> k degrees of freedom, H never formed densely).  Recipe: ``w`` = config ``c`` scaled to
+    k (spectrum, gap and nocc/k kept); Psi^T = thin QR of a seeded N(0,1) M x k matrix (seed 3000+c);
+    HPsi = w.H Psi + R with R a seeded N(0,1) k x M matrix (seed 4000+c) projected off span(Psi) twice and
+    scaled to ``resid`` x rms(w.H Psi) -- the part of H Psi that leaves the subspace, which the projection
+    must annihilate."""
+    w = make_workload(c, k=k, device="cpu" if device == "cpu" else device)
+    if device == "cpu":
+        A = np.random.default_rng(3000 + c).standard_normal((M, k))
+        Q, _ = np.linalg.qr(A)
+        Psi = np.ascontiguousarray(Q.T)
+        G = np.random.default_rng(4000 + c).standard_normal((k, M))
+        for _ in range(2):
+            G -= (G @ Psi.T) @ Psi
+        HP = np.asarray(w.H) @ Psi
+        G *= resid * np.sqrt(np.mean(HP * HP) / np.mean(G * G))
+        HPsi = np.ascontiguousarray(HP + G)
+    else:
+        import torch
+
+        g = torch.Generator(device=device)
+        g.manual_seed(3000 + c)
+        A = torch.randn((M, k), dtype=torch.float64, device=device, generator=g)
+        Q, _ = torch.linalg.qr(A)
+        del A
+        Psi = Q.T.contiguous()
+        del Q
+        g.manual_seed(4000 + c)
+        G = torch.randn((k, M), dtype=torch.float64, device=device, generator=g)
+        for _ in range(2):
+            G -= (G @ Psi.T) @ Psi
+        H = w.H if isinstance(w.H, torch.Tensor) else torch.from_numpy(w.H).to(device)
+        HP = H @ Psi
+        G *= resid * float(torch.sqrt(torch.mean(HP * HP) / torch.mean(G * G)))
+        HPsi = HP.add_(G).contiguous()
+        del G
+    return Subspace(k=k, M=M, Psi=Psi, HPsi=HPsi, w=w)
+
+
+def invariant_subspace(M: int, k: int, nocc: int, seed: int, *, gap: float = 0.3) -> Subspace:
+    """Tiny explicit instance: a full symmetric M x M matrix H_full = V diag(mu) V^T (mu ascending, a gap of
+    ``gap`` after the nocc-th value) and a basis Psi whose rows span the invariant subspace of its k lowest
+    eigenvectors, mixed by a seeded k x k rotation.  Everything downstream then has a plain definition through
+    an explicit eigendecomposition of H_full: H^p has the k lowest eigenvalues, and the density is
+    rho_m = sum_{i < nocc} V_mi^2."""
+    rng = np.random.default_rng(seed)
+    V = _haar_q_numpy(M, seed + 1)
+    lo = np.sort(rng.uniform(-1.0, -gap / 2, size=nocc))
+    hi = np.sort(rng.uniform(gap / 2, 2.0, size=M - nocc))
+    mu = np.concatenate([lo, hi])
+    H_full = (V * mu[None, :]) @ V.T
+    H_full = 0.5 * (H_full + H_full.T)
+    R = _haar_q_numpy(k, seed + 2)
+    Psi = np.ascontiguousarray(R @ V[:, :k].T)
+    HPsi = np.ascontiguousarray(Psi @ H_full)
+    w = Workload(name=f"invariant(M={M},k={k})", k=k, nocc=nocc, tol=1e-12, lam=mu[:k].copy(), H=None, Q=None,
+                 meta={"seed": seed, "V": V, "mu": mu})
+    return Subspace(k=k, M=M, Psi=Psi, HPsi=HPsi, w=w, H_full=H_full)
