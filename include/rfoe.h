@@ -142,6 +142,31 @@ int rfoe_square_reduced(rfoe_handle_t h, const double* X, int64_t k, double c2, 
 int rfoe_symm_product(rfoe_handle_t h, const double* A, const double* B, int64_t k, double c2, double c1, double c0,
                       double* Cout, double* scalars, float* kernel_ms, rfoe_stream_t stream);
 
+/* ---- steps either side of the expansion (sec. I, sec. III.A) -------------------
+ * The paper's setting: the M x M Kohn-Sham matrix H "is orthogonally projected onto a carefully constructed
+ * subspace ... (Rayleigh-Ritz step)", the resulting k x k H^p goes through the expansion above, which
+ * "approximate[s] the density matrix in the subspace".  Neither step is printed in the paper; both are taken by
+ * their plain definitions (reading R-RR) for a basis stored ONE STATE PER ROW:
+ *   Psi, HPsi, Y : device, k x M row-major FP64 with row pitch ld (ldy for Y) >= M doubles; ld even and the
+ *                  base 16-byte aligned (TMA pitch rule); 1 <= k <= k_max, 1 <= M <= 2^30 (rfoe_apply: M < 8.3e6).
+ *   Psi rows are the (orthonormal) subspace basis, row j of HPsi is H applied to state j (formed matrix-free by
+ *   the caller; H itself is never dense).  M need not be a multiple of anything: ragged tails are zero-filled. */
+
+/* Rayleigh-Ritz projection: Hp_ij = sum_m Psi_im HPsi_jm for i <= j, mirrored to j > i (exactly symmetric for a
+ * symmetric H; the mirror makes it bitwise symmetric, which rfoe_expand requires).  FP64 tensor cores, upper
+ * tiles only, the sum over M split into slices added in a fixed order (bitwise reproducible).
+ * Hp: device, k x k, ld = k, overwritten.  scalars (HOST, 2 doubles, may be null): Tr Hp, ||Hp||_F^2.
+ * kernel_ms (HOST, may be null): CUDA-event time of the product + slice reduction. */
+int rfoe_project(rfoe_handle_t h, const double* Psi, const double* HPsi, int64_t k, int64_t M, int64_t ld, double* Hp,
+                 double* scalars, float* kernel_ms, rfoe_stream_t stream);
+
+/* The subspace density matrix applied to the basis: Y = P Psi (Y_im = sum_j P_ij Psi_jm), and, when rho is not
+ * null, the diagonal of the full-space density matrix Psi^T P Psi: rho_m = sum_i Psi_im Y_im (device, M doubles;
+ * sum_m rho_m = Tr P = N_occ for an orthonormal basis).  P: device, k x k, ld = k (any k; it is copied into a
+ * padded work matrix of the handle).  Y must not overlap Psi.  kernel_ms: the product kernel alone. */
+int rfoe_apply(rfoe_handle_t h, const double* P, const double* Psi, int64_t k, int64_t M, int64_t ld, double* Y,
+               int64_t ldy, double* rho, float* kernel_ms, rfoe_stream_t stream);
+
 int rfoe_set_option(rfoe_handle_t h, int key, double value); /* INVALID_ARG on bad value, UNSUPPORTED on bad key */
 int rfoe_get_stats(rfoe_handle_t h, rfoe_stats_t* out);      /* copies the stats of the last call */
 int rfoe_destroy(rfoe_handle_t h);                           /* frees everything the handle owns; h may be null */

@@ -31,7 +31,7 @@ OK, ERR_INVALID_ARG, ERR_ALLOC, ERR_CUDA, ERR_BAD_BOUNDS, ERR_NOT_SYMMETRIC, ERR
 
 # every symbol include/rfoe.h declares
 EXPORTS = ("rfoe_create", "rfoe_bounds", "rfoe_expand", "rfoe_expand_host", "rfoe_square", "rfoe_square_reduced",
-           "rfoe_symm_product",
+           "rfoe_symm_product", "rfoe_project", "rfoe_apply",
            "rfoe_set_option", "rfoe_get_stats", "rfoe_destroy", "rfoe_strerror", "rfoe_version")
 
 
@@ -78,6 +78,8 @@ def load_library(path: str | None = None):
     L.rfoe_square.argtypes = [vp, vp, i64, dbl, dbl, dbl, vp, dp, C.POINTER(C.c_float), vp]
     L.rfoe_square_reduced.argtypes = [vp, vp, i64, dbl, dbl, dbl, vp, dp, C.POINTER(C.c_float), vp]
     L.rfoe_symm_product.argtypes = [vp, vp, vp, i64, dbl, dbl, dbl, vp, dp, C.POINTER(C.c_float), vp]
+    L.rfoe_project.argtypes = [vp, vp, vp, i64, i64, i64, vp, dp, C.POINTER(C.c_float), vp]
+    L.rfoe_apply.argtypes = [vp, vp, vp, i64, i64, i64, vp, i64, vp, C.POINTER(C.c_float), vp]
     L.rfoe_set_option.argtypes = [vp, C.c_int, dbl]
     L.rfoe_get_stats.argtypes = [vp, C.POINTER(_Stats)]
     L.rfoe_destroy.argtypes = [vp]
@@ -128,6 +130,14 @@ def _check_dev(x, name):
     if not (isinstance(x, torch.Tensor) and x.is_cuda and x.dtype == torch.float64 and x.dim() == 2
             and x.shape[0] == x.shape[1] and x.is_contiguous()):
         raise ValueError(f"{name}: contiguous square float64 CUDA tensor expected")
+
+
+def _check_rect(x, name):
+    import torch
+
+    if not (isinstance(x, torch.Tensor) and x.is_cuda and x.dtype == torch.float64 and x.dim() == 2 and x.stride(1) == 1
+            and x.stride(0) >= x.shape[1]):
+        raise ValueError(f"{name}: row-major float64 CUDA matrix (k x M, unit column stride) expected")
 
 
 class Rfoe:
@@ -261,3 +271,42 @@ class Rfoe:
         if rc != OK:
             self._raise(rc)
         return out, np.array(sc[:]), ms.value
+
+    def project(self, Psi, HPsi, out=None, stream=None):
+        """Rayleigh-Ritz step: Hp = Psi HPsi^T (upper triangle mirrored); returns (Hp, (Tr Hp, ||Hp||_F^2), kernel_ms)."""
+        import torch
+
+        _check_rect(Psi, "Psi")
+        _check_rect(HPsi, "HPsi")
+        if HPsi.shape != Psi.shape or HPsi.stride(0) != Psi.stride(0):
+            raise ValueError("Psi and HPsi must have the same shape and row pitch")
+        k, M = Psi.shape
+        out = torch.empty((k, k), dtype=torch.float64, device=Psi.device) if out is None else out
+        _check_dev(out, "Hp")
+        sc = (C.c_double * 2)()
+        ms = C.c_float()
+        rc = self._L.rfoe_project(self._h, C.c_void_p(Psi.data_ptr()), C.c_void_p(HPsi.data_ptr()), k, M, Psi.stride(0),
+                                  C.c_void_p(out.data_ptr()), sc, C.byref(ms), _stream_ptr(stream))
+        if rc != OK:
+            self._raise(rc)
+        return out, (sc[0], sc[1]), ms.value
+
+    def apply(self, P, Psi, out=None, density=True, stream=None):
+        """Y = P Psi and (density=True) rho_m = sum_i Psi_im Y_im; returns (Y, rho or None, kernel_ms)."""
+        import torch
+
+        _check_dev(P, "P")
+        _check_rect(Psi, "Psi")
+        k, M = Psi.shape
+        if P.shape[0] != k:
+            raise ValueError("P must be k x k with k = Psi.shape[0]")
+        out = torch.empty((k, M), dtype=torch.float64, device=Psi.device) if out is None else out
+        _check_rect(out, "Y")
+        rho = torch.empty((M,), dtype=torch.float64, device=Psi.device) if density else None
+        ms = C.c_float()
+        rc = self._L.rfoe_apply(self._h, C.c_void_p(P.data_ptr()), C.c_void_p(Psi.data_ptr()), k, M, Psi.stride(0),
+                                C.c_void_p(out.data_ptr()), out.stride(0), C.c_void_p(rho.data_ptr() if density else None),
+                                C.byref(ms), _stream_ptr(stream))
+        if rc != OK:
+            self._raise(rc)
+        return out, rho, ms.value

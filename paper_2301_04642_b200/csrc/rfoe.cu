@@ -13,6 +13,7 @@
 #include "../../include/rfoe.h"
 #include "control.cuh"
 #include "hbm_kernels.cuh"
+#include "subspace.cuh"
 #include "sym_square.cuh"
 #include "sym_square_tf32.cuh"
 
@@ -52,6 +53,8 @@ struct rfoe_handle_s {
     int n_tiles = 0;
     HostPage* hp = nullptr;
     int* d_word = nullptr; // device alias of hp->word
+    double* ws = nullptr;      // scratch of the projection / density steps (grown on demand)
+    size_t ws_bytes = 0;
     double* stage_H = nullptr;
     double* stage_P = nullptr;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
@@ -181,7 +184,8 @@ template <bool TWO_OP>
 static cudaError_t launch_square(rfoe_handle_s* h, const CUtensorMap& a, const CUtensorMap& b, const double* E, double* Out,
                                  int n, int ld, int k, const StepCoef* coef, double* partials, cudaStream_t st)
 {
-    sym_square_kernel<TWO_OP><<<h->n_tiles, SQ_THREADS, SQ_SMEM_BYTES, st>>>(a, b, E, Out, n, ld, k, coef, h->d_tiles, partials);
+    sym_square_kernel<TWO_OP ? 1 : 0><<<h->n_tiles, SQ_THREADS, SQ_SMEM_BYTES, st>>>(a, b, E, Out, n / SQ_BK, n / SQ_BK, ld, k, coef,
+                                                                                 h->d_tiles, partials);
     h->launches++;
     return cudaGetLastError();
 }
@@ -227,7 +231,7 @@ extern "C" int rfoe_destroy(rfoe_handle_t h)
     for (double* p : h->rows) cudaFree(p);
     cudaFree(h->d_bounds); cudaFree(h->d_scalars); cudaFree(h->d_flag); cudaFree(h->d_ctrl); cudaFree(h->d_tiles);
     cudaFree(h->d_pairs);
-    cudaFree(h->stage_H); cudaFree(h->stage_P);
+    cudaFree(h->stage_H); cudaFree(h->stage_P); cudaFree(h->ws);
     if (h->hp) cudaFreeHost(h->hp);
     if (h->ev0) cudaEventDestroy(h->ev0);
     if (h->ev1) cudaEventDestroy(h->ev1);
@@ -281,8 +285,10 @@ extern "C" int rfoe_create(rfoe_handle_t* out, int device, int64_t k_max)
         return RFOE_ERR_CUDA;
     }
     h->encode = (EncodeTiledFn)fn;
-    if (cudaFuncSetAttribute(sym_square_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SQ_SMEM_BYTES) != cudaSuccess ||
-        cudaFuncSetAttribute(sym_square_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SQ_SMEM_BYTES) != cudaSuccess ||
+    if (cudaFuncSetAttribute(sym_square_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, SQ_SMEM_BYTES) != cudaSuccess ||
+        cudaFuncSetAttribute(sym_square_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, SQ_SMEM_BYTES) != cudaSuccess ||
+        cudaFuncSetAttribute(sym_square_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, SQ_SMEM_BYTES) != cudaSuccess ||
+        cudaFuncSetAttribute(apply_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, AP_SMEM_BYTES) != cudaSuccess ||
         cudaFuncSetAttribute(sym_square_tf32_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TQ_SMEM_BYTES) != cudaSuccess) {
         rfoe_destroy(h);
         return RFOE_ERR_CUDA;
@@ -591,6 +597,147 @@ extern "C" int rfoe_symm_product(rfoe_handle_t h, const double* A, const double*
 {
     if (!B) return RFOE_ERR_INVALID_ARG;
     return single_product(h, A, B, k, c2, c1, c0, Cout, scalars, kernel_ms, (cudaStream_t)stream);
+}
+
+// ---------------------------------------------------------------------------------------------
+// steps either side of the expansion (NEXT-4): Rayleigh-Ritz projection before, P applied to the basis after
+static int make_map_rect(rfoe_handle_s* h, CUtensorMap* map, const double* base, int64_t M, int64_t k, int64_t ld, int box_rows)
+{
+    cuuint64_t dims[2] = {(cuuint64_t)M, (cuuint64_t)k};
+    cuuint64_t strides[1] = {(cuuint64_t)ld * sizeof(double)};
+    cuuint32_t box[2] = {(cuuint32_t)SQ_BK, (cuuint32_t)box_rows};
+    cuuint32_t estr[2] = {1, 1};
+    CUresult r = h->encode(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<double*>(base), dims, strides, box, estr,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);   // out-of-range rows / columns read as zero
+    if (r != CUDA_SUCCESS) {
+        h->stats.cuda_error = (int)cudaErrorInvalidValue;
+        return RFOE_ERR_CUDA;
+    }
+    return RFOE_OK;
+}
+
+static int ensure_ws(rfoe_handle_s* h, size_t bytes)
+{
+    if (h->ws_bytes >= bytes) return RFOE_OK;
+    if (h->ws) { cudaFree(h->ws); h->ws = nullptr; h->ws_bytes = 0; }
+    if (cudaMalloc(&h->ws, bytes) != cudaSuccess) { cudaGetLastError(); return RFOE_ERR_ALLOC; }
+    h->ws_bytes = bytes;
+    return RFOE_OK;
+}
+
+static bool rect_args_ok(const rfoe_handle_s* h, const void* a, int64_t k, int64_t M, int64_t ld)
+{
+    return a && k >= 1 && k <= h->k_max && M >= 1 && M <= (int64_t)1 << 30 && ld >= M && (ld & 1) == 0 &&
+           (reinterpret_cast<uintptr_t>(a) & 15) == 0;
+}
+
+// number of K-slices: the smallest S <= 16 whose tiles x slices fill the SMs to >= 97 % in whole waves (else the best)
+static void choose_slices(int n_tiles, int kt_total, int sm_count, int* n_slices, int* kt_per)
+{
+    int best_s = 1, best_per = kt_total;
+    double best_e = -1.0;
+    for (int s = 1; s <= 16; ++s) {
+        const int per = (kt_total + s - 1) / s;
+        if (s > 1 && per < 32) break;
+        const int eff_s = (kt_total + per - 1) / per;
+        const long long units = (long long)n_tiles * eff_s;
+        const long long waves = (units + sm_count - 1) / sm_count;
+        const double e = (double)units / (double)(waves * sm_count);
+        if (e > best_e + 1e-12) { best_e = e; best_s = eff_s; best_per = per; }
+        if (e >= 0.97) break;
+    }
+    *n_slices = best_s;
+    *kt_per = best_per;
+}
+
+extern "C" int rfoe_project(rfoe_handle_t h, const double* Psi, const double* HPsi, int64_t k64, int64_t M, int64_t ld,
+                            double* Hp, double* scalars, float* kernel_ms, rfoe_stream_t stream)
+{
+    if (!h || !Hp || !rect_args_ok(h, Psi, k64, M, ld) || !rect_args_ok(h, HPsi, k64, M, ld)) return RFOE_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int k = (int)k64, n = round_up(k, SQ_BM), m = n / SQ_BM;
+    int rc;
+    h->launches = 0;
+    h->stats.cuda_error = 0;
+    CK(cudaSetDevice(h->device));
+    if ((rc = ensure_tiles(h, m, st)) != RFOE_OK) return rc;
+    const int kt_total = (int)((M + SQ_BK - 1) / SQ_BK);
+    int n_slices, kt_per;
+    choose_slices(h->n_tiles, kt_total, h->sm_count, &n_slices, &kt_per);
+    if ((rc = ensure_ws(h, (size_t)n_slices * h->n_tiles * SQ_BM * SQ_BM * sizeof(double))) != RFOE_OK) return rc;
+    CUtensorMap tmA, tmB;
+    if ((rc = make_map_rect(h, &tmA, Psi, M, k, ld, SQ_BM)) != RFOE_OK) return rc;
+    if ((rc = make_map_rect(h, &tmB, HPsi, M, k, ld, SQ_BM)) != RFOE_OK) return rc;
+    CK(cudaEventRecord(h->ev0, st));
+    sym_square_kernel<2><<<dim3(h->n_tiles, n_slices), SQ_THREADS, SQ_SMEM_BYTES, st>>>(tmA, tmB, nullptr, h->ws, kt_total, kt_per, SQ_BM, k,
+                                                                                      nullptr, h->d_tiles, nullptr);
+    h->launches++;
+    CK(cudaGetLastError());
+    project_reduce_kernel<<<h->n_tiles, 256, 0, st>>>(h->ws, n_slices, h->n_tiles, h->d_tiles, k, Hp, h->part[0]);
+    h->launches++;
+    CK(cudaGetLastError());
+    CK(cudaEventRecord(h->ev1, st));
+    sum_partials_kernel<<<1, 256, 0, st>>>(h->part[0], h->n_tiles, h->d_scalars);
+    h->launches++;
+    CK(cudaGetLastError());
+    CK(cudaMemcpyAsync((void*)h->hp->scalars, h->d_scalars, 5 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    if (scalars) { scalars[0] = h->hp->scalars[0]; scalars[1] = h->hp->scalars[1]; }
+    if (kernel_ms) CK(cudaEventElapsedTime(kernel_ms, h->ev0, h->ev1));
+    h->stats.gpu_launches = h->launches;
+    h->stats.status = RFOE_OK;
+    return RFOE_OK;
+}
+
+extern "C" int rfoe_apply(rfoe_handle_t h, const double* P, const double* Psi, int64_t k64, int64_t M, int64_t ld, double* Y,
+                          int64_t ldy, double* rho, float* kernel_ms, rfoe_stream_t stream)
+{
+    if (!h || !P || !Y || !rect_args_ok(h, Psi, k64, M, ld) || ldy < M) return RFOE_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int k = (int)k64, n = round_up(k, SQ_BM), ldw = n + SQ_PAD, m = n / SQ_BM;
+    const int64_t tiles_m = (M + AP_BN - 1) / AP_BN;
+    if (tiles_m > 65535) return RFOE_ERR_INVALID_ARG;
+    int rc;
+    h->launches = 0;
+    h->stats.cuda_error = 0;
+    CK(cudaSetDevice(h->device));
+    CUtensorMap tmP, tmPsi;
+    if ((rc = make_map(h, &tmP, h->W[0], n, ldw)) != RFOE_OK) return rc;
+    if ((rc = make_map_rect(h, &tmPsi, Psi, M, k, ld, SQ_BK)) != RFOE_OK) return rc;
+    int n_slices = 1, rows_per = k;
+    const int64_t col_blocks = (M + 255) / 256;
+    if (rho) {
+        int64_t want = (h->sm_count * 8 + col_blocks - 1) / col_blocks;
+        if (want > 64) want = 64;
+        if (want > k) want = k;
+        if (want < 1) want = 1;
+        rows_per = (int)((k + want - 1) / want);
+        n_slices = (k + rows_per - 1) / rows_per;
+        if ((rc = ensure_ws(h, (size_t)n_slices * (size_t)M * sizeof(double))) != RFOE_OK) return rc;
+    }
+    pad_copy_kernel<<<hbm_grid(h, n), HBM_THREADS, 0, st>>>(P, k, n, ldw, h->W[0]);
+    h->launches++;
+    CK(cudaGetLastError());
+    const int vec_ok = ((ldy & 1) == 0) && ((reinterpret_cast<uintptr_t>(Y) & 15) == 0);
+    CK(cudaEventRecord(h->ev0, st));
+    apply_kernel<<<dim3(m, (unsigned)tiles_m), SQ_THREADS, AP_SMEM_BYTES, st>>>(tmP, tmPsi, Y, k, (long long)M, (long long)ldy, n / SQ_BK, vec_ok);
+    h->launches++;
+    CK(cudaGetLastError());
+    CK(cudaEventRecord(h->ev1, st));
+    if (rho) {
+        density_partial_kernel<<<dim3((unsigned)col_blocks, n_slices), 256, 0, st>>>(Psi, (long long)ld, Y, (long long)ldy, k, (long long)M,
+                                                                                   rows_per, h->ws);
+        h->launches++;
+        density_reduce_kernel<<<(unsigned)col_blocks, 256, 0, st>>>(h->ws, n_slices, (long long)M, rho);
+        h->launches++;
+        CK(cudaGetLastError());
+    }
+    CK(cudaStreamSynchronize(st));
+    if (kernel_ms) CK(cudaEventElapsedTime(kernel_ms, h->ev0, h->ev1));
+    h->stats.gpu_launches = h->launches;
+    h->stats.status = RFOE_OK;
+    return RFOE_OK;
 }
 
 // ---------------------------------------------------------------------------------------------

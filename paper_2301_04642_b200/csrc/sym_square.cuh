@@ -36,13 +36,20 @@ struct StepCoef {
     double c2, c1, c0;
 };
 
-template <bool TWO_OP>
+// MODE 0: squaring (A = B = X_n, one tensor map).  MODE 1: symmetric product of two matrices (McWeeny).
+// MODE 2: Rayleigh-Ritz projection H^p = Psi HPsi^T: the contraction runs over the M degrees
+//         of freedom (kt_total chunks of 16, ragged tail zero-filled by TMA), split into gridDim.y slices of
+//         kt_per_slice chunks so that tiles x slices fills the 148 SMs evenly; the raw 128 x 128 accumulators go
+//         to a tile-contiguous workspace, Out + (slice * gridDim.x + tile) * 128 * 128, and
+//         project_reduce_kernel (subspace.cuh) adds the slices in a fixed order and mirrors.
+template <int MODE>
 __global__ void __launch_bounds__(SQ_THREADS, 1)
 sym_square_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
-                  const double* __restrict__ E, double* __restrict__ Out, int n, int ld, int kvalid,
+                  const double* __restrict__ E, double* __restrict__ Out, int kt_total, int kt_per_slice, int ld, int kvalid,
                   const StepCoef* __restrict__ coef, const int2* __restrict__ tile_map,
                   double* __restrict__ partials)
 {
+    constexpr bool TWO_OP = (MODE != 0);
     extern __shared__ uint8_t smem_raw[];
     __shared__ __align__(8) uint64_t full_bar[SQ_STAGES];
     __shared__ __align__(8) uint64_t empty_bar[SQ_STAGES];
@@ -54,7 +61,8 @@ sym_square_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     const int I = tile.x, J = tile.y;
     const bool diag = (I == J);
     const bool two_panels = TWO_OP || !diag;
-    const int KT = n / SQ_BK;
+    const int kt0 = (MODE == 2) ? (int)blockIdx.y * kt_per_slice : 0;
+    const int KT = (MODE == 2) ? min(kt_per_slice, kt_total - kt0) : kt_total;
 
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     const uint32_t full0 = smem_u32(&full_bar[0]);
@@ -86,8 +94,8 @@ sym_square_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
             const uint32_t dstA = smem_base + ld_s * (2 * SQ_PANEL_BYTES);
             if (elect_one()) {
                 mbar_expect_tx(fb, stage_bytes);
-                tma_load_2d(dstA, &tmA, ld_kt * SQ_BK, I * SQ_BM, fb);
-                if (two_panels) tma_load_2d(dstA + SQ_PANEL_BYTES, TWO_OP ? &tmB : &tmA, ld_kt * SQ_BK, J * SQ_BM, fb);
+                tma_load_2d(dstA, &tmA, (kt0 + ld_kt) * SQ_BK, I * SQ_BM, fb);
+                if (two_panels) tma_load_2d(dstA + SQ_PANEL_BYTES, TWO_OP ? &tmB : &tmA, (kt0 + ld_kt) * SQ_BK, J * SQ_BM, fb);
             }
             __syncwarp();
             ++ld_kt;
@@ -162,6 +170,21 @@ sym_square_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
             s = s1; ph = ph1; st = stn;
         }
 
+        if (MODE == 2) {
+            // raw accumulators -> tile-contiguous workspace (row pitch 128); no update, no mirror, no partials
+            double* T = Out + ((size_t)blockIdx.y * gridDim.x + blockIdx.x) * (size_t)(SQ_BM * SQ_BM);
+#pragma unroll
+            for (int mi = 0; mi < 8; ++mi) {
+                const int row = warp_m * 64 + 2 * r + 16 * (mi >> 1) + (mi & 1);
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    const int col = warp_n * 32 + 4 * kk + 16 * h;
+                    *reinterpret_cast<double2*>(T + row * SQ_BM + col) = make_double2(acc[mi][2 * h][0], acc[mi][2 * h + 1][0]);
+                    *reinterpret_cast<double2*>(T + row * SQ_BM + col + 2) = make_double2(acc[mi][2 * h][1], acc[mi][2 * h + 1][1]);
+                }
+            }
+            return;
+        }
         // ===== fused epilogue =====
         const double c2 = coef->c2, c1 = coef->c1, c0 = coef->c0;
         double p_tr = 0.0, p_ss = 0.0, p_err = 0.0, p_trc = 0.0, p_ce = 0.0;
