@@ -184,8 +184,7 @@ template <bool TWO_OP>
 static cudaError_t launch_square(rfoe_handle_s* h, const CUtensorMap& a, const CUtensorMap& b, const double* E, double* Out,
                                  int n, int ld, int k, const StepCoef* coef, double* partials, cudaStream_t st)
 {
-    sym_square_kernel<TWO_OP ? 1 : 0><<<h->n_tiles, SQ_THREADS, SQ_SMEM_BYTES, st>>>(a, b, E, Out, n / SQ_BK, n / SQ_BK, ld, k, coef,
-                                                                                 h->d_tiles, partials);
+    sym_square_kernel<TWO_OP ? 1 : 0><<<h->n_tiles, SQ_THREADS, SQ_SMEM_BYTES, st>>>(a, b, E, Out, n, ld, k, coef, h->d_tiles, partials, 0);
     h->launches++;
     return cudaGetLastError();
 }
@@ -632,7 +631,7 @@ static bool rect_args_ok(const rfoe_handle_s* h, const void* a, int64_t k, int64
            (reinterpret_cast<uintptr_t>(a) & 15) == 0;
 }
 
-// number of K-slices: the smallest S <= 16 whose tiles x slices fill the SMs to >= 97 % in whole waves (else the best)
+// number of K-slices: the smallest S <= 16 whose tiles x slices fill the SMs to >= 99 % in whole waves (else the best)
 static void choose_slices(int n_tiles, int kt_total, int sm_count, int* n_slices, int* kt_per)
 {
     int best_s = 1, best_per = kt_total;
@@ -645,7 +644,7 @@ static void choose_slices(int n_tiles, int kt_total, int sm_count, int* n_slices
         const long long waves = (units + sm_count - 1) / sm_count;
         const double e = (double)units / (double)(waves * sm_count);
         if (e > best_e + 1e-12) { best_e = e; best_s = eff_s; best_per = per; }
-        if (e >= 0.97) break;
+        if (e >= 0.99) break;
     }
     *n_slices = best_s;
     *kt_per = best_per;
@@ -670,8 +669,8 @@ extern "C" int rfoe_project(rfoe_handle_t h, const double* Psi, const double* HP
     if ((rc = make_map_rect(h, &tmA, Psi, M, k, ld, SQ_BM)) != RFOE_OK) return rc;
     if ((rc = make_map_rect(h, &tmB, HPsi, M, k, ld, SQ_BM)) != RFOE_OK) return rc;
     CK(cudaEventRecord(h->ev0, st));
-    sym_square_kernel<2><<<dim3(h->n_tiles, n_slices), SQ_THREADS, SQ_SMEM_BYTES, st>>>(tmA, tmB, nullptr, h->ws, kt_total, kt_per, SQ_BM, k,
-                                                                                      nullptr, h->d_tiles, nullptr);
+    sym_square_kernel<2><<<dim3(h->n_tiles, n_slices), SQ_THREADS, SQ_SMEM_BYTES, st>>>(tmA, tmB, nullptr, h->ws, kt_total * SQ_BK, SQ_BM, k,
+                                                                                      nullptr, h->d_tiles, nullptr, kt_per);
     h->launches++;
     CK(cudaGetLastError());
     project_reduce_kernel<<<h->n_tiles, 256, 0, st>>>(h->ws, n_slices, h->n_tiles, h->d_tiles, k, Hp, h->part[0]);
