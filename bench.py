@@ -296,6 +296,10 @@ def run_ours(args) -> int:
         }
         if want_reduced:
             line["reduced_precision"] = reduced_report(h, rfoe, w, H, P, stream, ms_total / args.steps)
+        if world == 1 and not args.no_subspace:
+            del Hh, Ph
+            with rfoe.Rfoe(args.subspace_k, device=local) as h2:
+                line["subspace_steps"] = subspace_report(h2, rfoe, rfoe_inputs, args, dev, stream)
         if world == 1 and not args.no_cpu_baseline:
             dt, fl, its, ws = oracle_sample(args.config, args.cpu_k)
             line["cpu_baseline"] = {
@@ -352,6 +356,57 @@ def reduced_report(h, rfoe, w, H, P, stream, fp64_ms):
             "tolerances": {"errP": 1e-6, "band_energy": 1e-8}, "late_switch": late}
 
 
+def subspace_report(h, rfoe, rfoe_inputs, args, dev, stream):
+    """SURVEY.md 8(f) NEXT-4, reported separately from the headline: the steps either side of the expansion on a
+    synthetic Rayleigh-Ritz input with the paper's proportions (N is 0.1-0.5 % of M; the subspace is
+    ~1.3 N): the config's spectrum scaled to k = 4096 (nocc = 3150), M = 600000 degrees of freedom.
+    rfoe_project (H^p = Psi HPsi^T) -> rfoe_expand -> rfoe_apply (Y = P Psi, rho = diag(Psi^T P Psi)), each timed
+    with CUDA events on the launching stream; checks against the generator's own closed forms (harness algebra)."""
+    import torch
+
+    k, M = args.subspace_k, args.subspace_m
+    sub = rfoe_inputs.make_subspace(args.config, k=k, M=M, device=str(dev))
+    w = sub.w
+    Hp = torch.empty((k, k), dtype=torch.float64, device=dev)
+    P = torch.empty_like(Hp)
+    Y = torch.empty_like(sub.Psi)
+    m = (k + TILE - 1) // TILE
+    fl_proj = 2.0 * M * (m * (m + 1) // 2) * TILE * TILE            # executed: upper tiles only
+    fl_apply = 2.0 * M * float(m * TILE) ** 2                        # executed: P zero-padded to tiles
+    out = {"workload": f"config {args.config} spectrum scaled to k={k}, nocc={w.nocc}; M={M} (nocc/M = {100.0 * w.nocc / M:.2f} %); "
+                       "Psi = thin QR of seeded N(0,1), HPsi = H^p Psi + 10 % out-of-subspace residual",
+           "bytes_resident": 3 * 8 * k * M}
+    ms_p = ms_a = tot_e = None
+    for it in range(2):                                              # first pass warms up (workspaces, tile maps)
+        e = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+        torch.cuda.synchronize()
+        e[0].record(stream)
+        _, (tr, ss), ms_p = h.project(sub.Psi, sub.HPsi, out=Hp, stream=stream)
+        e[1].record(stream)
+        res = h.expand(Hp, w.nocc, rfoe.SP2, w.tol, P=P, stream=stream)
+        e[2].record(stream)
+        _, rho, ms_a = h.apply(P, sub.Psi, out=Y, density=True, stream=stream)
+        e[3].record(stream)
+        torch.cuda.synchronize()
+        tot_p, tot_e, tot_a = e[0].elapsed_time(e[1]), e[1].elapsed_time(e[2]), e[2].elapsed_time(e[3])
+    Hw = w.H if isinstance(w.H, torch.Tensor) else torch.from_numpy(w.H).to(dev)
+    Q = w.Q if isinstance(w.Q, torch.Tensor) else torch.from_numpy(w.Q).to(dev)
+    Qo = Q[:, : w.nocc]
+    rho_exact = ((Qo.T @ sub.Psi) ** 2).sum(dim=0)
+    out.update({
+        "project": {"kernel": "sym_square_kernel<2> + project_reduce_kernel", "ms": ms_p, "ms_call": tot_p,
+                    "tflops_executed": fl_proj / ms_p / 1e9, "frac_fp64_peak": fl_proj / ms_p / 1e9 / FP64_PEAK_TFLOPS,
+                    "max_abs_err_vs_construction": float((Hp - Hw).abs().max()), "bitwise_symmetric": bool(torch.equal(Hp, Hp.T))},
+        "expand": {"ms": tot_e, "iterations": res.iterations, "converged": bool(res.converged)},
+        "apply": {"kernel": "apply_kernel (+ density kernels in ms_call)", "ms": ms_a, "ms_call": tot_a,
+                  "tflops_executed": fl_apply / ms_a / 1e9, "frac_fp64_peak": fl_apply / ms_a / 1e9 / FP64_PEAK_TFLOPS,
+                  "electron_count_error": abs(float(rho.sum()) - w.nocc),
+                  "max_abs_density_err_vs_construction": float((rho - rho_exact).abs().max())},
+        "seconds_chain": (tot_p + tot_e + tot_a) / 1e3,
+    })
+    return out
+
+
 def main() -> int:
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -362,6 +417,9 @@ def main() -> int:
     ap.add_argument("--cpu-k", type=int, default=2048, help="size of the oracle's bounded sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-reduced", action="store_true", help="skip the separately reported reduced-precision run")
+    ap.add_argument("--no-subspace", action="store_true", help="skip the separately reported Rayleigh-Ritz / apply steps")
+    ap.add_argument("--subspace-k", type=int, default=4096)
+    ap.add_argument("--subspace-m", type=int, default=600000)
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         print("bench.py: note: fewer than 3 warm-up steps", file=sys.stderr)
