@@ -212,6 +212,12 @@ def run_ours(args) -> int:
             dist.barrier(device_ids=[local])
         torch.cuda.synchronize()
 
+    if args.only_subspace:          # profiling aid: only the separately reported NEXT-4 chain, one JSON line
+        if rank == 0:
+            with rfoe.Rfoe(args.subspace_k, device=local) as h2:
+                print(json.dumps({"subspace_steps": subspace_report(h2, rfoe, rfoe_inputs, args, dev, torch.cuda.current_stream())}),
+                      flush=True)
+        return 0
     cfg = rfoe_inputs.CONFIGS[args.config]
     # every rank owns an independent problem of the same configuration (replicas; no data-path collective)
     want_reduced = (world == 1 and not args.no_reduced)
@@ -418,6 +424,7 @@ def main() -> int:
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-reduced", action="store_true", help="skip the separately reported reduced-precision run")
     ap.add_argument("--no-subspace", action="store_true", help="skip the separately reported Rayleigh-Ritz / apply steps")
+    ap.add_argument("--only-subspace", action="store_true", help="run only the Rayleigh-Ritz / apply chain (ncu captures)")
     ap.add_argument("--subspace-k", type=int, default=4096)
     ap.add_argument("--subspace-m", type=int, default=600000)
     args = ap.parse_args()
