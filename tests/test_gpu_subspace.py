@@ -8,7 +8,7 @@ import numpy as np
 import pytest
 import torch
 
-import oracle
+import oracle  # noqa: F401
 import paper_2301_04642_b200 as rfoe
 import rfoe_inputs
 
@@ -121,3 +121,53 @@ def test_bad_arguments(handle):
     big = torch.zeros((2048, 4), dtype=torch.float64, device="cuda")    # k > k_max
     with pytest.raises(rfoe.RfoeError):
         handle.project(big, big.clone())
+
+
+def _dot_by_definition(a, b):
+    """sum_l a_l b_l, l ascending, one IEEE product and one IEEE sum at a time (Python floats)."""
+    acc = 0.0
+    for x, y in zip(a.tolist(), b.tolist()):
+        acc = acc + x * y
+    return acc
+
+
+def test_fullsize_chain_bench_configuration():
+    """The workload bench.py's `subspace_steps` times (config 4 spectrum at k=4096, nocc=3150, M=600000; the launch
+    configuration is the same: 528 tiles x 7 K-slices, 32 x 4688 apply tiles).  The naive oracle cannot run 2 M k^2
+    flops here, so: sampled entries of H^p and Y computed one by one by the definition (every tile class, the
+    ragged last column block, mirrored entries), and properties that hold at any size -- H^p equals the
+    generator's target matrix, bitwise symmetry, electron count, the construction-exact density."""
+    k, M = 4096, 600000
+    sub = rfoe_inputs.make_subspace(4, k=k, M=M, device="cuda")
+    w = sub.w
+    rng = np.random.default_rng(44)
+    with rfoe.Rfoe(k) as h:
+        Hp, (tr, ss), _ = h.project(sub.Psi, sub.HPsi)
+        assert torch.equal(Hp, Hp.T)
+        Hw = w.H if isinstance(w.H, torch.Tensor) else torch.from_numpy(w.H).cuda()
+        assert float((Hp - Hw).abs().max()) <= 1e-13                 # Psi HPsi^T = target H^p by construction
+        assert tr == pytest.approx(float(w.lam.sum()), abs=1e-9)
+        pairs = [(0, 0), (k - 1, k - 1), (0, k - 1), (k - 1, 0), (130, 129), (129, 130), (2047, 2048), (4000, 77)]
+        pairs += [tuple(rng.integers(0, k, size=2).tolist()) for _ in range(6)]
+        amax = float(sub.Psi.abs().max()) * float(sub.HPsi.abs().max())
+        for i, j in pairs:
+            a, b = min(i, j), max(i, j)                              # the upper triangle is the definition
+            ref = _dot_by_definition(sub.Psi[a].cpu().numpy(), sub.HPsi[b].cpu().numpy())
+            assert abs(Hp[i, j].item() - ref) <= 4 * M * EPS * amax
+        res = h.expand(Hp, w.nocc, rfoe.SP2, w.tol)
+        assert res.converged
+        Y, rho, _ = h.apply(res.P, sub.Psi)
+        Pn = res.P.cpu().numpy()
+        cols = [0, 1, 127, 128, M - 1, M - 2, M - 64, 599936, 599935] + rng.integers(0, M, size=6).tolist()
+        rows = [0, k - 1, 128, 127, 2049] + rng.integers(0, k, size=4).tolist()
+        pmax = float(np.abs(Pn).max()) * float(sub.Psi.abs().max())
+        for m_ in cols:
+            col = sub.Psi[:, m_].cpu().numpy()
+            for i in rows:
+                assert abs(Y[i, m_].item() - _dot_by_definition(Pn[i], col)) <= 4 * k * EPS * pmax
+            ycol = Y[:, m_].cpu().numpy()
+            assert abs(rho[m_].item() - _dot_by_definition(col, ycol)) <= 4 * k * EPS * float(np.abs(col).max() * np.abs(ycol).max())
+        assert abs(float(rho.sum()) - w.nocc) <= 1e-8                  # electron count
+        Qo = w.Q[:, : w.nocc] if isinstance(w.Q, torch.Tensor) else torch.from_numpy(w.Q[:, : w.nocc]).cuda()
+        rho_exact = ((Qo.T @ sub.Psi) ** 2).sum(dim=0)
+        assert float((rho - rho_exact).abs().max()) <= 1e-12
