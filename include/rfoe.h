@@ -167,6 +167,28 @@ int rfoe_project(rfoe_handle_t h, const double* Psi, const double* HPsi, int64_t
 int rfoe_apply(rfoe_handle_t h, const double* P, const double* Psi, int64_t k, int64_t M, int64_t ld, double* Y,
                int64_t ldy, double* rho, float* kernel_ms, rfoe_stream_t stream);
 
+/* ---- one expansion sharded over several GPUs (one process per GPU) -------------------------------------
+ * The paper distributes the product over a process grid and communicates inside every multiplication
+ * (PAPER.md:70-72).  Here every rank holds the whole X_n and squares a contiguous range of the upper-triangle
+ * tile list (rfoe_shard_range); the exchange step is ONE all-gather per recursion step of this rank's new tiles
+ * and their partial sums (4 n^2 (g-1)/g bytes received per GPU), after which every rank owns the whole X_{n+1}
+ * and takes the same branch decision from the same sums in the same order: P is bitwise the single-GPU P.
+ * Bounds, the affine map and the output pass are replicated on every rank (HBM-bound, O(k^2)).
+ *
+ * allgather(user, send, recv, bytes, stream): must gather `bytes` bytes from the DEVICE buffer `send` of every
+ * rank into the DEVICE buffer `recv` (world x bytes, rank order), ordered after the work already enqueued on
+ * `stream` and complete before work enqueued on `stream` afterwards (e.g. ncclAllGather on that stream, or
+ * torch.distributed.all_gather_into_tensor under that current stream).  Returns 0 on success.
+ * Every rank must call with the same H^p, k, nocc, variant, tol and options.  Variants: SP2 and SP2_ACCEL
+ * (and T-RFOE through RFOE_OPT_MAX_ITER); others -> UNSUPPORTED. */
+typedef int (*rfoe_allgather_fn)(void* user, const void* send, void* recv, int64_t bytes, rfoe_stream_t stream);
+int rfoe_expand_sharded(rfoe_handle_t h, const double* Hp, int64_t k, int64_t nocc, int variant, double tol, double* P,
+                        int rank, int world, rfoe_allgather_fn allgather, void* user, rfoe_stream_t stream);
+
+/* Host-only helper (no device needed): the range [begin, begin + count) of the n_tiles upper-triangle tiles that
+ * `rank` of `world` squares: ceil(n_tiles / world) tiles each, the last ranks possibly fewer (or none). */
+int rfoe_shard_range(int64_t n_tiles, int rank, int world, int64_t* begin, int64_t* count);
+
 int rfoe_set_option(rfoe_handle_t h, int key, double value); /* INVALID_ARG on bad value, UNSUPPORTED on bad key */
 int rfoe_get_stats(rfoe_handle_t h, rfoe_stats_t* out);      /* copies the stats of the last call */
 int rfoe_destroy(rfoe_handle_t h);                           /* frees everything the handle owns; h may be null */

@@ -17,7 +17,7 @@ import numpy as np
 
 from . import build as _build
 
-__all__ = ["Rfoe", "RfoeError", "ExpandResult", "load_library", "SP2", "MCWEENY", "SP2_MIXED", "SP2_ACCEL",
+__all__ = ["Rfoe", "RfoeError", "ExpandResult", "load_library", "shard_range", "torch_distributed_allgather", "SP2", "MCWEENY", "SP2_MIXED", "SP2_ACCEL",
            "RULE_A", "RULE_B", "EXPORTS"]
 
 SP2, MCWEENY, SP2_MIXED, SP2_ACCEL = 0, 1, 2, 3
@@ -31,8 +31,12 @@ OK, ERR_INVALID_ARG, ERR_ALLOC, ERR_CUDA, ERR_BAD_BOUNDS, ERR_NOT_SYMMETRIC, ERR
 
 # every symbol include/rfoe.h declares
 EXPORTS = ("rfoe_create", "rfoe_bounds", "rfoe_expand", "rfoe_expand_host", "rfoe_square", "rfoe_square_reduced",
-           "rfoe_symm_product", "rfoe_project", "rfoe_apply",
+           "rfoe_symm_product", "rfoe_project", "rfoe_apply", "rfoe_expand_sharded", "rfoe_shard_range",
            "rfoe_set_option", "rfoe_get_stats", "rfoe_destroy", "rfoe_strerror", "rfoe_version")
+
+
+# int allgather(void* user, const void* send, void* recv, int64_t bytes, stream)  -- see include/rfoe.h
+ALLGATHER_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p)
 
 
 class RfoeError(RuntimeError):
@@ -80,6 +84,8 @@ def load_library(path: str | None = None):
     L.rfoe_symm_product.argtypes = [vp, vp, vp, i64, dbl, dbl, dbl, vp, dp, C.POINTER(C.c_float), vp]
     L.rfoe_project.argtypes = [vp, vp, vp, i64, i64, i64, vp, dp, C.POINTER(C.c_float), vp]
     L.rfoe_apply.argtypes = [vp, vp, vp, i64, i64, i64, vp, i64, vp, C.POINTER(C.c_float), vp]
+    L.rfoe_expand_sharded.argtypes = [vp, vp, i64, i64, C.c_int, dbl, vp, C.c_int, C.c_int, ALLGATHER_FN, vp, vp]
+    L.rfoe_shard_range.argtypes = [i64, C.c_int, C.c_int, C.POINTER(i64), C.POINTER(i64)]
     L.rfoe_set_option.argtypes = [vp, C.c_int, dbl]
     L.rfoe_get_stats.argtypes = [vp, C.POINTER(_Stats)]
     L.rfoe_destroy.argtypes = [vp]
@@ -138,6 +144,40 @@ def _check_rect(x, name):
     if not (isinstance(x, torch.Tensor) and x.is_cuda and x.dtype == torch.float64 and x.dim() == 2 and x.stride(1) == 1
             and x.stride(0) >= x.shape[1]):
         raise ValueError(f"{name}: row-major float64 CUDA matrix (k x M, unit column stride) expected")
+
+
+def shard_range(n_tiles: int, rank: int, world: int):
+    """(begin, count) of the upper-triangle tile range `rank` of `world` squares (host-only C call)."""
+    b, c = C.c_int64(), C.c_int64()
+    rc = load_library().rfoe_shard_range(int(n_tiles), int(rank), int(world), C.byref(b), C.byref(c))
+    if rc != OK:
+        raise RfoeError(rc, "rfoe_shard_range: invalid argument")
+    return b.value, c.value
+
+
+class _DevBytes:
+    """A raw device range as a __cuda_array_interface__ object (so torch can wrap it without copying)."""
+
+    def __init__(self, ptr: int, nbytes: int):
+        self.__cuda_array_interface__ = {"shape": (int(nbytes),), "typestr": "|u1", "data": (int(ptr), False), "version": 2}
+
+
+def torch_distributed_allgather(group=None):
+    """The exchange step of rfoe_expand_sharded through torch.distributed (NCCL over NVLink): an all-gather of the
+    library's send buffer into its receive buffer, issued under the library's stream."""
+    import torch
+    import torch.distributed as dist
+
+    def allgather(send_ptr: int, recv_ptr: int, nbytes: int, stream_ptr) -> int:
+        world = dist.get_world_size(group)
+        ext = torch.cuda.ExternalStream(stream_ptr) if stream_ptr else torch.cuda.default_stream()
+        with torch.cuda.stream(ext):
+            send = torch.as_tensor(_DevBytes(send_ptr, nbytes), device="cuda")
+            recv = torch.as_tensor(_DevBytes(recv_ptr, nbytes * world), device="cuda")
+            dist.all_gather_into_tensor(recv, send, group=group)
+        return 0
+
+    return allgather
 
 
 class Rfoe:
@@ -310,3 +350,33 @@ class Rfoe:
         if rc != OK:
             self._raise(rc)
         return out, rho, ms.value
+
+    def expand_sharded(self, Hp, nocc: int, variant: int = SP2, tol: float = 1e-12, P=None, *, rank: int, world: int,
+                       allgather=None, stream=None) -> ExpandResult:
+        """One expansion sharded over `world` ranks (one process per GPU); every rank passes the same H^p and gets
+        the whole P.  `allgather(send_ptr, recv_ptr, nbytes, stream_ptr) -> int` performs the exchange step; the
+        default is torch.distributed's all_gather_into_tensor on the default process group."""
+        import torch
+
+        _check_dev(Hp, "Hp")
+        if P is None:
+            P = torch.empty_like(Hp)
+        _check_dev(P, "P")
+        fn = allgather if allgather is not None else torch_distributed_allgather()
+        err = []
+
+        def _cb(user, send, recv, nbytes, stream_ptr):
+            try:
+                return int(fn(send, recv, nbytes, stream_ptr))
+            except BaseException as e:  # an exception must not unwind through the C frames
+                err.append(e)
+                return 1
+
+        cb = ALLGATHER_FN(_cb)
+        rc = self._L.rfoe_expand_sharded(self._h, C.c_void_p(Hp.data_ptr()), Hp.shape[0], int(nocc), int(variant), float(tol),
+                                         C.c_void_p(P.data_ptr()), int(rank), int(world), cb, None, _stream_ptr(stream))
+        if err:
+            raise err[0]
+        if rc not in (OK, ERR_NOT_CONVERGED):
+            self._raise(rc)
+        return self._result(P, rc)

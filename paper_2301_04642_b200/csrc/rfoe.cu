@@ -13,6 +13,7 @@
 #include "../../include/rfoe.h"
 #include "control.cuh"
 #include "hbm_kernels.cuh"
+#include "shard.cuh"
 #include "subspace.cuh"
 #include "sym_square.cuh"
 #include "sym_square_tf32.cuh"
@@ -53,6 +54,10 @@ struct rfoe_handle_s {
     int n_tiles = 0;
     HostPage* hp = nullptr;
     int* d_word = nullptr; // device alias of hp->word
+    double* sh_send = nullptr; // sharded expansion: [c tiles | c records] to send, g such blocks received,
+    double* sh_recv = nullptr; //   and the records in global tile order (allocated on the first sharded call)
+    double* sh_parts = nullptr;
+    size_t sh_bytes = 0;
     double* ws = nullptr;      // scratch of the projection / density steps (grown on demand)
     size_t ws_bytes = 0;
     double* stage_H = nullptr;
@@ -231,6 +236,7 @@ extern "C" int rfoe_destroy(rfoe_handle_t h)
     cudaFree(h->d_bounds); cudaFree(h->d_scalars); cudaFree(h->d_flag); cudaFree(h->d_ctrl); cudaFree(h->d_tiles);
     cudaFree(h->d_pairs);
     cudaFree(h->stage_H); cudaFree(h->stage_P); cudaFree(h->ws);
+    cudaFree(h->sh_send); cudaFree(h->sh_recv); cudaFree(h->sh_parts);
     if (h->hp) cudaFreeHost(h->hp);
     if (h->ev0) cudaEventDestroy(h->ev0);
     if (h->ev1) cudaEventDestroy(h->ev1);
@@ -374,8 +380,27 @@ static int ensure_third(rfoe_handle_s* h)
     return RFOE_OK;
 }
 
-extern "C" int rfoe_expand(rfoe_handle_t h, const double* Hp, int64_t k64, int64_t nocc, int variant, double tol, double* P,
-                           rfoe_stream_t stream)
+struct ShardCtx {
+    int rank, world;
+    rfoe_allgather_fn allgather;
+    void* user;
+};
+
+extern "C" int rfoe_shard_range(int64_t n_tiles, int rank, int world, int64_t* begin, int64_t* count)
+{
+    if (n_tiles < 1 || world < 1 || rank < 0 || rank >= world || !begin || !count) return RFOE_ERR_INVALID_ARG;
+    const int64_t c = (n_tiles + world - 1) / world;
+    int64_t b = (int64_t)rank * c;
+    if (b > n_tiles) b = n_tiles;
+    int64_t e = b + c;
+    if (e > n_tiles) e = n_tiles;
+    *begin = b;
+    *count = e - b;
+    return RFOE_OK;
+}
+
+static int expand_impl(rfoe_handle_t h, const double* Hp, int64_t k64, int64_t nocc, int variant, double tol, double* P,
+                       rfoe_stream_t stream, const ShardCtx* sh)
 {
     int rc = check_common(h, Hp, P, k64);
     if (rc != RFOE_OK) return rc;
@@ -402,6 +427,30 @@ extern "C" int rfoe_expand(rfoe_handle_t h, const double* Hp, int64_t k64, int64
     if (variant == RFOE_VARIANT_MCWEENY && (rc = ensure_third(h)) != RFOE_OK) return fail(rc);
     if (variant == RFOE_VARIANT_SP2_MIXED && (rc = ensure_tf32(h)) != RFOE_OK) return fail(rc);
     if ((rc = ensure_tiles(h, m, st)) != RFOE_OK) return fail(rc);
+    // sharded run: this rank's contiguous range of the tile order, and the exchange buffers
+    int t_begin = 0, t_count = h->n_tiles, c_max = h->n_tiles;
+    size_t rank_stride = 0;
+    if (sh) {
+        if (variant != RFOE_VARIANT_SP2 && variant != RFOE_VARIANT_SP2_ACCEL) return fail(RFOE_ERR_UNSUPPORTED);
+        int64_t b, c;
+        if (rfoe_shard_range(h->n_tiles, sh->rank, sh->world, &b, &c) != RFOE_OK || !sh->allgather) return fail(RFOE_ERR_INVALID_ARG);
+        t_begin = (int)b; t_count = (int)c;
+        c_max = (h->n_tiles + sh->world - 1) / sh->world;
+        rank_stride = (size_t)c_max * (TILE_ELEMS + SQ_NPART);
+        const size_t need = rank_stride * sh->world * sizeof(double);
+        if (h->sh_bytes < need) {
+            cudaFree(h->sh_send); cudaFree(h->sh_recv); cudaFree(h->sh_parts);
+            h->sh_send = h->sh_recv = h->sh_parts = nullptr; h->sh_bytes = 0;
+            if (cudaMalloc(&h->sh_send, rank_stride * sizeof(double)) != cudaSuccess ||
+                cudaMalloc(&h->sh_recv, need) != cudaSuccess ||
+                cudaMalloc(&h->sh_parts, (size_t)c_max * sh->world * SQ_NPART * sizeof(double)) != cudaSuccess) {
+                cudaGetLastError();
+                return fail(RFOE_ERR_ALLOC);
+            }
+            h->sh_bytes = need;
+        }
+        CK(cudaMemsetAsync(h->sh_send, 0, rank_stride * sizeof(double), st));   // padding tiles / records of a short last range
+    }
     CUtensorMap tm[3];
     for (int i = 0; i < 3; ++i)
         if (h->W[i] && (rc = make_map(h, &tm[i], h->W[i], n, ld)) != RFOE_OK) return fail(rc);
@@ -469,7 +518,30 @@ extern "C" int rfoe_expand(rfoe_handle_t h, const double* Hp, int64_t k64, int64
     h->sq_n = 0;
     while (action != ACT_STOP) {
         const int nxt = cur ^ 1;
-        if (action == ACT_SP2) {
+        if (action == ACT_SP2 && sh) {
+            // this rank's tiles (and their mirrors) -> W[nxt]; pack them with their records; ONE all-gather; unpack
+            // the foreign tiles; the records, now in global tile order, feed the same control kernel on every rank
+            if (t_count > 0) {
+                CK(cudaEventRecord(h->sq_ev[2 * h->sq_n], st));
+                sym_square_kernel<0><<<t_count, SQ_THREADS, SQ_SMEM_BYTES, st>>>(tm[cur], tm[cur], h->W[cur], h->W[nxt], n, ld, k,
+                                                                              &h->d_ctrl->coef, h->d_tiles + t_begin,
+                                                                              h->sh_send + (size_t)c_max * TILE_ELEMS, 0);
+                h->launches++;
+                CK(cudaGetLastError());
+                CK(cudaEventRecord(h->sq_ev[2 * h->sq_n + 1], st));
+                h->sq_n++;
+                pack_tiles_kernel<<<t_count, 256, 0, st>>>(h->W[nxt], ld, h->d_tiles + t_begin, h->sh_send);
+                h->launches++;
+                CK(cudaGetLastError());
+            }
+            if (sh->allgather(sh->user, h->sh_send, h->sh_recv, (int64_t)(rank_stride * sizeof(double)), stream) != 0)
+                return fail(RFOE_ERR_CUDA);
+            unpack_tiles_kernel<<<h->n_tiles, 256, 0, st>>>(h->sh_recv, rank_stride, c_max, h->d_tiles, t_begin, t_count, h->W[nxt], ld,
+                                                           h->sh_parts);
+            h->launches++;
+            CK(cudaGetLastError());
+            control_kernel<<<1, 256, 0, st>>>(h->d_ctrl, 1, h->sh_parts, h->sh_parts, h->n_tiles, h->d_word);
+        } else if (action == ACT_SP2) {
             CK(timed_square<false>(h, tm[cur], tm[cur], h->W[cur], h->W[nxt], n, ld, k, &h->d_ctrl->coef, h->part[0], st));
             control_kernel<<<1, 256, 0, st>>>(h->d_ctrl, 1, h->part[0], h->part[0], h->n_tiles, h->d_word);
         } else if (action == ACT_SP2_FP32) {
@@ -523,6 +595,20 @@ extern "C" int rfoe_expand(rfoe_handle_t h, const double* Hp, int64_t k64, int64
     S.branch[ns] = 0;
     S.status = C.converged ? RFOE_OK : RFOE_ERR_NOT_CONVERGED;
     return S.status;
+}
+
+extern "C" int rfoe_expand(rfoe_handle_t h, const double* Hp, int64_t k, int64_t nocc, int variant, double tol, double* P,
+                           rfoe_stream_t stream)
+{
+    return expand_impl(h, Hp, k, nocc, variant, tol, P, stream, nullptr);
+}
+
+extern "C" int rfoe_expand_sharded(rfoe_handle_t h, const double* Hp, int64_t k, int64_t nocc, int variant, double tol, double* P,
+                                   int rank, int world, rfoe_allgather_fn allgather, void* user, rfoe_stream_t stream)
+{
+    if (world < 1 || rank < 0 || rank >= world || !allgather) return RFOE_ERR_INVALID_ARG;
+    ShardCtx sh = {rank, world, allgather, user};
+    return expand_impl(h, Hp, k, nocc, variant, tol, P, stream, &sh);
 }
 
 // ---------------------------------------------------------------------------------------------

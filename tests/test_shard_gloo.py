@@ -1,0 +1,68 @@
+"""Host logic of the sharded expansion on CPU: the tile partition
+(rfoe_shard_range, a host-only C call) single-process and across a world_size-2 gloo group."""
+import os
+import socket
+import sys
+
+import pytest
+
+torch = pytest.importorskip("torch")
+import torch.distributed as dist  # noqa: E402
+import torch.multiprocessing as mp  # noqa: E402
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.mark.parametrize("n_tiles,world", [(1, 1), (1, 4), (3, 2), (10, 4), (528, 8), (8256, 8), (8256, 7), (49141, 6)])
+def test_shard_ranges_partition_the_tile_list(n_tiles, world):
+    import paper_2301_04642_b200 as rfoe
+
+    c_max = -(-n_tiles // world)
+    nxt = 0
+    for r in range(world):
+        b, c = rfoe.shard_range(n_tiles, r, world)
+        assert b == min(r * c_max, n_tiles)            # rank r's block starts at r * c_max in the gathered buffer
+        assert b == nxt or c == 0
+        assert 0 <= c <= c_max
+        nxt = b + c
+    assert nxt == n_tiles
+    with pytest.raises(rfoe.RfoeError):
+        rfoe.shard_range(n_tiles, world, world)
+
+
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def _worker(rank, world, port, n_tiles, out):
+    sys.path.insert(0, ROOT)
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    import paper_2301_04642_b200 as rfoe
+
+    b, c = rfoe.shard_range(n_tiles, rank, world)
+    # the exchange step in miniature: every rank contributes a block of c_max slots holding the global indices of
+    # its tiles (padding = -1); the gathered buffer must list 0..n_tiles-1 in order, padding only at the end
+    c_max = -(-n_tiles // world)
+    send = torch.full((c_max,), -1, dtype=torch.int64)
+    send[:c] = torch.arange(b, b + c)
+    recv = torch.empty((world * c_max,), dtype=torch.int64)
+    dist.all_gather_into_tensor(recv, send)
+    out[rank] = recv.tolist()
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("n_tiles", [5, 528])
+def test_gathered_layout_is_global_tile_order_world2(n_tiles):
+    world, port = 2, _free_port()
+    with mp.Manager() as m:
+        out = m.dict()
+        mp.spawn(_worker, args=(world, port, n_tiles, out), nprocs=world, join=True)
+        res = dict(out)
+    assert res[0] == res[1]
+    got = res[0]
+    assert got[:n_tiles] == list(range(n_tiles))
+    assert all(v == -1 for v in got[n_tiles:])
