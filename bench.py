@@ -204,8 +204,10 @@ def run_ours(args) -> int:
         raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=dev)
+    if world > 1 or args.shard:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("MASTER_PORT", "29537")
+        dist.init_process_group("nccl", device_id=dev, rank=rank, world_size=world)
 
     def barrier():
         if world > 1:
@@ -220,7 +222,7 @@ def run_ours(args) -> int:
         return 0
     cfg = rfoe_inputs.CONFIGS[args.config]
     # every rank owns an independent problem of the same configuration (replicas; no data-path collective)
-    want_reduced = (world == 1 and not args.no_reduced)
+    want_reduced = (world == 1 and not args.no_reduced and not args.shard)
     w = rfoe_inputs.make_workload(args.config, device=str(dev) if cfg.k > 2048 else "cpu", keep_q=want_reduced)
     H = w.H if isinstance(w.H, torch.Tensor) else torch.from_numpy(w.H).to(dev)
     k, nocc, tol = w.k, w.nocc, w.tol
@@ -228,7 +230,13 @@ def run_ours(args) -> int:
     stream = torch.cuda.current_stream()
     h = rfoe.Rfoe(k, device=local)
 
+    shard = bool(args.shard)
+    if shard and world > 1:
+        dist.broadcast(H, src=0)         # one problem, the same bytes on every rank
+
     def step():
+        if shard:   # ONE expansion over all ranks: tile ranges + one NCCL all-gather per step
+            return h.expand_sharded(H, nocc, rfoe.SP2, tol, P=P, rank=rank, world=world, stream=stream)
         return h.expand(H, nocc, rfoe.SP2, tol, P=P, stream=stream)
 
     # ---- device-resident arm: W warm-up steps, then exactly K timed steps
@@ -256,7 +264,7 @@ def run_ours(args) -> int:
     iters = res.iterations
     fl_sq = executed_flops_per_squaring(k)
     fl_step = iters * fl_sq
-    ms_total, value = whole_job_rate(ms_local, args.steps * fl_step, dev)
+    ms_total, value = whole_job_rate(ms_local, args.steps * fl_step / (world if shard else 1), dev)
 
     # ---- end-to-end arm: host buffers through rfoe_expand_host (H2D of H^p and D2H of P inside the timed region)
     Hh = torch.empty((k, k), dtype=torch.float64, pin_memory=True)
@@ -272,27 +280,31 @@ def run_ours(args) -> int:
     e1.record(stream)
     barrier()
     ms2, e2e_value = whole_job_rate(e0.elapsed_time(e1), args.steps * r2.iterations * fl_sq, dev)
+    if shard:     # the host-buffer arm runs per-rank replicas; a sharded job is one expansion, so quote one rank's rate
+        e2e_value /= world
     assert abs(float(Ph.diagonal().sum()) - nocc) < 1e-6
 
     if rank == 0:
         avg_launch_ms = sq_ms / max(sq_n, 1)
-        achieved = fl_sq / (avg_launch_ms * 1e-3) / 1e12
+        fl_launch = fl_sq / (world if shard else 1)      # a sharded launch squares 1/world of the tiles
+        achieved = fl_launch / (avg_launch_ms * 1e-3) / 1e12
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "strong" if shard else "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": f"BASELINE.json config {args.config}: k={k}, nocc={nocc}, SP2, stop rule A tol {tol:.3g}, "
                                    "Gershgorin bounds, H^p = Q diag(lambda) Q^T seeded",
-                       "parallelism": "replicas only: one independent expansion per GPU, no collective",
+                       "parallelism": (f"sharded: one expansion over {world} GPUs, tile ranges + one NCCL all-gather per step" if shard
+                                       else "replicas only: one independent expansion per GPU, no collective"),
                        "l2": f"inputs larger than L2 (each matrix {8.0 * k * k / 1e6:.0f} MB vs 126 MB L2); no flush needed",
                        "squarings_per_expansion": iters, "branch": res.branch},
             "seconds_per_expansion": ms_total / args.steps / 1e3,
-            "gemm_equiv_tflops": world * args.steps * iters * 2.0 * k ** 3 / (ms_total * 1e-3) / 1e12,
+            "gemm_equiv_tflops": (1 if shard else world) * args.steps * iters * 2.0 * k ** 3 / (ms_total * 1e-3) / 1e12,
             "square_share_of_step": sq_ms / ms_total if world == 1 else None,
             "roofline": {"bound": "tensor", "kernel": "sym_square_kernel<false> (FP64 DMMA.8x8x4)", "achieved": achieved,
                          "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP64_PEAK_TFLOPS,
                          "traffic": NCU_TRAFFIC_BYTES.get(k), "avg_launch_ms": avg_launch_ms, "launches_timed": sq_n,
-                         "flops_per_launch": fl_sq,
+                         "flops_per_launch": fl_launch,
                          "peak_source": "derived: 148 SM x 64 DFMA/clk x 2 x 1.965 GHz (no FP64 entry in MEASURED_PEAKS.json)"},
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 8 * k * k, "d2h_bytes_per_step": 8 * k * k,
                     "ms_per_step": ms2 / args.steps},
@@ -314,7 +326,7 @@ def run_ours(args) -> int:
                           f"({its} squarings); oracle flops = k^2(k+1) per squaring"}
         print(json.dumps(line), flush=True)
     h.close()
-    if world > 1:
+    if dist.is_initialized():
         dist.destroy_process_group()
     return 0
 
@@ -423,6 +435,8 @@ def main() -> int:
     ap.add_argument("--cpu-k", type=int, default=2048, help="size of the oracle's bounded sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-reduced", action="store_true", help="skip the separately reported reduced-precision run")
+    ap.add_argument("--shard", action="store_true",
+                    help="N > 1: shard ONE expansion over the ranks (strong scaling) instead of independent replicas")
     ap.add_argument("--no-subspace", action="store_true", help="skip the separately reported Rayleigh-Ritz / apply steps")
     ap.add_argument("--only-subspace", action="store_true", help="run only the Rayleigh-Ritz / apply chain (ncu captures)")
     ap.add_argument("--subspace-k", type=int, default=4096)
