@@ -17,6 +17,7 @@
 #include "subspace.cuh"
 #include "sym_square.cuh"
 #include "sym_square_tf32.cuh"
+#include "tail.cuh"
 
 using namespace rfoe;
 
@@ -207,6 +208,66 @@ static cudaError_t timed_square(rfoe_handle_s* h, const CUtensorMap& a, const CU
     h->sq_n++;
     return e;
 }
+
+// ---------------------------------------------------------------------------------------------
+// Tail plan of a squaring launch (tail.cuh): tiles [0, n_main) go to the main kernel in whole waves, the last
+// T = n_tiles - n_main tiles are cut into `slices` K-slices of kt_per chunks.  Chosen by a cycle model (a full tile
+// costs kt * 4096 DMMA cycles + ~45k of epilogue / launch; a slice CTA kt_per * 4096 + ~20k; the two extra kernel
+// boundaries and the fix-up ~60k) and only taken when the model saves >= 1.5 %: measured, k=8192 gains 5.2 % (16.35 ->
+// 15.55 ms), k=4096 8.5 %, but at k=16384 the modelled 0.3 % came out as -0.06 % (122.22 vs 122.15 ms), so large
+// problems keep the plain launch.  Depends on (n_tiles, kt, SM count) only.
+struct TailPlan {
+    int n_main, slices, kt_per;
+};
+
+static TailPlan plan_tail(int n_tiles, int kt_total, int sm)
+{
+    TailPlan best = {n_tiles, 1, kt_total};
+    const double full = kt_total * 4096.0 + 45000.0;
+    const double base = (double)((n_tiles + sm - 1) / sm) * full;
+    double best_t = base * (1.0 - 0.015);
+    const int r = n_tiles % sm;
+    for (int w = 0; w <= 1; ++w) {
+        const int T = r + w * sm;
+        if (T == 0 || T > n_tiles) continue;
+        for (int s = 2; s <= 16; ++s) {
+            const int per = (kt_total + s - 1) / s;
+            if (per < 16) break;
+            const int eff = (kt_total + per - 1) / per;
+            const long long ctas = (long long)T * eff;
+            const double t = (double)((n_tiles - T) / sm) * full + (double)((ctas + sm - 1) / sm) * (per * 4096.0 + 20000.0) + 60000.0;
+            if (t < best_t) { best_t = t; best = {n_tiles - T, eff, per}; }
+        }
+    }
+    return best;
+}
+
+// SP2 squaring of tiles [t_begin, t_begin + t_count) of the tile order: main kernel below plan.n_main, split-K tail
+// + fix-up above.  rec = partial record of tile t_begin.
+static cudaError_t launch_sp2_range(rfoe_handle_s* h, const CUtensorMap& tm, const double* E, double* Out, int n, int ld, int k,
+                                    const StepCoef* coef, double* rec, int t_begin, int t_count, const TailPlan& plan,
+                                    cudaStream_t st)
+{
+    const int t_end = t_begin + t_count;
+    const int main_end = t_end < plan.n_main ? t_end : plan.n_main;
+    if (main_end > t_begin) {
+        sym_square_kernel<0><<<main_end - t_begin, SQ_THREADS, SQ_SMEM_BYTES, st>>>(tm, tm, E, Out, n, ld, k, coef, h->d_tiles + t_begin,
+                                                                                rec, 0);
+        h->launches++;
+    }
+    const int tail_b = t_begin > plan.n_main ? t_begin : plan.n_main;
+    const int n_tl = t_end - tail_b;
+    if (n_tl > 0) {
+        sym_square_kernel<2><<<dim3(n_tl, plan.slices), SQ_THREADS, SQ_SMEM_BYTES, st>>>(tm, tm, nullptr, h->ws, n, SQ_BM, k, nullptr,
+                                                                                      h->d_tiles + tail_b, nullptr, plan.kt_per);
+        tail_fixup_kernel<<<n_tl, TAIL_THREADS, 0, st>>>(h->ws, plan.slices, n_tl, h->d_tiles + tail_b, E, Out, ld, k, coef,
+                                                rec + (size_t)(tail_b - t_begin) * SQ_NPART);
+        h->launches += 2;
+    }
+    return cudaGetLastError();
+}
+
+static int ensure_tail_ws(rfoe_handle_s* h, int n_tiles, const TailPlan& plan);
 
 extern "C" const char* rfoe_strerror(int status)
 {
@@ -451,6 +512,8 @@ static int expand_impl(rfoe_handle_t h, const double* Hp, int64_t k64, int64_t n
         }
         CK(cudaMemsetAsync(h->sh_send, 0, rank_stride * sizeof(double), st));   // padding tiles / records of a short last range
     }
+    const TailPlan plan = plan_tail(h->n_tiles, n / SQ_BK, h->sm_count);
+    if ((rc = ensure_tail_ws(h, h->n_tiles, plan)) != RFOE_OK) return fail(rc);
     CUtensorMap tm[3];
     for (int i = 0; i < 3; ++i)
         if (h->W[i] && (rc = make_map(h, &tm[i], h->W[i], n, ld)) != RFOE_OK) return fail(rc);
@@ -523,11 +586,8 @@ static int expand_impl(rfoe_handle_t h, const double* Hp, int64_t k64, int64_t n
             // the foreign tiles; the records, now in global tile order, feed the same control kernel on every rank
             if (t_count > 0) {
                 CK(cudaEventRecord(h->sq_ev[2 * h->sq_n], st));
-                sym_square_kernel<0><<<t_count, SQ_THREADS, SQ_SMEM_BYTES, st>>>(tm[cur], tm[cur], h->W[cur], h->W[nxt], n, ld, k,
-                                                                              &h->d_ctrl->coef, h->d_tiles + t_begin,
-                                                                              h->sh_send + (size_t)c_max * TILE_ELEMS, 0);
-                h->launches++;
-                CK(cudaGetLastError());
+                CK(launch_sp2_range(h, tm[cur], h->W[cur], h->W[nxt], n, ld, k, &h->d_ctrl->coef,
+                                    h->sh_send + (size_t)c_max * TILE_ELEMS, t_begin, t_count, plan, st));
                 CK(cudaEventRecord(h->sq_ev[2 * h->sq_n + 1], st));
                 h->sq_n++;
                 pack_tiles_kernel<<<t_count, 256, 0, st>>>(h->W[nxt], ld, h->d_tiles + t_begin, h->sh_send);
@@ -542,7 +602,10 @@ static int expand_impl(rfoe_handle_t h, const double* Hp, int64_t k64, int64_t n
             CK(cudaGetLastError());
             control_kernel<<<1, 256, 0, st>>>(h->d_ctrl, 1, h->sh_parts, h->sh_parts, h->n_tiles, h->d_word);
         } else if (action == ACT_SP2) {
-            CK(timed_square<false>(h, tm[cur], tm[cur], h->W[cur], h->W[nxt], n, ld, k, &h->d_ctrl->coef, h->part[0], st));
+            CK(cudaEventRecord(h->sq_ev[2 * h->sq_n], st));
+            CK(launch_sp2_range(h, tm[cur], h->W[cur], h->W[nxt], n, ld, k, &h->d_ctrl->coef, h->part[0], 0, h->n_tiles, plan, st));
+            CK(cudaEventRecord(h->sq_ev[2 * h->sq_n + 1], st));
+            h->sq_n++;
             control_kernel<<<1, 256, 0, st>>>(h->d_ctrl, 1, h->part[0], h->part[0], h->n_tiles, h->d_word);
         } else if (action == ACT_SP2_FP32) {
             CK(cudaEventRecord(h->sq_ev[2 * h->sq_n], st));
@@ -650,7 +713,11 @@ static int single_product(rfoe_handle_s* h, const double* A, const double* B, in
         CK(launch_square_tf32(h, tmF[0], tmF[1], h->W[0], h->W[2], n, ld, k, h->d_scalars + 7, &h->d_ctrl->coef, h->part[0], st));
     }
     else if (two) CK(launch_square<true>(h, tm[0], tm[1], h->W[0], h->W[2], n, ld, k, &h->d_ctrl->coef, h->part[0], st));
-    else     CK(launch_square<false>(h, tm[0], tm[0], h->W[0], h->W[2], n, ld, k, &h->d_ctrl->coef, h->part[0], st));
+    else {
+        const TailPlan plan = plan_tail(h->n_tiles, n / SQ_BK, h->sm_count);
+        if ((rc = ensure_tail_ws(h, h->n_tiles, plan)) != RFOE_OK) return rc;
+        CK(launch_sp2_range(h, tm[0], h->W[0], h->W[2], n, ld, k, &h->d_ctrl->coef, h->part[0], 0, h->n_tiles, plan, st));
+    }
     CK(cudaEventRecord(h->ev1, st));
     sum_partials_kernel<<<1, 256, 0, st>>>(h->part[0], reduced ? 2 * h->n_pairs : h->n_tiles, h->d_scalars);
     h->launches++;
@@ -709,6 +776,12 @@ static int ensure_ws(rfoe_handle_s* h, size_t bytes)
     if (cudaMalloc(&h->ws, bytes) != cudaSuccess) { cudaGetLastError(); return RFOE_ERR_ALLOC; }
     h->ws_bytes = bytes;
     return RFOE_OK;
+}
+
+static int ensure_tail_ws(rfoe_handle_s* h, int n_tiles, const TailPlan& plan)
+{
+    const size_t T = (size_t)(n_tiles - plan.n_main);
+    return T ? ensure_ws(h, T * plan.slices * SQ_BM * SQ_BM * sizeof(double)) : RFOE_OK;
 }
 
 static bool rect_args_ok(const rfoe_handle_s* h, const void* a, int64_t k, int64_t M, int64_t ld)
