@@ -185,6 +185,27 @@ typedef int (*rfoe_allgather_fn)(void* user, const void* send, void* recv, int64
 int rfoe_expand_sharded(rfoe_handle_t h, const double* Hp, int64_t k, int64_t nocc, int variant, double tol, double* P,
                         int rank, int world, rfoe_allgather_fn allgather, void* user, rfoe_stream_t stream);
 
+/* ---- the same sharded expansion with the exchange fused into the squaring kernel (peer memory) --------------
+ * Instead of pack / all-gather / unpack, the epilogue of every tile stores the tile, its mirror and its partial
+ * record directly into the X_{n+1} and record arrays of ALL ranks through peer-mapped pointers (NVLink P2P), so
+ * the transfer is spread over the whole launch and overlaps the tensor-core work of the other tiles; the only
+ * collective left per step is a barrier.  Setup, once per handle (all ranks created with the same k_max):
+ *   same process (threads, tests):  rfoe_shard_local_ptrs on every handle, then rfoe_shard_set_peers(h, rank,
+ *       world, ptrs) with ptrs[4 d .. 4 d + 3] = rank d's four pointers (peer access enabled by the caller);
+ *   one process per GPU:            rfoe_shard_ipc_export -> all-gather the 4 x 64-byte handles -> 
+ *       rfoe_shard_ipc_import(h, rank, world, handles of all ranks in rank order) (cudaIpcOpenMemHandle).
+ * barrier(user, stream): must return after every rank's work enqueued on its stream so far has COMPLETED
+ * (e.g. cudaStreamSynchronize + an MPI / torch.distributed barrier).  Returns 0 on success.
+ * Variants and the bitwise-equality guarantee as for rfoe_expand_sharded. */
+#define RFOE_IPC_HANDLE_BYTES 64
+typedef int (*rfoe_barrier_fn)(void* user, rfoe_stream_t stream);
+int rfoe_shard_local_ptrs(rfoe_handle_t h, void** ptrs /* 4 device pointers out: W0, W1, records of even / odd steps */);
+int rfoe_shard_set_peers(rfoe_handle_t h, int rank, int world, void* const* ptrs /* 4 x world */);
+int rfoe_shard_ipc_export(rfoe_handle_t h, void* handles /* 4 x RFOE_IPC_HANDLE_BYTES out */);
+int rfoe_shard_ipc_import(rfoe_handle_t h, int rank, int world, const void* handles /* world x 4 x 64 bytes */);
+int rfoe_expand_sharded_p2p(rfoe_handle_t h, const double* Hp, int64_t k, int64_t nocc, int variant, double tol, double* P,
+                            rfoe_barrier_fn barrier, void* user, rfoe_stream_t stream);
+
 /* Host-only helper (no device needed): the range [begin, begin + count) of the n_tiles upper-triangle tiles that
  * `rank` of `world` squares: ceil(n_tiles / world) tiles each, the last ranks possibly fewer (or none). */
 int rfoe_shard_range(int64_t n_tiles, int rank, int world, int64_t* begin, int64_t* count);

@@ -32,11 +32,18 @@ OK, ERR_INVALID_ARG, ERR_ALLOC, ERR_CUDA, ERR_BAD_BOUNDS, ERR_NOT_SYMMETRIC, ERR
 # every symbol include/rfoe.h declares
 EXPORTS = ("rfoe_create", "rfoe_bounds", "rfoe_expand", "rfoe_expand_host", "rfoe_square", "rfoe_square_reduced",
            "rfoe_symm_product", "rfoe_project", "rfoe_apply", "rfoe_expand_sharded", "rfoe_shard_range",
+           "rfoe_shard_local_ptrs", "rfoe_shard_set_peers", "rfoe_shard_ipc_export", "rfoe_shard_ipc_import",
+           "rfoe_expand_sharded_p2p",
            "rfoe_set_option", "rfoe_get_stats", "rfoe_destroy", "rfoe_strerror", "rfoe_version")
 
 
 # int allgather(void* user, const void* send, void* recv, int64_t bytes, stream)  -- see include/rfoe.h
 ALLGATHER_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p)
+
+
+# int barrier(void* user, stream)  -- see include/rfoe.h
+BARRIER_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p)
+IPC_HANDLE_BYTES = 64
 
 
 class RfoeError(RuntimeError):
@@ -85,6 +92,11 @@ def load_library(path: str | None = None):
     L.rfoe_project.argtypes = [vp, vp, vp, i64, i64, i64, vp, dp, C.POINTER(C.c_float), vp]
     L.rfoe_apply.argtypes = [vp, vp, vp, i64, i64, i64, vp, i64, vp, C.POINTER(C.c_float), vp]
     L.rfoe_expand_sharded.argtypes = [vp, vp, i64, i64, C.c_int, dbl, vp, C.c_int, C.c_int, ALLGATHER_FN, vp, vp]
+    L.rfoe_shard_local_ptrs.argtypes = [vp, C.POINTER(vp)]
+    L.rfoe_shard_set_peers.argtypes = [vp, C.c_int, C.c_int, C.POINTER(vp)]
+    L.rfoe_shard_ipc_export.argtypes = [vp, vp]
+    L.rfoe_shard_ipc_import.argtypes = [vp, C.c_int, C.c_int, vp]
+    L.rfoe_expand_sharded_p2p.argtypes = [vp, vp, i64, i64, C.c_int, dbl, vp, BARRIER_FN, vp, vp]
     L.rfoe_shard_range.argtypes = [i64, C.c_int, C.c_int, C.POINTER(i64), C.POINTER(i64)]
     L.rfoe_set_option.argtypes = [vp, C.c_int, dbl]
     L.rfoe_get_stats.argtypes = [vp, C.POINTER(_Stats)]
@@ -375,6 +387,81 @@ class Rfoe:
         cb = ALLGATHER_FN(_cb)
         rc = self._L.rfoe_expand_sharded(self._h, C.c_void_p(Hp.data_ptr()), Hp.shape[0], int(nocc), int(variant), float(tol),
                                          C.c_void_p(P.data_ptr()), int(rank), int(world), cb, None, _stream_ptr(stream))
+        if err:
+            raise err[0]
+        if rc not in (OK, ERR_NOT_CONVERGED):
+            self._raise(rc)
+        return self._result(P, rc)
+
+    # ---- sharded expansion with the exchange fused into the squaring kernel (peer memory)
+    def shard_local_ptrs(self):
+        """The four device pointers (work matrices W0, W1, tile records of even / odd steps) peers must be able to write."""
+        out = (C.c_void_p * 4)()
+        rc = self._L.rfoe_shard_local_ptrs(self._h, out)
+        if rc != OK:
+            self._raise(rc)
+        return [int(p) for p in out]
+
+    def shard_set_peers(self, rank: int, world: int, ptrs):
+        """ptrs: 4 * world device pointers, rank d's four at [4 d, 4 d + 4) (same process; P2P enabled by the caller)."""
+        arr = (C.c_void_p * (4 * world))(*[C.c_void_p(int(p)) for p in ptrs])
+        rc = self._L.rfoe_shard_set_peers(self._h, int(rank), int(world), arr)
+        if rc != OK:
+            self._raise(rc)
+
+    def shard_ipc_export(self) -> bytes:
+        buf = C.create_string_buffer(4 * IPC_HANDLE_BYTES)
+        rc = self._L.rfoe_shard_ipc_export(self._h, buf)
+        if rc != OK:
+            self._raise(rc)
+        return buf.raw
+
+    def shard_ipc_import(self, rank: int, world: int, handles: bytes):
+        assert len(handles) == 4 * IPC_HANDLE_BYTES * world
+        rc = self._L.rfoe_shard_ipc_import(self._h, int(rank), int(world), C.create_string_buffer(handles, len(handles)))
+        if rc != OK:
+            self._raise(rc)
+
+    def shard_connect(self, group=None):
+        """One process per GPU: exchange CUDA IPC handles of the work buffers over torch.distributed and map the peers."""
+        import torch.distributed as dist
+
+        world, rank = dist.get_world_size(group), dist.get_rank(group)
+        mine = self.shard_ipc_export()
+        gathered = [None] * world
+        dist.all_gather_object(gathered, mine, group=group)
+        self.shard_ipc_import(rank, world, b"".join(gathered))
+        return rank, world
+
+    def expand_sharded_p2p(self, Hp, nocc: int, variant: int = SP2, tol: float = 1e-12, P=None, *, barrier=None,
+                           stream=None) -> ExpandResult:
+        """rfoe_expand_sharded_p2p after shard_set_peers / shard_connect.  `barrier(stream_ptr) -> int` must return once
+        every rank's enqueued work has completed; default: stream synchronize + torch.distributed.barrier()."""
+        import torch
+
+        _check_dev(Hp, "Hp")
+        if P is None:
+            P = torch.empty_like(Hp)
+        _check_dev(P, "P")
+        if barrier is None:
+            import torch.distributed as dist
+
+            def barrier(stream_ptr):
+                (torch.cuda.ExternalStream(stream_ptr) if stream_ptr else torch.cuda.default_stream()).synchronize()
+                dist.barrier()
+                return 0
+        err = []
+
+        def _cb(user, stream_ptr):
+            try:
+                return int(barrier(stream_ptr))
+            except BaseException as e:  # an exception must not unwind through the C frames
+                err.append(e)
+                return 1
+
+        cb = BARRIER_FN(_cb)
+        rc = self._L.rfoe_expand_sharded_p2p(self._h, C.c_void_p(Hp.data_ptr()), Hp.shape[0], int(nocc), int(variant), float(tol),
+                                             C.c_void_p(P.data_ptr()), cb, None, _stream_ptr(stream))
         if err:
             raise err[0]
         if rc not in (OK, ERR_NOT_CONVERGED):

@@ -55,6 +55,14 @@ struct rfoe_handle_s {
     int n_tiles = 0;
     HostPage* hp = nullptr;
     int* d_word = nullptr; // device alias of hp->word
+    // sharded expansion over peer memory (rfoe_shard_set_peers / rfoe_shard_ipc_import)
+    int p2p_world = 0, p2p_rank = 0;
+    double* peer_W[2][SQ_MAX_PEERS] = {};
+    double* peer_rec[2][SQ_MAX_PEERS] = {};   // records double-buffered by step parity: a fast rank's step n+1 must not
+                                              // overwrite the records its peer's control kernel of step n still reads
+    PeerSet* d_peers = nullptr;   // [2]: destinations of a step that writes W[0] / W[1] (device copy for the MODE 3 kernel)
+    void* ipc_opened[4 * SQ_MAX_PEERS] = {};
+    int n_ipc_opened = 0;
     double* sh_send = nullptr; // sharded expansion: [c tiles | c records] to send, g such blocks received,
     double* sh_recv = nullptr; //   and the records in global tile order (allocated on the first sharded call)
     double* sh_parts = nullptr;
@@ -243,16 +251,22 @@ static TailPlan plan_tail(int n_tiles, int kt_total, int sm)
 }
 
 // SP2 squaring of tiles [t_begin, t_begin + t_count) of the tile order: main kernel below plan.n_main, split-K tail
-// + fix-up above.  rec = partial record of tile t_begin.
+// + fix-up above.  rec = partial record of tile t_begin.  peers != nullptr (sharded P2P run): the epilogues store to
+// every rank's X_{n+1} (peers->out) and record array (peers->rec, global tile index) instead of Out / rec.
 static cudaError_t launch_sp2_range(rfoe_handle_s* h, const CUtensorMap& tm, const double* E, double* Out, int n, int ld, int k,
                                     const StepCoef* coef, double* rec, int t_begin, int t_count, const TailPlan& plan,
-                                    cudaStream_t st)
+                                    cudaStream_t st, const PeerSet* peers = nullptr, PeerSet* d_peers = nullptr)
 {
     const int t_end = t_begin + t_count;
     const int main_end = t_end < plan.n_main ? t_end : plan.n_main;
     if (main_end > t_begin) {
-        sym_square_kernel<0><<<main_end - t_begin, SQ_THREADS, SQ_SMEM_BYTES, st>>>(tm, tm, E, Out, n, ld, k, coef, h->d_tiles + t_begin,
-                                                                                rec, 0);
+        if (peers) {   // d_peers: the same PeerSet in device memory (rec_offset = t_begin), see sym_square.cuh MODE 3
+            sym_square_kernel<3><<<main_end - t_begin, SQ_THREADS, SQ_SMEM_BYTES, st>>>(tm, tm, E, reinterpret_cast<double*>(d_peers), n, ld, k,
+                                                                                    coef, h->d_tiles + t_begin, nullptr, 0);
+        } else {
+            sym_square_kernel<0><<<main_end - t_begin, SQ_THREADS, SQ_SMEM_BYTES, st>>>(tm, tm, E, Out, n, ld, k, coef,
+                                                                                    h->d_tiles + t_begin, rec, 0);
+        }
         h->launches++;
     }
     const int tail_b = t_begin > plan.n_main ? t_begin : plan.n_main;
@@ -260,8 +274,10 @@ static cudaError_t launch_sp2_range(rfoe_handle_s* h, const CUtensorMap& tm, con
     if (n_tl > 0) {
         sym_square_kernel<2><<<dim3(n_tl, plan.slices), SQ_THREADS, SQ_SMEM_BYTES, st>>>(tm, tm, nullptr, h->ws, n, SQ_BM, k, nullptr,
                                                                                       h->d_tiles + tail_b, nullptr, plan.kt_per);
-        tail_fixup_kernel<<<n_tl, TAIL_THREADS, 0, st>>>(h->ws, plan.slices, n_tl, h->d_tiles + tail_b, E, Out, ld, k, coef,
-                                                rec + (size_t)(tail_b - t_begin) * SQ_NPART);
+        PeerSet ps;
+        if (peers) { ps = *peers; ps.rec_offset = tail_b; }
+        else { ps = PeerSet{}; ps.n = 1; ps.out[0] = Out; ps.rec[0] = rec + (size_t)(tail_b - t_begin) * SQ_NPART; ps.rec_offset = 0; }
+        tail_fixup_kernel<<<n_tl, TAIL_THREADS, 0, st>>>(h->ws, plan.slices, n_tl, h->d_tiles + tail_b, E, ld, k, coef, ps);
         h->launches += 2;
     }
     return cudaGetLastError();
@@ -298,6 +314,8 @@ extern "C" int rfoe_destroy(rfoe_handle_t h)
     cudaFree(h->d_pairs);
     cudaFree(h->stage_H); cudaFree(h->stage_P); cudaFree(h->ws);
     cudaFree(h->sh_send); cudaFree(h->sh_recv); cudaFree(h->sh_parts);
+    for (int i = 0; i < h->n_ipc_opened; ++i) cudaIpcCloseMemHandle(h->ipc_opened[i]);
+    cudaFree(h->d_peers);
     if (h->hp) cudaFreeHost(h->hp);
     if (h->ev0) cudaEventDestroy(h->ev0);
     if (h->ev1) cudaEventDestroy(h->ev1);
@@ -354,6 +372,7 @@ extern "C" int rfoe_create(rfoe_handle_t* out, int device, int64_t k_max)
     if (cudaFuncSetAttribute(sym_square_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, SQ_SMEM_BYTES) != cudaSuccess ||
         cudaFuncSetAttribute(sym_square_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, SQ_SMEM_BYTES) != cudaSuccess ||
         cudaFuncSetAttribute(sym_square_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, SQ_SMEM_BYTES) != cudaSuccess ||
+        cudaFuncSetAttribute(sym_square_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, SQ_SMEM_BYTES) != cudaSuccess ||
         cudaFuncSetAttribute(apply_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, AP_SMEM_BYTES) != cudaSuccess ||
         cudaFuncSetAttribute(sym_square_tf32_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TQ_SMEM_BYTES) != cudaSuccess) {
         rfoe_destroy(h);
@@ -443,7 +462,8 @@ static int ensure_third(rfoe_handle_s* h)
 
 struct ShardCtx {
     int rank, world;
-    rfoe_allgather_fn allgather;
+    rfoe_allgather_fn allgather;   // exchange by all-gather (rfoe_expand_sharded) ...
+    rfoe_barrier_fn barrier;       // ... or stores to peer memory + a barrier (rfoe_expand_sharded_p2p)
     void* user;
 };
 
@@ -494,9 +514,23 @@ static int expand_impl(rfoe_handle_t h, const double* Hp, int64_t k64, int64_t n
     if (sh) {
         if (variant != RFOE_VARIANT_SP2 && variant != RFOE_VARIANT_SP2_ACCEL) return fail(RFOE_ERR_UNSUPPORTED);
         int64_t b, c;
-        if (rfoe_shard_range(h->n_tiles, sh->rank, sh->world, &b, &c) != RFOE_OK || !sh->allgather) return fail(RFOE_ERR_INVALID_ARG);
+        if (rfoe_shard_range(h->n_tiles, sh->rank, sh->world, &b, &c) != RFOE_OK || (!sh->allgather && !sh->barrier))
+            return fail(RFOE_ERR_INVALID_ARG);
         t_begin = (int)b; t_count = (int)c;
         c_max = (h->n_tiles + sh->world - 1) / sh->world;
+    }
+    PeerSet psets[2] = {};
+    if (sh && sh->barrier) {
+        for (int w = 0; w < 2; ++w) {
+            psets[w].n = sh->world;
+            psets[w].rec_offset = t_begin;
+            for (int d = 0; d < sh->world; ++d) { psets[w].out[d] = h->peer_W[w][d]; psets[w].rec[d] = h->peer_rec[w][d]; }
+        }
+        if (!h->d_peers && cudaMalloc(&h->d_peers, 2 * sizeof(PeerSet)) != cudaSuccess) { cudaGetLastError(); return fail(RFOE_ERR_ALLOC); }
+        CK(cudaMemcpyAsync(h->d_peers, psets, sizeof(psets), cudaMemcpyHostToDevice, st));
+        CK(cudaStreamSynchronize(st));   // psets lives on this stack frame
+    }
+    if (sh && sh->allgather) {
         rank_stride = (size_t)c_max * (TILE_ELEMS + SQ_NPART);
         const size_t need = rank_stride * sh->world * sizeof(double);
         if (h->sh_bytes < need) {
@@ -581,7 +615,19 @@ static int expand_impl(rfoe_handle_t h, const double* Hp, int64_t k64, int64_t n
     h->sq_n = 0;
     while (action != ACT_STOP) {
         const int nxt = cur ^ 1;
-        if (action == ACT_SP2 && sh) {
+        if (action == ACT_SP2 && sh && sh->barrier) {
+            // the epilogues of this rank's tiles store X_{n+1} and the records into EVERY rank's arrays (peer memory);
+            // after the barrier every rank holds the whole X_{n+1} and all records in global tile order
+            if (t_count > 0) {
+                CK(cudaEventRecord(h->sq_ev[2 * h->sq_n], st));
+                CK(launch_sp2_range(h, tm[cur], h->W[cur], nullptr, n, ld, k, &h->d_ctrl->coef, nullptr, t_begin, t_count, plan, st,
+                                    &psets[nxt], h->d_peers + nxt));
+                CK(cudaEventRecord(h->sq_ev[2 * h->sq_n + 1], st));
+                h->sq_n++;
+            }
+            if (sh->barrier(sh->user, stream) != 0) return fail(RFOE_ERR_CUDA);
+            control_kernel<<<1, 256, 0, st>>>(h->d_ctrl, 1, h->part[nxt], h->part[nxt], h->n_tiles, h->d_word);
+        } else if (action == ACT_SP2 && sh) {
             // this rank's tiles (and their mirrors) -> W[nxt]; pack them with their records; ONE all-gather; unpack
             // the foreign tiles; the records, now in global tile order, feed the same control kernel on every rank
             if (t_count > 0) {
@@ -670,7 +716,75 @@ extern "C" int rfoe_expand_sharded(rfoe_handle_t h, const double* Hp, int64_t k,
                                    int rank, int world, rfoe_allgather_fn allgather, void* user, rfoe_stream_t stream)
 {
     if (world < 1 || rank < 0 || rank >= world || !allgather) return RFOE_ERR_INVALID_ARG;
-    ShardCtx sh = {rank, world, allgather, user};
+    ShardCtx sh = {rank, world, allgather, nullptr, user};
+    return expand_impl(h, Hp, k, nocc, variant, tol, P, stream, &sh);
+}
+
+// ---- sharded expansion over peer memory ------------------------------------------------------------------
+extern "C" int rfoe_shard_local_ptrs(rfoe_handle_t h, void** ptrs)
+{
+    if (!h || !ptrs) return RFOE_ERR_INVALID_ARG;
+    ptrs[0] = h->W[0]; ptrs[1] = h->W[1]; ptrs[2] = h->part[0]; ptrs[3] = h->part[1];
+    return RFOE_OK;
+}
+
+extern "C" int rfoe_shard_set_peers(rfoe_handle_t h, int rank, int world, void* const* ptrs)
+{
+    if (!h || !ptrs || world < 1 || world > SQ_MAX_PEERS || rank < 0 || rank >= world) return RFOE_ERR_INVALID_ARG;
+    if (ptrs[4 * rank] != h->W[0] || ptrs[4 * rank + 1] != h->W[1] || ptrs[4 * rank + 2] != h->part[0] ||
+        ptrs[4 * rank + 3] != h->part[1])
+        return RFOE_ERR_INVALID_ARG;
+    for (int d = 0; d < world; ++d) {
+        for (int q = 0; q < 4; ++q)
+            if (!ptrs[4 * d + q]) return RFOE_ERR_INVALID_ARG;
+        h->peer_W[0][d] = (double*)ptrs[4 * d];
+        h->peer_W[1][d] = (double*)ptrs[4 * d + 1];
+        h->peer_rec[0][d] = (double*)ptrs[4 * d + 2];
+        h->peer_rec[1][d] = (double*)ptrs[4 * d + 3];
+    }
+    h->p2p_world = world;
+    h->p2p_rank = rank;
+    return RFOE_OK;
+}
+
+extern "C" int rfoe_shard_ipc_export(rfoe_handle_t h, void* handles)
+{
+    if (!h || !handles) return RFOE_ERR_INVALID_ARG;
+    static_assert(sizeof(cudaIpcMemHandle_t) == RFOE_IPC_HANDLE_BYTES, "IPC handle size");
+    cudaIpcMemHandle_t* out = (cudaIpcMemHandle_t*)handles;
+    CK(cudaSetDevice(h->device));
+    CK(cudaIpcGetMemHandle(&out[0], h->W[0]));
+    CK(cudaIpcGetMemHandle(&out[1], h->W[1]));
+    CK(cudaIpcGetMemHandle(&out[2], h->part[0]));
+    CK(cudaIpcGetMemHandle(&out[3], h->part[1]));
+    return RFOE_OK;
+}
+
+extern "C" int rfoe_shard_ipc_import(rfoe_handle_t h, int rank, int world, const void* handles)
+{
+    if (!h || !handles || world < 1 || world > SQ_MAX_PEERS || rank < 0 || rank >= world) return RFOE_ERR_INVALID_ARG;
+    const cudaIpcMemHandle_t* in = (const cudaIpcMemHandle_t*)handles;
+    CK(cudaSetDevice(h->device));
+    for (int i = 0; i < h->n_ipc_opened; ++i) cudaIpcCloseMemHandle(h->ipc_opened[i]);
+    h->n_ipc_opened = 0;
+    void* ptrs[4 * SQ_MAX_PEERS];
+    for (int d = 0; d < world; ++d) {
+        if (d == rank) { ptrs[4 * d] = h->W[0]; ptrs[4 * d + 1] = h->W[1]; ptrs[4 * d + 2] = h->part[0]; ptrs[4 * d + 3] = h->part[1]; continue; }
+        for (int q = 0; q < 4; ++q) {
+            void* p = nullptr;
+            CK(cudaIpcOpenMemHandle(&p, in[4 * d + q], cudaIpcMemLazyEnablePeerAccess));
+            h->ipc_opened[h->n_ipc_opened++] = p;
+            ptrs[4 * d + q] = p;
+        }
+    }
+    return rfoe_shard_set_peers(h, rank, world, ptrs);
+}
+
+extern "C" int rfoe_expand_sharded_p2p(rfoe_handle_t h, const double* Hp, int64_t k, int64_t nocc, int variant, double tol, double* P,
+                                       rfoe_barrier_fn barrier, void* user, rfoe_stream_t stream)
+{
+    if (!h || !barrier || h->p2p_world < 1) return RFOE_ERR_INVALID_ARG;
+    ShardCtx sh = {h->p2p_rank, h->p2p_world, nullptr, barrier, user};
     return expand_impl(h, Hp, k, nocc, variant, tol, P, stream, &sh);
 }
 

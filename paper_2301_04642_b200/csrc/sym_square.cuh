@@ -36,7 +36,20 @@ struct StepCoef {
     double c2, c1, c0;
 };
 
+// MODE 3 (one expansion sharded over several GPUs): the epilogue stores every output tile, its
+// mirror and its partial record into the X_{n+1} / record arrays of ALL ranks -- out[d], rec[d] are peer-mapped
+// device pointers (NVLink P2P), own rank included -- so the all-gather IS the epilogue's stores, spread over the
+// whole launch, and no pack / collective / unpack pass exists.  rec_offset = global index of the launch's first tile.
+constexpr int SQ_MAX_PEERS = 16;
+struct PeerSet {
+    double* out[SQ_MAX_PEERS];
+    double* rec[SQ_MAX_PEERS];
+    int n;
+    int rec_offset;
+};
+
 // MODE 0: squaring (A = B = X_n, one tensor map).  MODE 1: symmetric product of two matrices (McWeeny).
+// MODE 3: MODE 0 with the epilogue's stores going to every rank of a sharded run (PeerSet above, passed through `Out`).
 // MODE 2: Rayleigh-Ritz projection H^p = Psi HPsi^T: the contraction runs over the M degrees
 //         of freedom (kt_total chunks of 16, ragged tail zero-filled by TMA), split into gridDim.y slices of
 //         kt_per_slice chunks so that tiles x slices fills the 148 SMs evenly; the raw 128 x 128 accumulators go
@@ -52,7 +65,11 @@ sym_square_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
                   const StepCoef* __restrict__ coef, const int2* __restrict__ tile_map,
                   double* __restrict__ partials, int kt_per_slice)
 {
-    constexpr bool TWO_OP = (MODE != 0);
+    constexpr bool TWO_OP = (MODE == 1 || MODE == 2);
+    constexpr bool P2P = (MODE == 3);
+    // MODE 3 has no single output matrix: `Out` carries a pointer to the PeerSet in device memory instead (the
+    // parameter list is kept as it is because any change to it perturbs ptxas' schedule of the MODE 0 main loop)
+    const PeerSet& peers = *reinterpret_cast<const PeerSet*>(Out);
     extern __shared__ uint8_t smem_raw[];
     __shared__ __align__(8) uint64_t full_bar[SQ_STAGES];
     __shared__ __align__(8) uint64_t empty_bar[SQ_STAGES];
@@ -226,6 +243,7 @@ sym_square_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
                         p_err = fma(w * d, d, p_err);
                         p_ce = fma(w * cv[u], ev[u], p_ce);
                     }
+                    if (P2P) continue;
                     if (!diag) {
                         *reinterpret_cast<double2*>(Out + (size_t)row * ld + col) = make_double2(o[p][0], o[p][1]);
                         *reinterpret_cast<double2*>(Out + (size_t)row * ld + col + 2) = make_double2(o[p][2], o[p][3]);
@@ -234,6 +252,35 @@ sym_square_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
                         for (int u = 0; u < 4; ++u)
                             if (col + u >= row) Out[(size_t)row * ld + col + u] = o[p][u];
                     }
+                }
+                if (P2P) {
+                    // the same direct and mirrored stores, to every rank's X_{n+1}
+                    const int row0 = row_base + 16 * g;
+                    for (int d = 0; d < peers.n; ++d) {
+                        double* O = peers.out[d];
+#pragma unroll
+                        for (int p = 0; p < 2; ++p) {
+                            const int row = row0 + p;
+                            if (!diag) {
+                                *reinterpret_cast<double2*>(O + (size_t)row * ld + col) = make_double2(o[p][0], o[p][1]);
+                                *reinterpret_cast<double2*>(O + (size_t)row * ld + col + 2) = make_double2(o[p][2], o[p][3]);
+                            } else {
+#pragma unroll
+                                for (int u = 0; u < 4; ++u)
+                                    if (col + u >= row) O[(size_t)row * ld + col + u] = o[p][u];
+                            }
+                        }
+#pragma unroll
+                        for (int u = 0; u < 4; ++u) {
+                            if (!diag) {
+                                *reinterpret_cast<double2*>(O + (size_t)(col + u) * ld + row0) = make_double2(o[0][u], o[1][u]);
+                            } else {
+                                if (col + u > row0) O[(size_t)(col + u) * ld + row0] = o[0][u];
+                                if (col + u > row0 + 1) O[(size_t)(col + u) * ld + row0 + 1] = o[1][u];
+                            }
+                        }
+                    }
+                    continue;
                 }
                 // mirrored store: element (row, col+u) -> (col+u, row); rows 2r and 2r+1 are adjacent
                 const int row0 = row_base + 16 * g;
@@ -266,7 +313,11 @@ sym_square_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
         double v = 0.0;
 #pragma unroll
         for (int w = 0; w < SQ_CONSUMER_WARPS; ++w) v += red[w][threadIdx.x];
-        partials[(size_t)blockIdx.x * SQ_NPART + threadIdx.x] = v;
+        if (P2P) {
+            for (int d = 0; d < peers.n; ++d) peers.rec[d][(size_t)(peers.rec_offset + (int)blockIdx.x) * SQ_NPART + threadIdx.x] = v;
+        } else {
+            partials[(size_t)blockIdx.x * SQ_NPART + threadIdx.x] = v;
+        }
     }
 }
 

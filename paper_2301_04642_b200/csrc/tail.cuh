@@ -5,7 +5,8 @@
 // into S slices (T x S CTAs fill whole waves of 1/S the length) and stores raw accumulators tile-contiguously;
 // tail_fixup_kernel below adds the slices in ascending order and applies exactly the fused epilogue of the main
 // kernel: Out = c2 C + c1 E + c0 I to (I,J) and mirrored to (J,I), and the five partial sums of the tile
-// (PAPER.md:39, 72).  Which tiles are tail tiles depends only on (n_t, K extent, SM count), so a sharded run
+// (PAPER.md:39, 72), to every destination of `dst` (one for a single-GPU run, all ranks for a sharded P2P run).
+// Which tiles are tail tiles depends only on (n_t, K extent, SM count), so a sharded run
 // computes every tile with the same arithmetic as the single-GPU run.
 #pragma once
 #include "sym_square.cuh"
@@ -16,8 +17,8 @@ constexpr int TAIL_THREADS = 1024;   // 32 x 32: one element of every 32 x 32 su
 
 __global__ void __launch_bounds__(TAIL_THREADS)
 tail_fixup_kernel(const double* __restrict__ ws, int n_slices, int n_tail, const int2* __restrict__ tile_map,
-                  const double* __restrict__ E, double* __restrict__ Out, int ld, int kvalid,
-                  const StepCoef* __restrict__ coef, double* __restrict__ rec)
+                  const double* __restrict__ E, int ld, int kvalid,
+                  const StepCoef* __restrict__ coef, const __grid_constant__ PeerSet dst)
 {
     __shared__ double sm[32][33];
     __shared__ double red[5][32];
@@ -57,7 +58,8 @@ tail_fixup_kernel(const double* __restrict__ ws, int n_slices, int n_tail, const
                     }
                 }
                 sm[ty][tx] = v;
-                if (!diag || col >= row) Out[(size_t)row * ld + col] = v;
+                if (!diag || col >= row)
+                    for (int q = 0; q < dst.n; ++q) dst.out[q][(size_t)row * ld + col] = v;
                 p_ss = fma(w * v, v, p_ss);
                 p_err = fma(w * d, d, p_err);
                 p_ce = fma(w * cv, ev, p_ce);
@@ -66,7 +68,8 @@ tail_fixup_kernel(const double* __restrict__ ws, int n_slices, int n_tail, const
             {
                 // mirrored element (col, row): col = J*128 + bj*32 + ty, row = I*128 + bi*32 + tx
                 const int col = J * SQ_BM + bj * 32 + ty, row = I * SQ_BM + bi * 32 + tx;
-                if (!diag || col > row) Out[(size_t)col * ld + row] = sm[tx][ty];
+                if (!diag || col > row)
+                    for (int q = 0; q < dst.n; ++q) dst.out[q][(size_t)col * ld + row] = sm[tx][ty];
             }
         }
     if (!diag) { p_ss *= 2.0; p_err *= 2.0; p_ce *= 2.0; }
@@ -84,7 +87,7 @@ tail_fixup_kernel(const double* __restrict__ ws, int n_slices, int n_tail, const
         double v = 0.0;
         if (threadIdx.x < 5)
             for (int w = 0; w < 32; ++w) v += red[threadIdx.x][w];
-        rec[(size_t)blockIdx.x * SQ_NPART + threadIdx.x] = v;
+        for (int q = 0; q < dst.n; ++q) dst.rec[q][(size_t)(dst.rec_offset + (int)blockIdx.x) * SQ_NPART + threadIdx.x] = v;
     }
 }
 

@@ -114,3 +114,99 @@ def test_sharded_rejects_unsupported_variants_and_failing_exchange():
             h.expand_sharded(H, w.nocc, rfoe.SP2, w.tol, rank=2, world=2, allgather=lambda *a: 0)
         with pytest.raises(ZeroDivisionError):                            # an exception in the callback surfaces in Python
             h.expand_sharded(H, w.nocc, rfoe.SP2, w.tol, rank=0, world=1, allgather=lambda *a: 1 // 0)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# the exchange fused into the squaring kernel: epilogue stores go to every rank's X_{n+1} (peer memory)
+def _run_p2p_threads(H, nocc, variant, tol, g, configure=None):
+    """g ranks as threads of this process: raw device pointers stand in for peer-mapped ones (same GPU)."""
+    bar = threading.Barrier(g, timeout=120)
+    handles = [rfoe.Rfoe(H.shape[0]) for _ in range(g)]
+    ptrs = [p for h in handles for p in h.shard_local_ptrs()]
+    out, errs = [None] * g, []
+
+    def work(rank):
+        try:
+            torch.cuda.set_device(0)
+            h = handles[rank]
+            h.shard_set_peers(rank, g, ptrs)
+            if configure:
+                h.configure(**configure)
+            st = torch.cuda.Stream()
+
+            def barrier(stream_ptr):
+                st.synchronize()
+                bar.wait()
+                return 0
+
+            with torch.cuda.stream(st):
+                out[rank] = h.expand_sharded_p2p(H, nocc, variant, tol, barrier=barrier, stream=st)
+                st.synchronize()
+        except BaseException as e:  # noqa: BLE001
+            errs.append(e)
+            bar.abort()
+
+    th = [threading.Thread(target=work, args=(r,)) for r in range(g)]
+    [t.start() for t in th]
+    [t.join(300) for t in th]
+    [h.close() for h in handles]
+    if errs:
+        raise errs[0]
+    return out
+
+
+@pytest.mark.parametrize("c,k,g", [(1, 200, 2), (2, 333, 3), (3, 640, 2), (2, 130, 5), (3, 1024, 4), (1, 100, 1)])
+def test_p2p_sharded_equals_single_gpu_bitwise(c, k, g):
+    w = rfoe_inputs.make_workload(c, k=k)
+    H = torch.from_numpy(w.H).cuda()
+    with rfoe.Rfoe(k) as h:
+        one = h.expand(H, w.nocc, rfoe.SP2, w.tol)
+    for r in _run_p2p_threads(H, w.nocc, rfoe.SP2, w.tol, g):
+        assert r.converged and r.iterations == one.iterations and r.branch == one.branch
+        assert torch.equal(r.P, one.P)
+        assert np.array_equal(r.t, one.t) and np.array_equal(r.s, one.s) and np.array_equal(r.e, one.e)
+
+
+def _ipc_worker(rank, world, port, k, c, out):
+    import os
+    import torch.distributed as dist
+
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    torch.cuda.set_device(0)
+    w = rfoe_inputs.make_workload(c, k=k)
+    H = torch.from_numpy(w.H).cuda()
+    with rfoe.Rfoe(k) as h:
+        h.shard_connect()
+        res = h.expand_sharded_p2p(H, w.nocc, rfoe.SP2, w.tol)
+        torch.cuda.synchronize()
+        dist.barrier()
+        if rank == 0:
+            one = h.expand(H, w.nocc, rfoe.SP2, w.tol)
+            out["single"] = (one.iterations, one.branch)
+            out["equal"] = bool(torch.equal(one.P, res.P))
+        out[rank] = (res.iterations, res.branch, bool(res.converged), float(torch.diagonal(res.P).sum()))
+        dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_p2p_sharded_two_processes_ipc_handles():
+    """One process per rank, CUDA IPC handles exchanged over torch.distributed (gloo), both ranks on the one GPU the
+    test box has: exercises rfoe_shard_ipc_export / _import and the default barrier."""
+    import socket
+
+    import torch.multiprocessing as mp
+
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    k, c, world = 333, 2, 2
+    with mp.Manager() as m:
+        out = m.dict()
+        mp.spawn(_ipc_worker, args=(world, port, k, c, out), nprocs=world, join=True)
+        res = dict(out)
+    w = rfoe_inputs.make_workload(c, k=k)
+    assert res["equal"]
+    for r in range(world):
+        it, br, conv, tr = res[r]
+        assert conv and (it, br) == res["single"] and abs(tr - w.nocc) < 1e-9
