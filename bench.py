@@ -234,8 +234,19 @@ def run_ours(args) -> int:
     if shard and world > 1:
         dist.broadcast(H, src=0)         # one problem, the same bytes on every rank
 
+    if args.shard == "p2p":
+        h.shard_connect()                # CUDA IPC handles of the work buffers, exchanged over the process group
+
+    def p2p_barrier(stream_ptr):         # every rank's enqueued work complete, then a cross-rank barrier
+        stream.synchronize()
+        if world > 1:
+            dist.barrier(device_ids=[local])
+        return 0
+
     def step():
-        if shard:   # ONE expansion over all ranks: tile ranges + one NCCL all-gather per step
+        if args.shard == "p2p":    # ONE expansion over all ranks, exchange fused into the epilogue
+            return h.expand_sharded_p2p(H, nocc, rfoe.SP2, tol, P=P, barrier=p2p_barrier, stream=stream)
+        if shard:                  # the same with pack + one NCCL all-gather + unpack per step
             return h.expand_sharded(H, nocc, rfoe.SP2, tol, P=P, rank=rank, world=world, stream=stream)
         return h.expand(H, nocc, rfoe.SP2, tol, P=P, stream=stream)
 
@@ -294,7 +305,9 @@ def run_ours(args) -> int:
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": f"BASELINE.json config {args.config}: k={k}, nocc={nocc}, SP2, stop rule A tol {tol:.3g}, "
                                    "Gershgorin bounds, H^p = Q diag(lambda) Q^T seeded",
-                       "parallelism": (f"sharded: one expansion over {world} GPUs, tile ranges + one NCCL all-gather per step" if shard
+                       "parallelism": (f"sharded ({args.shard}): one expansion over {world} GPUs, tile ranges, "
+                                        + ("epilogue stores to every rank over peer memory + one barrier per step" if args.shard == "p2p"
+                                           else "one NCCL all-gather per step") if shard
                                        else "replicas only: one independent expansion per GPU, no collective"),
                        "l2": f"inputs larger than L2 (each matrix {8.0 * k * k / 1e6:.0f} MB vs 126 MB L2); no flush needed",
                        "squarings_per_expansion": iters, "branch": res.branch},
@@ -435,8 +448,9 @@ def main() -> int:
     ap.add_argument("--cpu-k", type=int, default=2048, help="size of the oracle's bounded sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-reduced", action="store_true", help="skip the separately reported reduced-precision run")
-    ap.add_argument("--shard", action="store_true",
-                    help="N > 1: shard ONE expansion over the ranks (strong scaling) instead of independent replicas")
+    ap.add_argument("--shard", nargs="?", const="p2p", default=None, choices=["p2p", "allgather"],
+                    help="N > 1: shard ONE expansion over the ranks (strong scaling) instead of independent replicas; p2p (default): "
+                         "epilogue stores to all ranks' memory over NVLink + one barrier per step; allgather: NCCL all-gather per step")
     ap.add_argument("--no-subspace", action="store_true", help="skip the separately reported Rayleigh-Ritz / apply steps")
     ap.add_argument("--only-subspace", action="store_true", help="run only the Rayleigh-Ritz / apply chain (ncu captures)")
     ap.add_argument("--subspace-k", type=int, default=4096)
