@@ -82,7 +82,7 @@ class ClockSampler:
         return self
 
     def stop(self) -> dict:
-        out = {"sm_mhz": None, "sm_max_mhz": None, "power_w_max": None, "samples": 0, "reasons": []}
+        out = {"sm_mhz": None, "sm_max_mhz": None, "power_w_max": None, "power_w_mean": None, "samples": 0, "reasons": []}
         if self.proc is not None:
             time.sleep(0.25)
             self.proc.terminate()
@@ -108,7 +108,8 @@ class ClockSampler:
                 if val == "Active":
                     reasons.add(name)
         if sm:
-            out.update(sm_mhz=statistics.median(sm), sm_max_mhz=max(smax), power_w_max=max(pw), samples=len(sm),
+            out.update(sm_mhz=statistics.median(sm), sm_max_mhz=max(smax), power_w_max=max(pw), power_w_mean=statistics.fmean(pw),
+                       samples=len(sm),
                        reasons=sorted(reasons))
         return out
 
@@ -325,6 +326,13 @@ def run_ours(args) -> int:
             "clocks": {"sm_mhz": clocks["sm_mhz"], "sm_max_mhz": clocks["sm_max_mhz"], "reasons": clocks["reasons"],
                        "power_w_max": clocks["power_w_max"], "samples": clocks["samples"]},
         }
+        if clocks.get("power_w_mean"):
+            # the paper's energy metric is TDP x time, an upper bound; here: mean board power sampled by
+            # nvidia-smi during the timed region x seconds per expansion
+            sec = ms_total / args.steps / 1e3
+            line["energy"] = {"mean_power_w": clocks["power_w_mean"], "joules_per_expansion": clocks["power_w_mean"] * sec,
+                              "wh_per_expansion": clocks["power_w_mean"] * sec / 3600.0,
+                              "gflops_per_watt": value * 1e3 / clocks["power_w_mean"]}
         if want_reduced:
             line["reduced_precision"] = reduced_report(h, rfoe, w, H, P, stream, ms_total / args.steps)
         if world == 1 and not args.no_subspace:
