@@ -354,7 +354,7 @@ def run_ours(args) -> int:
 
 def reduced_report(h, rfoe, w, H, P, stream, fp64_ms):
     """Row A8, reported separately from the FP64 headline: the same workload through RFOE_VARIANT_SP2_MIXED with
-    the paper's schedule (reduced-precision squarings -- 3xTF32 on tcgen05 -- from the first step until
+    the paper's schedule (reduced-precision squarings -- three FP16-part products on tcgen05 -- from the first step until
     RelTr <= 5e-4, FP64 afterwards).  Accuracy is measured against the construction-exact
     projector Q_occ Q_occ^T and the exact band energy (harness algebra in torch)."""
     import torch
@@ -388,7 +388,7 @@ def reduced_report(h, rfoe, w, H, P, stream, fp64_ms):
             "errP_vs_exact_projector": torch.linalg.norm(P - Pex).item() / math.sqrt(k),
             "rel_band_energy_error": abs(r_late.tr_PH - eband) / abs(eband)}
     h.configure(mixed_reltr=5e-4)
-    return {"variant": "SP2_MIXED, paper schedule (reduced precision until RelTr <= 5e-4)", "dtype": "3xTF32 (tcgen05 kind::tf32, FP32 accumulate) + f64",
+    return {"variant": "SP2_MIXED, paper schedule (reduced precision until RelTr <= 5e-4)", "dtype": "3xFP16 parts (tcgen05 kind::f16, FP32 accumulate, FP64 epilogue) + f64",
             "seconds_per_expansion": ms / 1e3, "speedup_vs_fp64": fp64_ms / ms, "iterations": r.iterations,
             "reduced_steps": r.fp32_steps, "converged": bool(r.converged),
             "errP_vs_exact_projector": err, "rel_band_energy_error": abs(r.tr_PH - eband) / abs(eband),

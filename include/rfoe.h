@@ -45,7 +45,7 @@ typedef enum {
  *  SP2        Z-RFOE with second-order projection polynomials           PAPER.md:35-39 (sec. II.B.1)
  *  MCWEENY    SP2 until (Tr X - Tr X^2) < 3/16 and |Tr X - N_occ| < 1/2, then X <- 3X^2 - 2X^3
  *             (purification, cited only: PAPER.md:23; reading R11 in DESIGN.md)
- *  SP2_MIXED  reduced-precision (3xTF32, FP32 accumulate) squarings far from convergence, FP64 afterwards,
+ *  SP2_MIXED  reduced-precision (three FP16-part products on tcgen05, FP32 accumulate) squarings far from convergence, FP64 afterwards,
  *             switch tied to RelTr; optional FP64 head (RFOE_OPT_MIXED_HEAD)
  *  SP2_ACCEL  A-Z-RFOE: shifted-and-scaled SP2 polynomials from HOMO/LUMO estimates
  *                                                                       PAPER.md:43 (sec. II.B.2)
@@ -130,9 +130,10 @@ int rfoe_square(rfoe_handle_t h, const double* X, int64_t k, double c2, double c
                 double* scalars, float* kernel_ms, rfoe_stream_t stream);
 
 /* The same step with the reduced-precision product of the mixed variant: X is split into
- * tf32 parts X = Xh + Xl and X X is taken as Xh Xh + Xh Xl + Xl Xh on the tcgen05 tensor cores with FP32
+ * 11-bit (scaled FP16) parts X = Xh + Xl and X X is taken as Xh Xh + Xh Xl + Xl Xh on the tcgen05 tensor cores with FP32
  * accumulation (about FP32 accuracy); the update, mirror and the five scalars are FP64 as in rfoe_square.
- * kernel_ms covers the split pass and the product kernel. */
+ * kernel_ms covers the split pass and the product kernel.  Contract: |X_ij - (Tr X / k) delta_ij| < 2 (true for every
+ * iterate of an expansion, whose spectrum lies in [0,1]); larger entries are clamped. */
 int rfoe_square_reduced(rfoe_handle_t h, const double* X, int64_t k, double c2, double c1, double c0, double* Xout,
                         double* scalars, float* kernel_ms, rfoe_stream_t stream);
 

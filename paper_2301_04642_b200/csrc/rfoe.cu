@@ -16,7 +16,7 @@
 #include "shard.cuh"
 #include "subspace.cuh"
 #include "sym_square.cuh"
-#include "sym_square_tf32.cuh"
+#include "sym_square_reduced.cuh"
 #include "tail.cuh"
 
 using namespace rfoe;
@@ -41,7 +41,7 @@ struct rfoe_handle_s {
     int64_t k_max = 0;
     int ld_max = 0;
     double* W[3] = {nullptr, nullptr, nullptr};
-    float* F[2] = {nullptr, nullptr};   // tf32 hi / lo copies of X_n for the reduced-precision squaring (lazy)
+    tq_elem_t* F[2] = {nullptr, nullptr};   // hi / lo parts (FP16, scaled) of X_n - (Tr X_n / k) I for the reduced-precision squaring (lazy)
     double* part[2] = {nullptr, nullptr};
     double* rows[2] = {nullptr, nullptr};
     double* d_bounds = nullptr;
@@ -146,13 +146,13 @@ static int make_map(rfoe_handle_s* h, CUtensorMap* map, double* base, int n, int
     return RFOE_OK;
 }
 
-static int make_map32(rfoe_handle_s* h, CUtensorMap* map, float* base, int n, int ld32)
+static int make_map_parts(rfoe_handle_s* h, CUtensorMap* map, tq_elem_t* base, int n, int ld32)
 {
     cuuint64_t dims[2] = {(cuuint64_t)n, (cuuint64_t)n};
-    cuuint64_t strides[1] = {(cuuint64_t)ld32 * sizeof(float)};
+    cuuint64_t strides[1] = {(cuuint64_t)ld32 * sizeof(tq_elem_t)};
     cuuint32_t box[2] = {(cuuint32_t)TQ_BK, (cuuint32_t)(TQ_BM / 2)};   // half panels: 64 rows x 128 bytes
     cuuint32_t estr[2] = {1, 1};
-    CUresult r = h->encode(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, base, dims, strides, box, estr,
+    CUresult r = h->encode(map, sizeof(tq_elem_t) == 2 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, base, dims, strides, box, estr,
                            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) {
@@ -162,20 +162,20 @@ static int make_map32(rfoe_handle_s* h, CUtensorMap* map, float* base, int n, in
     return RFOE_OK;
 }
 
-static int ensure_tf32(rfoe_handle_s* h)
+static int ensure_parts(rfoe_handle_s* h)
 {
     const size_t ld = (size_t)h->ld_max;
-    for (float*& p : h->F)
-        if (!p && cudaMalloc(&p, ld * (ld + TQ_PAD) * sizeof(float)) != cudaSuccess) { cudaGetLastError(); return RFOE_ERR_ALLOC; }
+    for (tq_elem_t*& p : h->F)
+        if (!p && cudaMalloc(&p, ld * (ld + TQ_PAD) * sizeof(tq_elem_t)) != cudaSuccess) { cudaGetLastError(); return RFOE_ERR_ALLOC; }
     return RFOE_OK;
 }
 
-// reduced-precision step: split X (FP64, in Xin) into tf32 hi / lo, then the tcgen05 squaring with the FP64 epilogue
-static cudaError_t launch_square_tf32(rfoe_handle_s* h, const CUtensorMap& hi, const CUtensorMap& lo, const double* Xin,
+// reduced-precision step: split X (FP64, in Xin) into its hi / lo parts, then the tcgen05 squaring with the FP64 epilogue
+static cudaError_t launch_square_reduced(rfoe_handle_s* h, const CUtensorMap& hi, const CUtensorMap& lo, const double* Xin,
                                       double* Out, int n, int ld, int k, const double* trace, const StepCoef* coef,
                                       double* partials, cudaStream_t st)
 {
-    split_tf32_kernel<<<hbm_grid(h, n), 256, 0, st>>>(Xin, n, ld, k, trace, h->F[0], h->F[1], n + TQ_PAD);
+    split_parts_kernel<<<hbm_grid(h, n), 256, 0, st>>>(Xin, n, ld, k, trace, h->F[0], h->F[1], n + TQ_PAD);
     h->launches++;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(2 * h->n_pairs);
@@ -190,7 +190,7 @@ static cudaError_t launch_square_tf32(rfoe_handle_s* h, const CUtensorMap& hi, c
     cfg.attrs = attr;
     cfg.numAttrs = 1;
     h->launches++;
-    return cudaLaunchKernelEx(&cfg, sym_square_tf32_kernel, hi, lo, Xin, Out, n, ld, k, trace, coef, (const int2*)h->d_pairs,
+    return cudaLaunchKernelEx(&cfg, sym_square_reduced_kernel, hi, lo, Xin, Out, n, ld, k, trace, coef, (const int2*)h->d_pairs,
                               n / TQ_BM, partials);
 }
 
@@ -307,7 +307,7 @@ extern "C" int rfoe_destroy(rfoe_handle_t h)
     if (!h) return RFOE_OK;
     cudaSetDevice(h->device);
     for (double* p : h->W) cudaFree(p);
-    for (float* p : h->F) cudaFree(p);
+    for (tq_elem_t* p : h->F) cudaFree(p);
     for (double* p : h->part) cudaFree(p);
     for (double* p : h->rows) cudaFree(p);
     cudaFree(h->d_bounds); cudaFree(h->d_scalars); cudaFree(h->d_flag); cudaFree(h->d_ctrl); cudaFree(h->d_tiles);
@@ -374,7 +374,7 @@ extern "C" int rfoe_create(rfoe_handle_t* out, int device, int64_t k_max)
         cudaFuncSetAttribute(sym_square_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, SQ_SMEM_BYTES) != cudaSuccess ||
         cudaFuncSetAttribute(sym_square_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, SQ_SMEM_BYTES) != cudaSuccess ||
         cudaFuncSetAttribute(apply_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, AP_SMEM_BYTES) != cudaSuccess ||
-        cudaFuncSetAttribute(sym_square_tf32_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TQ_SMEM_BYTES) != cudaSuccess) {
+        cudaFuncSetAttribute(sym_square_reduced_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TQ_SMEM_BYTES) != cudaSuccess) {
         rfoe_destroy(h);
         return RFOE_ERR_CUDA;
     }
@@ -506,7 +506,7 @@ static int expand_impl(rfoe_handle_t h, const double* Hp, int64_t k64, int64_t n
     h->launches = 0;
     CK(cudaSetDevice(h->device));
     if (variant == RFOE_VARIANT_MCWEENY && (rc = ensure_third(h)) != RFOE_OK) return fail(rc);
-    if (variant == RFOE_VARIANT_SP2_MIXED && (rc = ensure_tf32(h)) != RFOE_OK) return fail(rc);
+    if (variant == RFOE_VARIANT_SP2_MIXED && (rc = ensure_parts(h)) != RFOE_OK) return fail(rc);
     if ((rc = ensure_tiles(h, m, st)) != RFOE_OK) return fail(rc);
     // sharded run: this rank's contiguous range of the tile order, and the exchange buffers
     int t_begin = 0, t_count = h->n_tiles, c_max = h->n_tiles;
@@ -554,7 +554,7 @@ static int expand_impl(rfoe_handle_t h, const double* Hp, int64_t k64, int64_t n
     CUtensorMap tmF[2];
     if (variant == RFOE_VARIANT_SP2_MIXED)
         for (int i = 0; i < 2; ++i)
-            if ((rc = make_map32(h, &tmF[i], h->F[i], n, n + TQ_PAD)) != RFOE_OK) return fail(rc);
+            if ((rc = make_map_parts(h, &tmF[i], h->F[i], n, n + TQ_PAD)) != RFOE_OK) return fail(rc);
 
     CK(cudaEventRecord(h->ev0, st));
     // --- symmetry check, bounds, affine map, first decision -------------------------------------
@@ -655,7 +655,7 @@ static int expand_impl(rfoe_handle_t h, const double* Hp, int64_t k64, int64_t n
             control_kernel<<<1, 256, 0, st>>>(h->d_ctrl, 1, h->part[0], h->part[0], h->n_tiles, h->d_word);
         } else if (action == ACT_SP2_FP32) {
             CK(cudaEventRecord(h->sq_ev[2 * h->sq_n], st));
-            CK(launch_square_tf32(h, tmF[0], tmF[1], h->W[cur], h->W[nxt], n, ld, k, &h->d_ctrl->t, &h->d_ctrl->coef, h->part[0], st));
+            CK(launch_square_reduced(h, tmF[0], tmF[1], h->W[cur], h->W[nxt], n, ld, k, &h->d_ctrl->t, &h->d_ctrl->coef, h->part[0], st));
             CK(cudaEventRecord(h->sq_ev[2 * h->sq_n + 1], st));
             h->sq_n++;
             control_kernel<<<1, 256, 0, st>>>(h->d_ctrl, 1, h->part[0], h->part[0], 2 * h->n_pairs, h->d_word);
@@ -806,9 +806,9 @@ static int single_product(rfoe_handle_s* h, const double* A, const double* B, in
     for (int i = 0; i < 3; ++i)
         if ((rc = make_map(h, &tm[i], h->W[i], n, ld)) != RFOE_OK) return rc;
     if (reduced) {
-        if ((rc = ensure_tf32(h)) != RFOE_OK) return rc;
+        if ((rc = ensure_parts(h)) != RFOE_OK) return rc;
         for (int i = 0; i < 2; ++i)
-            if ((rc = make_map32(h, &tmF[i], h->F[i], n, n + TQ_PAD)) != RFOE_OK) return rc;
+            if ((rc = make_map_parts(h, &tmF[i], h->F[i], n, n + TQ_PAD)) != RFOE_OK) return rc;
     }
     pad_copy_kernel<<<hbm_grid(h, n), HBM_THREADS, 0, st>>>(A, k, n, ld, h->W[0]);
     h->launches++;
@@ -824,7 +824,7 @@ static int single_product(rfoe_handle_s* h, const double* A, const double* B, in
     if (reduced) {
         diag_sum_kernel<<<1, 256, 0, st>>>(h->W[0], k, ld, h->d_scalars + 7);      // Tr X for the shift d = Tr X / k
         h->launches++;
-        CK(launch_square_tf32(h, tmF[0], tmF[1], h->W[0], h->W[2], n, ld, k, h->d_scalars + 7, &h->d_ctrl->coef, h->part[0], st));
+        CK(launch_square_reduced(h, tmF[0], tmF[1], h->W[0], h->W[2], n, ld, k, h->d_scalars + 7, &h->d_ctrl->coef, h->part[0], st));
     }
     else if (two) CK(launch_square<true>(h, tm[0], tm[1], h->W[0], h->W[2], n, ld, k, &h->d_ctrl->coef, h->part[0], st));
     else {

@@ -1,8 +1,9 @@
 // Reduced-precision symmetric squaring on the 5th-generation tensor cores (row A8 of DESIGN.md):
 // the paper's mixed-precision RFOE runs the squarings far from convergence in FP32.
-// Here an "FP32 step" is a 3xTF32 product: X = Xh + Xl with Xh = tf32(X), Xl = tf32(X - Xh), and
+// Here an "FP32 step" is a three-product split: X = Xh + Xl with two 11-significant-bit parts (FP16, scaled; see
+// "Operand format" below), and
 //     C = Xh Xh^T  +  (Xh Xl^T + Xl Xh^T)          (Xl Xl^T, 2^-22 relative, is dropped)
-// computed by tcgen05.mma.kind::tf32 with TWO FP32 accumulators in tensor memory (the exact-product
+// computed by tcgen05.mma (kind::f16) with TWO FP32 accumulators in tensor memory (the exact-product
 // head term and the small cross terms are accumulated separately and added in FP64 in the epilogue).
 // Two measures keep the tensor cores' FP32 accumulation (which TRUNCATES: measured, a systematic bias of
 // ~(k/8) 2^-24 on coherent sums such as the diagonal of X^2, enough to push eigenvalues past 1 and make SP2
@@ -24,31 +25,57 @@
 // read it (multicast tcgen05.commit on both empty barriers).  A row with an odd number of tiles ends in a
 // phantom tile (J0+1 = m): that CTA loads zeros (TMA out-of-bounds fill), serves its half of the shared
 // panels and writes nothing but a zero partial record.
+//
+// Operand format (RFOE_REDUCED_F16, default 1).  The two parts only carry 11 significant bits each, which is what
+// FP16 holds, and |Z_ij| <= ||Z||_2 <= 1 bounds their range: with Zh = fp16(2^15 z) 2^-15 and Zl = fp16(2^26 (z - Zh))
+// 2^-26 every product Zh Zh, Zh Zl is exact in FP32 exactly as with tf32 parts, entries down to 2^-29 keep full
+// precision, and the three products run as tcgen05.mma.kind::f16 (K = 16 per instruction, twice the tf32 rate, half
+// the operand bytes through TMA and shared memory).  The scalings 2^-30 / 2^-41 are undone in the FP64 epilogue.
+// RFOE_REDUCED_F16 = 0 keeps the original tf32 parts (kind::tf32, K = 8).
 #pragma once
+#include <cuda_fp16.h>
+
 #include "ptx_sm100.cuh"
 #include "sym_square.cuh"
 
+#ifndef RFOE_REDUCED_F16
+#define RFOE_REDUCED_F16 1
+#endif
+
 namespace rfoe {
 
-constexpr int TQ_BM = 128;                 // tile rows = cols (UMMA M = N = 128, cta_group::1)
-constexpr int TQ_BK = 32;                  // floats per K chunk = one 128-byte swizzle row
+#if RFOE_REDUCED_F16
+typedef __half tq_elem_t;
+constexpr int TQ_UK = 16;                  // K of one tcgen05.mma.kind::f16
+constexpr double TQ_SCALE_HI = 32768.0;    // 2^15
+constexpr double TQ_SCALE_LO = 67108864.0; // 2^26
+#else
+typedef float tq_elem_t;
 constexpr int TQ_UK = 8;                   // K of one tcgen05.mma.kind::tf32
+constexpr double TQ_SCALE_HI = 1.0;
+constexpr double TQ_SCALE_LO = 1.0;
+#endif
+constexpr double TQ_UNSCALE_HEAD = 1.0 / (TQ_SCALE_HI * TQ_SCALE_HI);
+constexpr double TQ_UNSCALE_CROSS = 1.0 / (TQ_SCALE_HI * TQ_SCALE_LO);
+constexpr int TQ_BM = 128;                 // tile rows = cols (UMMA M = N = 128, cta_group::1)
+constexpr int TQ_BK = 128 / (int)sizeof(tq_elem_t);   // elements per K chunk = one 128-byte swizzle row (32 tf32 / 64 f16)
 constexpr int TQ_STAGES = 3;
 constexpr int TQ_THREADS = 192;
-constexpr int TQ_PANEL_BYTES = TQ_BM * TQ_BK * 4;                 // 16 KiB
+constexpr int TQ_PANEL_BYTES = TQ_BM * 128;                       // 16 KiB
 constexpr int TQ_STAGE_BYTES = 4 * TQ_PANEL_BYTES;               // A_hi, A_lo, B_hi, B_lo
 constexpr int TQ_SMEM_BYTES = TQ_STAGES * TQ_STAGE_BYTES + 1024; // + slack for 1024-byte alignment
-constexpr int TQ_CHUNK_KT = 8;             // K chunks (of 32) per tensor-memory accumulation run: 256 k values
+constexpr int TQ_CHUNK_KT = 256 / TQ_BK;   // K chunks per tensor-memory accumulation run: 256 k values
 constexpr int TQ_TMEM_COLS = 512;          // head accumulator x 2 (double-buffered) + cross-term accumulator
 constexpr int TQ_HALF_BYTES = TQ_PANEL_BYTES / 2;                // 64 rows of a panel
-constexpr int TQ_PAD = 32;                 // floats added to the row pitch of the hi / lo matrices
+constexpr int TQ_PAD = 128 / (int)sizeof(tq_elem_t);   // elements added to the row pitch of the hi / lo matrices
 
-// HBM-bound: split the FP64 work matrix (n x n, pitch ld) into tf32-rounded hi and lo FP32 matrices
-// (n x n, pitch ld32) of Z = X - d I, d = *trace / kvalid (rows >= kvalid stay zero).
-// hi = tf32(fl32(z)), lo = tf32(fl32(z - hi)) with z - hi exact in FP64.
+// HBM-bound: split the FP64 work matrix (n x n, pitch ld) into the hi and lo part matrices (n x n, pitch ld32
+// elements) of Z = X - d I, d = *trace / kvalid (rows >= kvalid stay zero).
+// FP16 parts: hi = fp16(2^15 z), lo = fp16(2^26 (z - 2^-15 hi)), the residual exact in FP64 (|z| <= 1: no overflow).
+// tf32 parts (RFOE_REDUCED_F16 = 0): hi = tf32(fl32(z)), lo = tf32(fl32(z - hi)).
 __global__ void __launch_bounds__(256)
-split_tf32_kernel(const double* __restrict__ X, int n, int ld, int kvalid, const double* __restrict__ trace,
-                  float* __restrict__ Hi, float* __restrict__ Lo, int ld32)
+split_parts_kernel(const double* __restrict__ X, int n, int ld, int kvalid, const double* __restrict__ trace,
+                  tq_elem_t* __restrict__ Hi, tq_elem_t* __restrict__ Lo, int ld32)
 {
     const double d = *trace / (double)kvalid;
     const int lane = threadIdx.x & 31;
@@ -56,13 +83,29 @@ split_tf32_kernel(const double* __restrict__ X, int n, int ld, int kvalid, const
     const int wtotal = gridDim.x * 8;
     for (int i = wglobal; i < n; i += wtotal) {
         const double2* row = reinterpret_cast<const double2*>(X + (size_t)i * ld);
+#if RFOE_REDUCED_F16
+        __half2* hrow = reinterpret_cast<__half2*>(Hi + (size_t)i * ld32);
+        __half2* lrow = reinterpret_cast<__half2*>(Lo + (size_t)i * ld32);
+#else
         float2* hrow = reinterpret_cast<float2*>(Hi + (size_t)i * ld32);
         float2* lrow = reinterpret_cast<float2*>(Lo + (size_t)i * ld32);
+#endif
 #pragma unroll 4
         for (int j = lane; j < n / 2; j += 32) {
             double2 x = row[j];
             if (2 * j == i && i < kvalid) x.x -= d;
             if (2 * j + 1 == i && i < kvalid) x.y -= d;
+#if RFOE_REDUCED_F16
+            // |z| <= ||Z||_2 <= 1 inside an expansion (spectrum of X in [0,1]); the clamp only keeps a caller's
+            // out-of-contract matrix (|z| >= 2) from producing infinities
+            x.x = fmin(fmax(x.x, -1.99), 1.99);
+            x.y = fmin(fmax(x.y, -1.99), 1.99);
+            const __half hx = __double2half(x.x * TQ_SCALE_HI), hy = __double2half(x.y * TQ_SCALE_HI);
+            const double rx = x.x - (double)__half2float(hx) * (1.0 / TQ_SCALE_HI);      // exact in FP64
+            const double ry = x.y - (double)__half2float(hy) * (1.0 / TQ_SCALE_HI);
+            hrow[j] = __halves2half2(hx, hy);
+            lrow[j] = __halves2half2(__double2half(rx * TQ_SCALE_LO), __double2half(ry * TQ_SCALE_LO));
+#else
             float2 h, l;
             h.x = to_tf32((float)x.x);
             h.y = to_tf32((float)x.y);
@@ -70,12 +113,13 @@ split_tf32_kernel(const double* __restrict__ X, int n, int ld, int kvalid, const
             l.y = to_tf32((float)(x.y - (double)h.y));
             hrow[j] = h;
             lrow[j] = l;
+#endif
         }
     }
 }
 
 __global__ void __launch_bounds__(TQ_THREADS, 1)
-sym_square_tf32_kernel(const __grid_constant__ CUtensorMap tmHi, const __grid_constant__ CUtensorMap tmLo,
+sym_square_reduced_kernel(const __grid_constant__ CUtensorMap tmHi, const __grid_constant__ CUtensorMap tmLo,
                        const double* __restrict__ E, double* __restrict__ Out, int n, int ld, int kvalid,
                        const double* __restrict__ trace, const StepCoef* __restrict__ coef,
                        const int2* __restrict__ pair_map, int m_tiles, double* __restrict__ partials)
@@ -150,7 +194,13 @@ sym_square_tf32_kernel(const __grid_constant__ CUtensorMap tmHi, const __grid_co
     } else if (warp == 1) {
         // ===== MMA issuer (converged warp, one elected lane): 3 tcgen05.mma per 8-wide k step =====
         {
+#if RFOE_REDUCED_F16
+            constexpr uint32_t idesc = umma_idesc_f16(TQ_BM, TQ_BM);
+#define RFOE_UMMA umma_f16
+#else
             constexpr uint32_t idesc = umma_idesc_tf32(TQ_BM, TQ_BM);
+#define RFOE_UMMA umma_tf32
+#endif
             int s = 0;
             uint32_t ph = 0;
             for (int kt = 0; kt < KT; ++kt) {
@@ -171,10 +221,10 @@ sym_square_tf32_kernel(const __grid_constant__ CUtensorMap tmHi, const __grid_co
                 if (elect_one()) {
 #pragma unroll
                 for (int ks = 0; ks < TQ_BK / TQ_UK; ++ks) {
-                    const uint64_t o = (uint64_t)(ks * TQ_UK * 4 >> 4);      // 32 bytes per k step, in 16-byte units
-                    umma_tf32(t_head, dAh + o, dBh + o, idesc, (kc | ks) != 0);   // head: Zh Zh^T (products exact in FP32)
-                    umma_tf32(t_cross, dAh + o, dBl + o, idesc, (kt | ks) != 0);  // cross terms: tiny, one long accumulation
-                    umma_tf32(t_cross, dAl + o, dBh + o, idesc, 1u);
+                    const uint64_t o = (uint64_t)(ks * TQ_UK * (int)sizeof(tq_elem_t) >> 4);   // 32 bytes per k step, in 16-byte units
+                    RFOE_UMMA(t_head, dAh + o, dBh + o, idesc, (kc | ks) != 0);   // head: Zh Zh^T (products exact in FP32)
+                    RFOE_UMMA(t_cross, dAh + o, dBl + o, idesc, (kt | ks) != 0);  // cross terms: tiny, one long accumulation
+                    RFOE_UMMA(t_cross, dAl + o, dBh + o, idesc, 1u);
                 }
                 umma_commit_mc(empty0 + 8 * s, (uint16_t)3);   // frees the stage in BOTH CTAs' producers' view
                 if (kc == TQ_CHUNK_KT - 1 || kt == KT - 1) umma_commit(hfull0 + 8 * hb);   // chunk complete
@@ -230,7 +280,7 @@ sym_square_tf32_kernel(const __grid_constant__ CUtensorMap tmHi, const __grid_co
 #pragma unroll
             for (int u = 0; u < 16; ++u) {
                 // X^2 = Z^2 + 2 d X - d^2 I   (Z = X - d I on rows < kvalid)
-                double cv = fma(2.0 * d, ev[u], (double)hsum[cb + u] + (double)xx[u]);
+                double cv = fma(2.0 * d, ev[u], (double)hsum[cb + u] * TQ_UNSCALE_HEAD + (double)xx[u] * TQ_UNSCALE_CROSS);
                 double v;
                 const double d0 = cv - ev[u];
                 double w = 1.0;                   // off-diagonal tiles: x2 applied once at the end

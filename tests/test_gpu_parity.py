@@ -248,8 +248,8 @@ def test_error_paths(handle):
 # ------------------------------------------------------------------ A8: reduced-precision path (reported separately)
 @pytest.mark.parametrize("k", [1, 5, 128, 130, 257, 777])
 def test_square_reduced_error_bound(handle, k):
-    """3xTF32 product with FP32 tensor-core accumulation against the FP64 oracle product.  Bound:
-    dropped Zl Zl term and tf32 rounding of Zl: 3 * 2^-22 per product; FP32 accumulation in tensor memory, one
+    """Three-part (scaled FP16 hi / lo) product with FP32 tensor-core accumulation against the FP64 oracle product.  Bound:
+    dropped Zl Zl term and 11-bit rounding of Zl: 3 * 2^-22 per product; FP32 accumulation in tensor memory, one
     truncation per 8-wide MMA block plus the in-block tree, over chunks of 256: (k/8 + 8) * 2^-23 bounds it,
     all relative to sum_l |z_il||z_lj| with Z = X - (Tr X / k) I."""
     X = _sym(k, 100 + k, scale=1.0 / math.sqrt(k))
