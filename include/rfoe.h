@@ -64,7 +64,8 @@ enum {
     RFOE_OPT_MIXED_HEAD = 5,   /* SP2_MIXED: FP64 while (Tr X - Tr X^2) >= value; 0 (default) = paper schedule */
     RFOE_OPT_MIXED_RELTR = 6,  /* SP2_MIXED: FP32 steps until RelTr <= value (default 5e-4) */
     RFOE_OPT_HOMO = 7,         /* SP2_ACCEL: estimate of the highest occupied eigenvalue of H^p */
-    RFOE_OPT_LUMO = 8          /* SP2_ACCEL: estimate of the lowest unoccupied eigenvalue of H^p */
+    RFOE_OPT_LUMO = 8,         /* SP2_ACCEL: estimate of the lowest unoccupied eigenvalue of H^p */
+    RFOE_OPT_LANCZOS_STEPS = 9 /* 0 (default): Gershgorin bounds in rfoe_expand; m in 1..64: rfoe_bounds_lanczos with m steps */
 };
 
 #define RFOE_MAX_STEPS 256
@@ -106,6 +107,17 @@ int rfoe_create(rfoe_handle_t* h, int device, int64_t k_max);
  * PAPER.md:56): eps_min = min_i (H_ii - r_i), eps_max = max_i (H_ii + r_i), r_i = sum_{j != i} |H_ij|.
  * Hp: device, k x k, read only.  eps_min / eps_max: HOST doubles, written on success.  Pure query. */
 int rfoe_bounds(rfoe_handle_t h, const double* Hp, int64_t k, double* eps_min, double* eps_max, rfoe_stream_t stream);
+
+/* Tighter "spectral bound estimates" than Gershgorin's: m steps (1..64; 24 is plenty) of the Lanczos
+ * recursion from a fixed pseudo-random start vector, T_m = tridiag(alpha, beta), and
+ *     eps_min = theta_min(T_m) - beta_m,   eps_max = theta_max(T_m) + beta_m
+ * (the estimator of Chebyshev-filtering codes: safe in practice, not a proof; reading R3b).  On a dense
+ * rotated H^p the interval is within ~1.5x of the true spectral width, against ~14x for Gershgorin at k=16384, which
+ * saves SP2 about 17 of 56 squarings.  m matrix-vector products of 8 k^2 bytes, all on the device.
+ * Hp: device, k x k, read only.  eps_min / eps_max: HOST doubles.  Use through RFOE_OPT_LANCZOS_STEPS (rfoe_expand then
+ * computes these bounds itself) or pass the result as RFOE_OPT_EPS_MIN / _MAX. */
+int rfoe_bounds_lanczos(rfoe_handle_t h, const double* Hp, int64_t k, int m, double* eps_min, double* eps_max,
+                        rfoe_stream_t stream);
 
 /* The expansion.  Hp: device, k x k, bitwise symmetric, never written.  P: device, k x k, overwritten
  * with the final iterate (bitwise symmetric); must not overlap Hp.  0 < nocc < k.  tol: threshold of

@@ -77,6 +77,8 @@ def lib():
             f = getattr(L, name)
             f.argtypes = [dp, dp, C.c_int64, C.c_int64, C.c_int64, dp]
             f.restype = None
+        L.rfoe_oracle_bounds_lanczos.argtypes = [dp, C.c_int64, C.c_int32, dp, dp, dp, dp]
+        L.rfoe_oracle_bounds_lanczos.restype = C.c_int
         L.rfoe_oracle_is_symmetric.argtypes = [dp, C.c_int64]
         L.rfoe_oracle_is_symmetric.restype = C.c_int
         L.rfoe_oracle_expand.argtypes = [dp, C.c_int64, C.c_int64, C.POINTER(_Run), dp]
@@ -238,3 +240,13 @@ def density(Psi, Y) -> np.ndarray:
     rho = np.empty(M)
     lib().rfoe_oracle_density(_p(Psi), _p(Y), k, M, M, _p(rho))
     return rho
+
+
+def bounds_lanczos(H, m: int = 24):
+    """m-step Lanczos spectral bounds (theta_min - beta_m, theta_max + beta_m); returns (emin, emax, alpha, beta)."""
+    H = _sq(H)
+    lo, hi = C.c_double(), C.c_double()
+    a = np.zeros(64)
+    b = np.zeros(65)
+    steps = lib().rfoe_oracle_bounds_lanczos(_p(H), H.shape[0], int(m), C.byref(lo), C.byref(hi), _p(a), _p(b))
+    return lo.value, hi.value, a[:steps].copy(), b[: steps + 1].copy()

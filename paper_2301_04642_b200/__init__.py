@@ -25,12 +25,12 @@ RULE_A, RULE_B = 0, 1
 MAX_STEPS = 256
 
 (OPT_STOP_RULE, OPT_MAX_ITER, OPT_EPS_MIN, OPT_EPS_MAX, OPT_CHECK_SYMMETRY, OPT_MIXED_HEAD, OPT_MIXED_RELTR,
- OPT_HOMO, OPT_LUMO) = range(9)
+ OPT_HOMO, OPT_LUMO, OPT_LANCZOS_STEPS) = range(10)
 
 OK, ERR_INVALID_ARG, ERR_ALLOC, ERR_CUDA, ERR_BAD_BOUNDS, ERR_NOT_SYMMETRIC, ERR_UNSUPPORTED, ERR_NOT_CONVERGED = range(8)
 
 # every symbol include/rfoe.h declares
-EXPORTS = ("rfoe_create", "rfoe_bounds", "rfoe_expand", "rfoe_expand_host", "rfoe_square", "rfoe_square_reduced",
+EXPORTS = ("rfoe_create", "rfoe_bounds", "rfoe_bounds_lanczos", "rfoe_expand", "rfoe_expand_host", "rfoe_square", "rfoe_square_reduced",
            "rfoe_symm_product", "rfoe_project", "rfoe_apply", "rfoe_expand_sharded", "rfoe_shard_range",
            "rfoe_shard_local_ptrs", "rfoe_shard_set_peers", "rfoe_shard_ipc_export", "rfoe_shard_ipc_import",
            "rfoe_expand_sharded_p2p",
@@ -84,6 +84,7 @@ def load_library(path: str | None = None):
     vp, i64, dbl, dp = C.c_void_p, C.c_int64, C.c_double, C.POINTER(C.c_double)
     L.rfoe_create.argtypes = [C.POINTER(vp), C.c_int, i64]
     L.rfoe_bounds.argtypes = [vp, vp, i64, dp, dp, vp]
+    L.rfoe_bounds_lanczos.argtypes = [vp, vp, i64, C.c_int, dp, dp, vp]
     L.rfoe_expand.argtypes = [vp, vp, i64, i64, C.c_int, dbl, vp, vp]
     L.rfoe_expand_host.argtypes = [vp, vp, i64, i64, C.c_int, dbl, vp, vp]
     L.rfoe_square.argtypes = [vp, vp, i64, dbl, dbl, dbl, vp, dp, C.POINTER(C.c_float), vp]
@@ -235,7 +236,8 @@ class Rfoe:
             raise RfoeError(rc, self._L.rfoe_strerror(rc).decode())
 
     def configure(self, *, stop_rule=None, max_iter=None, bounds=None, check_symmetry=None, mixed_head=None,
-                  mixed_reltr=None, homo=None, lumo=None):
+                  mixed_reltr=None, homo=None, lumo=None, lanczos_steps=None):
+        if lanczos_steps is not None: self.set_option(OPT_LANCZOS_STEPS, lanczos_steps)
         if stop_rule is not None: self.set_option(OPT_STOP_RULE, stop_rule)
         if max_iter is not None: self.set_option(OPT_MAX_ITER, max_iter)
         if bounds is not None:
@@ -264,6 +266,16 @@ class Rfoe:
         _check_dev(Hp, "Hp")
         lo, hi = C.c_double(), C.c_double()
         rc = self._L.rfoe_bounds(self._h, C.c_void_p(Hp.data_ptr()), Hp.shape[0], C.byref(lo), C.byref(hi), _stream_ptr(stream))
+        if rc != OK:
+            self._raise(rc)
+        return lo.value, hi.value
+
+    def bounds_lanczos(self, Hp, m: int = 24, stream=None):
+        """m-step Lanczos spectral bounds (theta_min - beta_m, theta_max + beta_m)."""
+        _check_dev(Hp, "Hp")
+        lo, hi = C.c_double(), C.c_double()
+        rc = self._L.rfoe_bounds_lanczos(self._h, C.c_void_p(Hp.data_ptr()), Hp.shape[0], int(m), C.byref(lo), C.byref(hi),
+                                         _stream_ptr(stream))
         if rc != OK:
             self._raise(rc)
         return lo.value, hi.value

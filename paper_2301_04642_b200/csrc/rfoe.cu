@@ -13,6 +13,7 @@
 #include "../../include/rfoe.h"
 #include "control.cuh"
 #include "hbm_kernels.cuh"
+#include "lanczos.cuh"
 #include "shard.cuh"
 #include "subspace.cuh"
 #include "sym_square.cuh"
@@ -67,6 +68,9 @@ struct rfoe_handle_s {
     double* sh_recv = nullptr; //   and the records in global tile order (allocated on the first sharded call)
     double* sh_parts = nullptr;
     size_t sh_bytes = 0;
+    double* lz_vec = nullptr;  // Lanczos bounds: v, v_prev, w (ld_max doubles each) + block partials
+    LanczosState* lz_state = nullptr;
+    int lanczos_steps = 0;     // RFOE_OPT_LANCZOS_STEPS: 0 = Gershgorin bounds in rfoe_expand
     double* ws = nullptr;      // scratch of the projection / density steps (grown on demand)
     size_t ws_bytes = 0;
     double* stage_H = nullptr;
@@ -312,7 +316,7 @@ extern "C" int rfoe_destroy(rfoe_handle_t h)
     for (double* p : h->rows) cudaFree(p);
     cudaFree(h->d_bounds); cudaFree(h->d_scalars); cudaFree(h->d_flag); cudaFree(h->d_ctrl); cudaFree(h->d_tiles);
     cudaFree(h->d_pairs);
-    cudaFree(h->stage_H); cudaFree(h->stage_P); cudaFree(h->ws);
+    cudaFree(h->stage_H); cudaFree(h->stage_P); cudaFree(h->ws); cudaFree(h->lz_vec); cudaFree(h->lz_state);
     cudaFree(h->sh_send); cudaFree(h->sh_recv); cudaFree(h->sh_parts);
     for (int i = 0; i < h->n_ipc_opened; ++i) cudaIpcCloseMemHandle(h->ipc_opened[i]);
     cudaFree(h->d_peers);
@@ -401,6 +405,9 @@ extern "C" int rfoe_set_option(rfoe_handle_t h, int key, double value)
         case RFOE_OPT_MIXED_RELTR:
             if (!(value >= 0.0)) return RFOE_ERR_INVALID_ARG;
             h->mixed_reltr = value; return RFOE_OK;
+        case RFOE_OPT_LANCZOS_STEPS:
+            if (!(value >= 0.0 && value <= (double)LZ_MAX_STEPS)) return RFOE_ERR_INVALID_ARG;
+            h->lanczos_steps = (int)llround(value); return RFOE_OK;
         case RFOE_OPT_HOMO: h->homo = value; return RFOE_OK;
         case RFOE_OPT_LUMO: h->lumo = value; return RFOE_OK;
         default: return RFOE_ERR_UNSUPPORTED;
@@ -427,6 +434,33 @@ static int run_bounds(rfoe_handle_s* h, const double* Hp, int k, cudaStream_t st
     return RFOE_OK;
 }
 
+// A1 (optional): m-step Lanczos bounds into h->d_bounds (device) -- lanczos.cuh
+static int run_bounds_lanczos(rfoe_handle_s* h, const double* Hp, int k, int m, cudaStream_t st)
+{
+    if (m > k) m = k;
+    if (m < 1) m = 1;
+    const size_t ld = (size_t)h->ld_max;
+    if (!h->lz_vec && cudaMalloc(&h->lz_vec, (3 * ld + 4096) * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return RFOE_ERR_ALLOC; }
+    if (!h->lz_state && cudaMalloc(&h->lz_state, sizeof(LanczosState)) != cudaSuccess) { cudaGetLastError(); return RFOE_ERR_ALLOC; }
+    double* v = h->lz_vec, *vp = v + ld, *w = vp + ld, *part = w + ld;
+    int nb = (k + 255) / 256;
+    if (nb > 2 * h->sm_count) nb = 2 * h->sm_count;
+    lanczos_init_kernel<<<nb, 256, 0, st>>>(v, vp, k, part, h->lz_state);
+    h->launches++;
+    for (int j = 0; j < m; ++j) {
+        lanczos_symv_kernel<<<hbm_grid(h, k), HBM_THREADS, 0, st>>>(Hp, k, v, w, h->rows[0], part, nb, j == 0, h->lz_state);
+        if (j == 0) { lanczos_normalise_kernel<<<nb, 256, 0, st>>>(v, k, part, nb, h->lz_state); h->launches++; }
+        lanczos_update_kernel<<<nb, 256, 0, st>>>(w, v, vp, k, h->rows[0], j, part, h->lz_state);
+        lanczos_next_kernel<<<nb, 256, 0, st>>>(v, vp, w, k, part, nb, j, h->lz_state);
+        lanczos_flag_kernel<<<1, 1, 0, st>>>(h->lz_state, j);
+        h->launches += 4;
+    }
+    lanczos_bounds_kernel<<<1, 32, 0, st>>>(h->lz_state, h->d_bounds);
+    h->launches++;
+    CK(cudaGetLastError());
+    return RFOE_OK;
+}
+
 static int check_common(rfoe_handle_s* h, const void* a, const void* b, int64_t k)
 {
     if (!h) return RFOE_ERR_INVALID_ARG;
@@ -442,6 +476,25 @@ extern "C" int rfoe_bounds(rfoe_handle_t h, const double* Hp, int64_t k, double*
     h->stats.cuda_error = 0;
     CK(cudaSetDevice(h->device));
     int rc = run_bounds(h, Hp, (int)k, st);
+    if (rc != RFOE_OK) return rc;
+    CK(cudaMemcpyAsync((void*)h->hp->bounds, h->d_bounds, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    *eps_min = h->hp->bounds[0];
+    *eps_max = h->hp->bounds[1];
+    h->stats.gpu_launches = h->launches;
+    h->stats.status = RFOE_OK;
+    return RFOE_OK;
+}
+
+extern "C" int rfoe_bounds_lanczos(rfoe_handle_t h, const double* Hp, int64_t k, int m, double* eps_min, double* eps_max,
+                                   rfoe_stream_t stream)
+{
+    if (!h || !Hp || !eps_min || !eps_max || k < 1 || k > h->k_max || m < 1 || m > LZ_MAX_STEPS) return RFOE_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    h->launches = 0;
+    h->stats.cuda_error = 0;
+    CK(cudaSetDevice(h->device));
+    int rc = run_bounds_lanczos(h, Hp, (int)k, m, st);
     if (rc != RFOE_OK) return rc;
     CK(cudaMemcpyAsync((void*)h->hp->bounds, h->d_bounds, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
@@ -575,7 +628,8 @@ static int expand_impl(rfoe_handle_t h, const double* Hp, int64_t k64, int64_t n
         h->hp->bounds[0] = h->eps_min; h->hp->bounds[1] = h->eps_max;
         CK(cudaMemcpyAsync(h->d_bounds, (void*)h->hp->bounds, 2 * sizeof(double), cudaMemcpyHostToDevice, st));
     } else {
-        if ((rc = run_bounds(h, Hp, k, st)) != RFOE_OK) return fail(rc);
+        if ((rc = (h->lanczos_steps > 0 ? run_bounds_lanczos(h, Hp, k, h->lanczos_steps, st) : run_bounds(h, Hp, k, st))) != RFOE_OK)
+            return fail(rc);
         CK(cudaMemcpyAsync((void*)h->hp->bounds, h->d_bounds, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
     }
     // the check of the bounds needs them on the host before X0 is trusted: one sync (also covers sym_flag)

@@ -50,12 +50,14 @@ def main() -> int:
         runs = [("SP2 rule A, Gershgorin (normative)", rfoe.SP2, w.tol, {}),
                 ("SP2 rule B RelTr 5e-8 (paper's criterion)", rfoe.SP2, 5e-8, dict(stop_rule=rfoe.RULE_B)),
                 ("SP2 rule A, exact spectral bounds", rfoe.SP2, w.tol, dict(bounds=(float(lam.min()), float(lam.max())))),
+                ("SP2 rule A, Lanczos bounds (24 steps, on the device)", rfoe.SP2, w.tol, dict(lanczos_steps=24)),
+                ("mixed (late switch 5e-7) + Lanczos bounds", rfoe.SP2_MIXED, w.tol, dict(lanczos_steps=24, mixed_head=0.0, mixed_reltr=5e-7)),
                 ("A-Z-RFOE (accelerated), exact HOMO/LUMO", rfoe.SP2_ACCEL, w.tol, dict(homo=homo, lumo=lumo)),
                 ("McWeeny-style tail", rfoe.MCWEENY, w.tol, {}),
                 ("mixed, paper schedule (reduced until RelTr 5e-4)", rfoe.SP2_MIXED, w.tol, dict(mixed_head=0.0, mixed_reltr=5e-4))]
         with rfoe.Rfoe(k) as h:
             for name, variant, tol, opts in runs:
-                h.configure(stop_rule=rfoe.RULE_A, bounds=False, mixed_head=0.0, mixed_reltr=5e-4)
+                h.configure(stop_rule=rfoe.RULE_A, bounds=False, mixed_head=0.0, mixed_reltr=5e-4, lanczos_steps=0)
                 h.configure(**opts)
                 r = None
                 for _ in range(2):                                   # second run is the timed one (warm)
