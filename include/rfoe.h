@@ -112,8 +112,8 @@ int rfoe_bounds(rfoe_handle_t h, const double* Hp, int64_t k, double* eps_min, d
  * recursion from a fixed pseudo-random start vector, T_m = tridiag(alpha, beta), and
  *     eps_min = theta_min(T_m) - beta_m,   eps_max = theta_max(T_m) + beta_m
  * (the estimator of Chebyshev-filtering codes: safe in practice, not a proof; reading R3b).  On a dense
- * rotated H^p the interval is within ~1.5x of the true spectral width, against ~14x for Gershgorin at k=16384, which
- * saves SP2 about 17 of 56 squarings.  m matrix-vector products of 8 k^2 bytes, all on the device.
+ * rotated H^p the interval is within ~1.5x of the true spectral width, against ~50x for Gershgorin at k=16384, which
+ * saves SP2 18 of 56 squarings.  m matrix-vector products of 8 k^2 bytes, all on the device.
  * Hp: device, k x k, read only.  eps_min / eps_max: HOST doubles.  Use through RFOE_OPT_LANCZOS_STEPS (rfoe_expand then
  * computes these bounds itself) or pass the result as RFOE_OPT_EPS_MIN / _MAX. */
 int rfoe_bounds_lanczos(rfoe_handle_t h, const double* Hp, int64_t k, int m, double* eps_min, double* eps_max,

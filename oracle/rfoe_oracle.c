@@ -178,7 +178,7 @@ void rfoe_oracle_matmul(const double* A, const double* B, int64_t k, double* Y) 
 
 /* ---- tighter spectral bounds: m-step Lanczos estimate (reading R3b) ---------------------------------
  * The paper only says "spectral bound estimates"; Gershgorin (above) is the normative choice and
- * over-estimates the width of a dense rotated H^p by ~sqrt(k), which costs ~20 extra squarings.  This is the
+ * over-estimates the width of a dense rotated H^p ~50x at k=16384, which costs ~18 extra squarings.  This is the
  * standard alternative of Chebyshev-filtering codes: m steps of the Lanczos recursion from a fixed pseudo-random
  * start vector, T_m = tridiag(alpha, beta), and the bounds
  *        emin = theta_min(T_m) - beta_m,      emax = theta_max(T_m) + beta_m

@@ -1,6 +1,6 @@
 // Tighter spectral bounds than Gershgorin's (row A1, optional; reading R3b): m steps of the Lanczos
 // recursion.  The paper only says "spectral bound estimates"; on a dense rotated H^p Gershgorin
-// over-estimates the spectral width by ~sqrt(k) (14x at k=16384), which costs SP2 about 17 of its 56 squarings;
+// over-estimates the spectral width ~50x at k=16384 (radius ~0.8 sigma sqrt(k)), which costs SP2 about 18 of its 56 squarings;
 // emin = theta_min(T_m) - beta_m, emax = theta_max(T_m) + beta_m is within 1.5x of the true width after m = 24
 // matrix-vector products (8 k^2 bytes each, HBM-bound).  Everything stays on the device: the recursion's scalars
 // live in a small state block, the extreme eigenvalues of T_m come from a bisection on its Sturm count.
