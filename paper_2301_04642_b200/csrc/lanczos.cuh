@@ -207,7 +207,7 @@ __global__ void lanczos_bounds_kernel(const LanczosState* __restrict__ st, doubl
         hi = fmax(hi, a[i] + r);
     }
     const int target = (threadIdx.x == 0) ? 1 : m;     // smallest / largest eigenvalue
-    for (int it = 0; it < 200; ++it) {
+    for (int it = 0; it < 64; ++it) {    // 64 halvings of an interval a few units wide: below one ulp
         const double mid = 0.5 * (lo + hi);
         if (lz_sturm(a, b, m, mid) >= target) hi = mid; else lo = mid;
     }
