@@ -230,6 +230,24 @@ def test_paper_workload_k65536():
     del HP
     out["Z-RFOE"].update(idem=idem, comm=comm, trace_err=abs(torch.diagonal(Pz).sum().item() - nocc))
     assert torch.equal(Pz, Pz.T) and idem <= 1e-2 and comm <= 1e-2
+    # ---- the paper's mixed-precision Z-RFOE on the same problem: reduced-precision squarings until
+    # RelTr <= 5e-7 (late switch), FP64 to 5e-8; Pz waits on the host meanwhile (34 GB per matrix)
+    Pz_host = Pz.cpu()
+    del Pz
+    torch.cuda.empty_cache()
+    with rfoe.Rfoe(k) as h:
+        h.configure(stop_rule=rfoe.RULE_B, mixed_head=0.0, mixed_reltr=5e-7)
+        mres = h.expand(H, nocc, rfoe.SP2_MIXED, 5e-8)
+        Pm = mres.P
+        out["mixed Z-RFOE (late switch)"] = dict(steps=mres.iterations, reduced=mres.fp32_steps, seconds=mres.device_ms / 1e3,
+                                                 speedup=z.device_ms / mres.device_ms)
+        assert mres.converged and abs(mres.iterations - z.iterations) <= 2
+    del H
+    torch.cuda.empty_cache()
+    Pz = Pz_host.cuda()
+    eps1 = (torch.linalg.norm(Pm - Pz) / torch.linalg.norm(Pz)).item()          # the paper's eps_1 against the FP64 run
+    out["mixed Z-RFOE (late switch)"].update(eps1_vs_fp64=eps1, trace_err=abs(torch.diagonal(Pm).sum().item() - nocc))
+    assert eps1 <= 1e-5 and torch.equal(Pm, Pm.T)
     print(out)
     os.makedirs("gpurun_out", exist_ok=True)
     with open("gpurun_out/paper_k65536.txt", "w") as f:
