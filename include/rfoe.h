@@ -223,6 +223,12 @@ int rfoe_expand_sharded_p2p(rfoe_handle_t h, const double* Hp, int64_t k, int64_
  * `rank` of `world` squares: ceil(n_tiles / world) tiles each, the last ranks possibly fewer (or none). */
 int rfoe_shard_range(int64_t n_tiles, int rank, int world, int64_t* begin, int64_t* count);
 
+/* Host-only introspection (no device needed): how one squaring at size k is launched on a GPU with sm_count SMs.
+ * n_tiles upper-triangle 128 x 128 tiles; tiles [0, n_main) go to the main kernel in whole waves; the last
+ * n_tiles - n_main tiles are cut into `slices` K-slices of kt_per_slice 16-wide chunks so that the otherwise nearly
+ * empty last wave fills the SMs (slices = 1: no tail, plain launch).  DESIGN.md "Tail of a launch". */
+int rfoe_plan_squaring(int64_t k, int sm_count, int64_t* n_tiles, int64_t* n_main, int* slices, int* kt_per_slice);
+
 int rfoe_set_option(rfoe_handle_t h, int key, double value); /* INVALID_ARG on bad value, UNSUPPORTED on bad key */
 int rfoe_get_stats(rfoe_handle_t h, rfoe_stats_t* out);      /* copies the stats of the last call */
 int rfoe_destroy(rfoe_handle_t h);                           /* frees everything the handle owns; h may be null */

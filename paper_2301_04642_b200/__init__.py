@@ -31,7 +31,7 @@ OK, ERR_INVALID_ARG, ERR_ALLOC, ERR_CUDA, ERR_BAD_BOUNDS, ERR_NOT_SYMMETRIC, ERR
 
 # every symbol include/rfoe.h declares
 EXPORTS = ("rfoe_create", "rfoe_bounds", "rfoe_bounds_lanczos", "rfoe_expand", "rfoe_expand_host", "rfoe_square", "rfoe_square_reduced",
-           "rfoe_symm_product", "rfoe_project", "rfoe_apply", "rfoe_expand_sharded", "rfoe_shard_range",
+           "rfoe_symm_product", "rfoe_project", "rfoe_apply", "rfoe_expand_sharded", "rfoe_shard_range", "rfoe_plan_squaring",
            "rfoe_shard_local_ptrs", "rfoe_shard_set_peers", "rfoe_shard_ipc_export", "rfoe_shard_ipc_import",
            "rfoe_expand_sharded_p2p",
            "rfoe_set_option", "rfoe_get_stats", "rfoe_destroy", "rfoe_strerror", "rfoe_version")
@@ -98,6 +98,7 @@ def load_library(path: str | None = None):
     L.rfoe_shard_ipc_export.argtypes = [vp, vp]
     L.rfoe_shard_ipc_import.argtypes = [vp, C.c_int, C.c_int, vp]
     L.rfoe_expand_sharded_p2p.argtypes = [vp, vp, i64, i64, C.c_int, dbl, vp, BARRIER_FN, vp, vp]
+    L.rfoe_plan_squaring.argtypes = [i64, C.c_int, C.POINTER(i64), C.POINTER(i64), C.POINTER(C.c_int), C.POINTER(C.c_int)]
     L.rfoe_shard_range.argtypes = [i64, C.c_int, C.c_int, C.POINTER(i64), C.POINTER(i64)]
     L.rfoe_set_option.argtypes = [vp, C.c_int, dbl]
     L.rfoe_get_stats.argtypes = [vp, C.POINTER(_Stats)]
@@ -157,6 +158,15 @@ def _check_rect(x, name):
     if not (isinstance(x, torch.Tensor) and x.is_cuda and x.dtype == torch.float64 and x.dim() == 2 and x.stride(1) == 1
             and x.stride(0) >= x.shape[1]):
         raise ValueError(f"{name}: row-major float64 CUDA matrix (k x M, unit column stride) expected")
+
+
+def plan_squaring(k: int, sm_count: int = 148):
+    """(n_tiles, n_main, slices, kt_per_slice): how one squaring at size k is launched (host-only C call)."""
+    nt, nm, sl, per = C.c_int64(), C.c_int64(), C.c_int(), C.c_int()
+    rc = load_library().rfoe_plan_squaring(int(k), int(sm_count), C.byref(nt), C.byref(nm), C.byref(sl), C.byref(per))
+    if rc != OK:
+        raise RfoeError(rc, "rfoe_plan_squaring: invalid argument")
+    return nt.value, nm.value, sl.value, per.value
 
 
 def shard_range(n_tiles: int, rank: int, world: int):

@@ -520,6 +520,16 @@ struct ShardCtx {
     void* user;
 };
 
+extern "C" int rfoe_plan_squaring(int64_t k, int sm_count, int64_t* n_tiles, int64_t* n_main, int* slices, int* kt_per_slice)
+{
+    if (k < 1 || k > (1 << 20) || sm_count < 1 || !n_tiles || !n_main || !slices || !kt_per_slice) return RFOE_ERR_INVALID_ARG;
+    const int n = round_up(k, SQ_BM), m = n / SQ_BM;
+    const long long nt = (long long)m * (m + 1) / 2;
+    const TailPlan p = plan_tail((int)nt, n / SQ_BK, sm_count);
+    *n_tiles = nt; *n_main = p.n_main; *slices = p.slices; *kt_per_slice = p.kt_per;
+    return RFOE_OK;
+}
+
 extern "C" int rfoe_shard_range(int64_t n_tiles, int rank, int world, int64_t* begin, int64_t* count)
 {
     if (n_tiles < 1 || world < 1 || rank < 0 || rank >= world || !begin || !count) return RFOE_ERR_INVALID_ARG;

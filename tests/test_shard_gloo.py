@@ -66,3 +66,27 @@ def test_gathered_layout_is_global_tile_order_world2(n_tiles):
     got = res[0]
     assert got[:n_tiles] == list(range(n_tiles))
     assert all(v == -1 for v in got[n_tiles:])
+
+
+def test_squaring_launch_plan():
+    """Host logic of the split-K tail: whole waves for the main kernel, a tail only
+    where the cycle model gains >= 1.5 %, slices that cover the contraction."""
+    import paper_2301_04642_b200 as rfoe
+
+    for k in (1, 100, 256, 1000, 1024, 2048, 4096, 8192, 16384, 40000, 65536):
+        nt, nm, sl, per = rfoe.plan_squaring(k)
+        m = -(-k // 128)
+        kt = m * 128 // 16
+        assert nt == m * (m + 1) // 2 and 0 <= nm <= nt
+        if sl == 1:
+            assert nm == nt and per == kt                 # plain launch
+        else:
+            assert nm % 148 == 0 and nt - nm > 0          # the main kernel runs whole waves only
+            assert per >= 16 and sl * per >= kt and (sl - 1) * per < kt
+    assert rfoe.plan_squaring(16384)[2] == 1              # the headline size keeps the plain launch (measured: no gain)
+    assert rfoe.plan_squaring(40000)[2] == 1
+    nt, nm, sl, per = rfoe.plan_squaring(8192)            # 2080 tiles = 14.05 waves: the 8 left-over tiles are split 16-way
+    assert (nt, nm, sl, per) == (2080, 2072, 16, 32)
+    assert rfoe.plan_squaring(4096)[:3] == (528, 444, 7)
+    with pytest.raises(rfoe.RfoeError):
+        rfoe.plan_squaring(0)
