@@ -233,6 +233,7 @@ def test_paper_workload_k65536():
     # ---- the paper's mixed-precision Z-RFOE on the same problem: reduced-precision squarings until
     # RelTr <= 5e-7 (late switch), FP64 to 5e-8; Pz waits on the host meanwhile (34 GB per matrix)
     Pz_host = Pz.cpu()
+    z.P = None                      # the result object holds the other reference to the 34 GB matrix
     del Pz
     torch.cuda.empty_cache()
     with rfoe.Rfoe(k) as h:

@@ -171,3 +171,21 @@ def test_fullsize_chain_bench_configuration():
         Qo = w.Q[:, : w.nocc] if isinstance(w.Q, torch.Tensor) else torch.from_numpy(w.Q[:, : w.nocc]).cuda()
         rho_exact = ((Qo.T @ sub.Psi) ** 2).sum(dim=0)
         assert float((rho - rho_exact).abs().max()) <= 1e-12
+
+
+def test_project_apply_lanczos_are_bitwise_reproducible(handle):
+    """No FP atomics anywhere: K-slices, density slices and the Lanczos sums are added in a fixed order."""
+    rng = np.random.default_rng(77)
+    k, M = 640, 20002
+    Psi, Phi = _dev(rng.standard_normal((k, M))), _dev(rng.standard_normal((k, M)))
+    P = rng.standard_normal((k, k))
+    P = _dev(0.5 * (P + P.T))
+    a = handle.project(Psi, Phi)[0].clone()
+    ya, ra, _ = handle.apply(P, Psi)
+    ya, ra = ya.clone(), ra.clone()
+    la = handle.bounds_lanczos(P, 24)
+    for _ in range(3):
+        assert torch.equal(handle.project(Psi, Phi)[0], a)
+        yb, rb, _ = handle.apply(P, Psi)
+        assert torch.equal(yb, ya) and torch.equal(rb, ra)
+        assert handle.bounds_lanczos(P, 24) == la
