@@ -98,7 +98,8 @@ typedef struct {
 
 /* Create a handle on CUDA device `device` able to expand matrices up to k_max x k_max.
  * Allocates (device) three zero-padded work matrices of ceil(k_max/128)*128 squared doubles (the third
- * lazily, on the first McWeeny call; two FP32 matrices lazily on the first mixed call), per-tile reduction scratch and one pinned host page.
+ * lazily, on the first McWeeny call; two FP16 part matrices lazily on the first mixed call; further scratch lazily by
+ * the projection / apply / sharded / Lanczos entry points), per-tile reduction scratch and one pinned host page.
  * Errors: INVALID_ARG (h null, k_max < 1), CUDA (no device / wrong device), UNSUPPORTED (not sm_100),
  * ALLOC. */
 int rfoe_create(rfoe_handle_t* h, int device, int64_t k_max);
@@ -121,7 +122,7 @@ int rfoe_bounds_lanczos(rfoe_handle_t h, const double* Hp, int64_t k, int m, dou
 
 /* The expansion.  Hp: device, k x k, bitwise symmetric, never written.  P: device, k x k, overwritten
  * with the final iterate (bitwise symmetric); must not overlap Hp.  0 < nocc < k.  tol: threshold of
- * the active stop rule (finite, >= 0).  Steps: Gershgorin bounds (or the override) -> X_0 =
+ * the active stop rule (finite, >= 0).  Steps: Gershgorin bounds (or the override / Lanczos option) -> X_0 =
  * (eps_max I - H^p)/(eps_max - eps_min) -> recursion steered by Tr X_n vs N_occ (S iff Tr X_n > N_occ,
  * PAPER.md:39) -> P, tr(P H^p).  Returns OK, NOT_CONVERGED (P and stats still valid) or an error
  * (P unspecified). */
