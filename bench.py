@@ -337,7 +337,7 @@ def run_ours(args) -> int:
             line["lanczos_bounds"] = lanczos_report(h, rfoe, w, H, P, stream, ms_total / args.steps)
         if want_reduced:
             line["reduced_precision"] = reduced_report(h, rfoe, w, H, P, stream, ms_total / args.steps)
-        if world == 1 and not args.no_subspace:
+        if world == 1 and not args.no_subspace and k <= 16384:   # 59 GB of basis + generator temporaries: not beside config 5
             del Hh, Ph
             with rfoe.Rfoe(args.subspace_k, device=local) as h2:
                 line["subspace_steps"] = subspace_report(h2, rfoe, rfoe_inputs, args, dev, stream)
