@@ -334,6 +334,7 @@ def run_ours(args) -> int:
                               "wh_per_expansion": clocks["power_w_mean"] * sec / 3600.0,
                               "gflops_per_watt": value * 1e3 / clocks["power_w_mean"]}
         if world == 1 and not shard:
+            line["hbm_kernels"] = hbm_report(h, H, stream)
             line["lanczos_bounds"] = lanczos_report(h, rfoe, w, H, P, stream, ms_total / args.steps)
         if want_reduced:
             line["reduced_precision"] = reduced_report(h, rfoe, w, H, P, stream, ms_total / args.steps)
@@ -352,6 +353,31 @@ def run_ours(args) -> int:
     if dist.is_initialized():
         dist.destroy_process_group()
     return 0
+
+
+def hbm_report(h, H, stream):
+    """HBM GB/s of the bound kernels, live: rfoe_bounds = gershgorin_rows_kernel (8 k^2 bytes read) + a
+    one-block reduction, CUDA events around the call (best of 5), against the measured copy peak."""
+    import torch
+
+    k = H.shape[0]
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    best = float("inf")
+    for _ in range(5):
+        torch.cuda.synchronize()
+        e0.record(stream)
+        h.bounds(H, stream=stream)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        best = min(best, e0.elapsed_time(e1))
+    peak = None
+    try:
+        peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))).get("hbm_gbs")
+    except (OSError, ValueError):
+        pass
+    gbs = 8.0 * k * k / (best * 1e-3) / 1e9
+    return {"rfoe_bounds_ms": best, "gershgorin_gbs": gbs, "peak_gbs": peak, "frac": gbs / peak if peak else None,
+            "note": "whole rfoe_bounds call (rows kernel + reduction + 16-byte D2H); per-kernel figures: profiles/r01f_launches_k16384.md"}
 
 
 def lanczos_report(h, rfoe, w, H, P, stream, fp64_ms, m=24):
