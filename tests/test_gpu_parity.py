@@ -78,6 +78,32 @@ def test_square_parity(handle, k, coef):
         assert np.array_equal(outi.cpu().numpy(), oracle.square(Xi))
 
 
+@pytest.mark.parametrize("k", [2100, 3000])
+def test_square_parity_main_plus_tail_launch(k):
+    """Sizes whose launch is a whole-wave main part PLUS a split-K tail (rfoe_plan_squaring: n_main > 0, slices > 1),
+    ragged in both (2100 = 16*128 + 52, 3000 = 23*128 + 56): every element against the oracle, both SP2 branches."""
+    nt, nm, sl, _ = rfoe.plan_squaring(k, torch.cuda.get_device_properties(0).multi_processor_count)
+    assert 0 < nm < nt and sl > 1
+    X = _sym(k, 100 + k, scale=1.0 / math.sqrt(k))
+    Y = oracle.square(X)
+    xmax = np.abs(X).max()
+    with rfoe.Rfoe(k) as h:
+        for c2, c1 in [(1.0, 0.0), (-1.0, 2.0)]:
+            out, sc, _ = h.square(_dev(X), c2, c1, 0.0)
+            out = out.cpu().numpy()
+            ref = c2 * Y + c1 * X
+            assert np.abs(out - ref).max() <= 8 * k * EPS * xmax * xmax + 4 * EPS * np.abs(ref).max()
+            assert np.array_equal(out, out.T)
+            assert sc[0] == pytest.approx(np.trace(ref), rel=1e-12)
+            assert sc[1] == pytest.approx(np.sum(ref * ref), rel=1e-12)
+            assert sc[2] == pytest.approx(np.sum((Y - X) ** 2), rel=1e-12)
+            assert sc[3] == pytest.approx(np.sum(X * X), rel=1e-12)
+        Xi = np.random.default_rng(k).integers(-3, 4, size=(k, k)).astype(np.float64)
+        Xi = np.triu(Xi) + np.triu(Xi, 1).T
+        outi, _, _ = h.square(_dev(Xi))
+        assert np.array_equal(outi.cpu().numpy(), oracle.square(Xi))       # exact on small integers
+
+
 @pytest.mark.parametrize("k", [3, 128, 200, 515])
 def test_symm_product_parity(handle, k):
     X = _sym(k, 300 + k, scale=1.0 / math.sqrt(k))
