@@ -230,6 +230,20 @@ int rfoe_shard_range(int64_t n_tiles, int rank, int world, int64_t* begin, int64
  * empty last wave fills the SMs (slices = 1: no tail, plain launch).  DESIGN.md "Tail of a launch". */
 int rfoe_plan_squaring(int64_t k, int sm_count, int64_t* n_tiles, int64_t* n_main, int* slices, int* kt_per_slice);
 
+/* HOMO / LUMO estimates for A-Z-RFOE from the history of a finished Z-RFOE run (host only, no device needed).
+ * The paper chooses the accelerated polynomials "based on HOMO ... and LUMO ... eigenvalues" and does not
+ * say where they come from; in an SCF loop they come from the previous expansion (its refs. 31, 38; DESIGN.md reading
+ * R-HL).  Every eigenvalue x of X_n obeys x (1 - x) <= e_n = ||X_n^2 - X_n||_F, so once the occupation is settled
+ * (Tr X_n - Tr X_n^2 < 3/16 and |Tr X_n - N_occ| < 1/2, the McWeeny switch of reading R11) the image of the LUMO is
+ * <= a_n = (1 - sqrt(1 - 4 e_n))/2 and the image of the HOMO is >= 1 - a_n.  Both are carried back through the inverses
+ * of the steps taken ('S': sqrt(x), 'L': 1 - sqrt(1 - x), monotone) to X_0 and through the affine map to H^p; the
+ * tightest pair over all admissible steps with e_n >= 1e-6 (below that, rounding in X_n shows) is returned:
+ *     homo >= lambda_HOMO,  lumo <= lambda_LUMO  (up to rounding),   both inside the gap, typically within 1 % of it.
+ * stats: the rfoe_stats_t of a plain SP2 run (FP64 steps only; any stop rule; also the sharded entry points).
+ * Returns OK; UNSUPPORTED (other variant / reduced steps in the history); NOT_CONVERGED (no admissible step: run
+ * stopped too early); INVALID_ARG.  Feed the result to RFOE_OPT_HOMO / RFOE_OPT_LUMO for the next SP2_ACCEL call. */
+int rfoe_estimate_homo_lumo(const rfoe_stats_t* stats, double* homo, double* lumo);
+
 int rfoe_set_option(rfoe_handle_t h, int key, double value); /* INVALID_ARG on bad value, UNSUPPORTED on bad key */
 int rfoe_get_stats(rfoe_handle_t h, rfoe_stats_t* out);      /* copies the stats of the last call */
 int rfoe_destroy(rfoe_handle_t h);                           /* frees everything the handle owns; h may be null */

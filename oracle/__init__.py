@@ -5,8 +5,9 @@ see that file's header for the passages of PAPER.md it follows and for its pins)
 ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` / ``--impl reference``
 legs may import this package; it imports nothing from ``paper_2301_04642_b200``.
 
-Parity status: every function is pinned by tests/test_oracle_pins.py except the exact bit patterns
-of the iterates X_n ("parity unpinned" for bits -- the paper prints no worked example).
+Parity status: every function is pinned by tests/test_oracle_pins.py (estimate_homo_lumo: by
+tests/test_oracle_homo_lumo_pins.py) except the exact bit patterns of the iterates X_n ("parity unpinned" for
+bits -- the paper prints no worked example).
 """
 from __future__ import annotations
 
@@ -186,6 +187,39 @@ def expand(H, nocc: int, *, variant: int = SP2, tol: float = 1e-12, stop_rule: i
         fp32_steps=run.fp32_steps, converged=bool(run.converged), branch=run.branch.decode()[:n],
         emin=run.emin, emax=run.emax, tr_PH=run.tr_PH,
         t=np.array(run.t[: n + 1]), s=np.array(run.s[: n + 1]), e=np.array(run.e[:n]), reltr=np.array(run.reltr[:n]))
+
+
+def estimate_homo_lumo(res: OracleResult, nocc: int, e_floor: float = 1e-6):
+    """HOMO / LUMO estimates for A-Z-RFOE (PAPER.md:43: polynomials chosen "based on HOMO ... and LUMO ... eigenvalues";
+    the paper is silent on their source, reading R-HL: the history of the previous Z-RFOE run, refs. 31, 38).
+
+    Step by step: for every step n whose occupation is settled (t_n - s_n < 3/16 and |t_n - nocc| < 1/2, reading R11) and
+    whose e_n = ||X_n^2 - X_n||_F lies in [e_floor, 1/4): every eigenvalue x of X_n has x(1 - x) <= e_n, so the LUMO image
+    is <= a = (1 - sqrt(1 - 4 e_n))/2 and the HOMO image is >= 1 - a.  Undo steps n-1 .. 0 ('S' x^2 -> sqrt(x);
+    'L' 2x - x^2 -> 1 - sqrt(1 - x); both monotone), undo X_0 = (emax - lambda)/(emax - emin), keep the tightest pair.
+    Returns (homo_est, lumo_est) with homo_est >= lambda_HOMO and lumo_est <= lambda_LUMO."""
+    import math
+
+    if any(ch not in "SL" for ch in res.branch):
+        raise ValueError("history of a plain FP64 SP2 run expected")
+    w = res.emax - res.emin
+    homo, lumo = math.inf, -math.inf
+    for n in range(res.iterations):
+        t, s, e = float(res.t[n]), float(res.s[n]), float(res.e[n])
+        if not (t - s < 3.0 / 16.0 and abs(t - nocc) < 0.5 and e_floor <= e < 0.25):
+            continue
+        a = 0.5 * (1.0 - math.sqrt(1.0 - 4.0 * e))
+        x_lumo, x_homo = a, 1.0 - a
+        for j in range(n - 1, -1, -1):
+            if res.branch[j] == "S":
+                x_lumo, x_homo = math.sqrt(x_lumo), math.sqrt(x_homo)
+            else:
+                x_lumo, x_homo = 1.0 - math.sqrt(1.0 - x_lumo), 1.0 - math.sqrt(1.0 - x_homo)
+        lumo = max(lumo, res.emax - w * x_lumo)
+        homo = min(homo, res.emax - w * x_homo)
+    if not (math.isfinite(homo) and math.isfinite(lumo)):
+        raise RuntimeError("no admissible step in the history")
+    return homo, lumo
 
 
 def square_entries(X, pairs):

@@ -34,7 +34,7 @@ EXPORTS = ("rfoe_create", "rfoe_bounds", "rfoe_bounds_lanczos", "rfoe_expand", "
            "rfoe_symm_product", "rfoe_project", "rfoe_apply", "rfoe_expand_sharded", "rfoe_shard_range", "rfoe_plan_squaring",
            "rfoe_shard_local_ptrs", "rfoe_shard_set_peers", "rfoe_shard_ipc_export", "rfoe_shard_ipc_import",
            "rfoe_expand_sharded_p2p",
-           "rfoe_set_option", "rfoe_get_stats", "rfoe_destroy", "rfoe_strerror", "rfoe_version")
+           "rfoe_estimate_homo_lumo", "rfoe_set_option", "rfoe_get_stats", "rfoe_destroy", "rfoe_strerror", "rfoe_version")
 
 
 # int allgather(void* user, const void* send, void* recv, int64_t bytes, stream)  -- see include/rfoe.h
@@ -102,6 +102,7 @@ def load_library(path: str | None = None):
     L.rfoe_shard_range.argtypes = [i64, C.c_int, C.c_int, C.POINTER(i64), C.POINTER(i64)]
     L.rfoe_set_option.argtypes = [vp, C.c_int, dbl]
     L.rfoe_get_stats.argtypes = [vp, C.POINTER(_Stats)]
+    L.rfoe_estimate_homo_lumo.argtypes = [C.POINTER(_Stats), dp, dp]
     L.rfoe_destroy.argtypes = [vp]
     L.rfoe_strerror.argtypes = [C.c_int]
     L.rfoe_strerror.restype = C.c_char_p
@@ -158,6 +159,16 @@ def _check_rect(x, name):
     if not (isinstance(x, torch.Tensor) and x.is_cuda and x.dtype == torch.float64 and x.dim() == 2 and x.stride(1) == 1
             and x.stride(0) >= x.shape[1]):
         raise ValueError(f"{name}: row-major float64 CUDA matrix (k x M, unit column stride) expected")
+
+
+def estimate_homo_lumo(stats: _Stats):
+    """rfoe_estimate_homo_lumo on a raw stats structure (host only, no device needed)."""
+    L = load_library()
+    ho, lu = C.c_double(), C.c_double()
+    rc = L.rfoe_estimate_homo_lumo(C.byref(stats), C.byref(ho), C.byref(lu))
+    if rc != OK:
+        raise RfoeError(rc, "rfoe_estimate_homo_lumo: " + L.rfoe_strerror(rc).decode())
+    return ho.value, lu.value
 
 
 def plan_squaring(k: int, sm_count: int = 148):
@@ -239,6 +250,10 @@ class Rfoe:
         st = _Stats()
         self._L.rfoe_get_stats(self._h, C.byref(st))
         return st
+
+    def estimate_homo_lumo(self):
+        """(homo, lumo) estimates from the history of the last plain SP2 run of this handle (rfoe_estimate_homo_lumo)."""
+        return estimate_homo_lumo(self.stats_raw())
 
     def set_option(self, key: int, value: float):
         rc = self._L.rfoe_set_option(self._h, key, float(value))

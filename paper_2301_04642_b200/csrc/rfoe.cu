@@ -421,6 +421,45 @@ extern "C" int rfoe_get_stats(rfoe_handle_t h, rfoe_stats_t* out)
     return RFOE_OK;
 }
 
+// HOMO / LUMO estimates from the history of an SP2 run (host only; rfoe.h, reading R-HL).
+// u = image of the LUMO bound (small), v = 1 - image of the HOMO bound (small): both are carried back as distances
+// from 0 and from 1, in the cancellation-free forms  1 - sqrt(1 - u) = u / (1 + sqrt(1 - u)).
+extern "C" int rfoe_estimate_homo_lumo(const rfoe_stats_t* S, double* homo, double* lumo)
+{
+    if (!S || !homo || !lumo) return RFOE_ERR_INVALID_ARG;
+    const int steps = S->iterations;
+    const double width = S->eps_max - S->eps_min;
+    if (steps < 1 || steps > RFOE_MAX_STEPS || !(width > 0.0) || !isfinite(width) || S->nocc < 1) return RFOE_ERR_INVALID_ARG;
+    if (S->variant != RFOE_VARIANT_SP2 || S->fp32_steps != 0) return RFOE_ERR_UNSUPPORTED;
+    for (int j = 0; j < steps; ++j)
+        if (S->branch[j] != 'S' && S->branch[j] != 'L') return RFOE_ERR_UNSUPPORTED;
+    constexpr double E_FLOOR = 1e-6;
+    double u_best = INFINITY, v_best = INFINITY;   // smallest LUMO image / smallest (1 - HOMO image) in X_0
+    for (int n = 0; n < steps; ++n) {
+        const double e = S->e[n];
+        const bool settled = (S->t[n] - S->s[n]) < 3.0 / 16.0 && fabs(S->t[n] - (double)S->nocc) < 0.5;
+        if (!settled || !(e >= E_FLOOR) || !(e < 0.25)) continue;
+        const double a = 2.0 * e / (1.0 + sqrt(1.0 - 4.0 * e));   // = (1 - sqrt(1 - 4e)) / 2
+        double u = a, v = a;
+        for (int j = n - 1; j >= 0; --j) {
+            if (S->branch[j] == 'S') {            // x' = x^2:           x = sqrt(x'),  1 - x = (1 - x') / (1 + sqrt(x'))
+                u = sqrt(u);
+                v = v / (1.0 + sqrt(1.0 - v));
+            } else {                              // 1 - x' = (1 - x)^2: 1 - x = sqrt(1 - x'),  x = x' / (1 + sqrt(1 - x'))
+                u = u / (1.0 + sqrt(1.0 - u));
+                v = sqrt(v);
+            }
+        }
+        u_best = fmin(u_best, u);
+        v_best = fmin(v_best, v);
+    }
+    if (!isfinite(u_best) || !isfinite(v_best)) return RFOE_ERR_NOT_CONVERGED;
+    // X_0 = (eps_max I - H) / width:  lambda = eps_max - width x
+    *lumo = S->eps_max - width * u_best;
+    *homo = S->eps_min + width * v_best;          // = eps_max - width (1 - v)
+    return RFOE_OK;
+}
+
 // ---------------------------------------------------------------------------------------------
 // A1: Gershgorin bounds into h->d_bounds (device) -- two launches
 static int run_bounds(rfoe_handle_s* h, const double* Hp, int k, cudaStream_t st)

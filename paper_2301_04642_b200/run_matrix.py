@@ -53,15 +53,20 @@ def main() -> int:
                 ("SP2 rule A, Lanczos bounds (24 steps, on the device)", rfoe.SP2, w.tol, dict(lanczos_steps=24)),
                 ("mixed (late switch 5e-7) + Lanczos bounds", rfoe.SP2_MIXED, w.tol, dict(lanczos_steps=24, mixed_head=0.0, mixed_reltr=5e-7)),
                 ("A-Z-RFOE (accelerated), exact HOMO/LUMO", rfoe.SP2_ACCEL, w.tol, dict(homo=homo, lumo=lumo)),
+                ("A-Z-RFOE, HOMO/LUMO estimated from the normative run's history", rfoe.SP2_ACCEL, w.tol, "estimated"),
                 ("McWeeny-style tail", rfoe.MCWEENY, w.tol, {}),
                 ("mixed, paper schedule (reduced until RelTr 5e-4)", rfoe.SP2_MIXED, w.tol, dict(mixed_head=0.0, mixed_reltr=5e-4))]
         with rfoe.Rfoe(k) as h:
             for name, variant, tol, opts in runs:
                 h.configure(stop_rule=rfoe.RULE_A, bounds=False, mixed_head=0.0, mixed_reltr=5e-4, lanczos_steps=0)
+                if opts == "estimated":                              # rfoe_estimate_homo_lumo on the first row's history
+                    opts = dict(homo=est[0], lumo=est[1])
                 h.configure(**opts)
                 r = None
                 for _ in range(2):                                   # second run is the timed one (warm)
                     r = h.expand(H, nocc, variant, tol)
+                if name.endswith("(normative)"):
+                    est = h.estimate_homo_lumo()
                 P = r.P
                 err = torch.linalg.norm(P - Pex).item() / math.sqrt(k)
                 dE = abs(r.tr_PH - eband) / abs(eband)

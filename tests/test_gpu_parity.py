@@ -212,6 +212,29 @@ def test_expand_accelerated(handle):
     assert res.iterations < plain.iterations
 
 
+@pytest.mark.parametrize("c,k", [(1, 256), (2, 333), (4, 450)])
+def test_homo_lumo_from_sp2_history_feed_accelerated(handle, c, k):
+    """Z-RFOE, then rfoe_estimate_homo_lumo on its history, then A-Z-RFOE with those estimates (reading R-HL): each side
+    uses its own history and its own estimates; estimates, iteration counts and P agree."""
+    w = rfoe_inputs.make_workload(c, k=k)
+    ref0 = oracle.expand(w.H, w.nocc, tol=w.tol)
+    oh, ol = oracle.estimate_homo_lumo(ref0, w.nocc)
+    res0 = handle.expand(_dev(w.H), w.nocc, rfoe.SP2, w.tol)
+    homo, lumo = handle.estimate_homo_lumo()
+    width = res0.eps_max - res0.eps_min
+    assert homo == pytest.approx(oh, abs=1e-8 * width) and lumo == pytest.approx(ol, abs=1e-8 * width)
+    lam_homo, lam_lumo = float(w.lam[: w.nocc].max()), float(w.lam[w.nocc:].min())
+    assert lam_homo - 1e-9 * width <= homo < lumo <= lam_lumo + 1e-9 * width
+    ref = oracle.expand(w.H, w.nocc, variant=oracle.SP2_ACCEL, tol=w.tol, homo=oh, lumo=ol)
+    handle.configure(homo=homo, lumo=lumo)
+    res = handle.expand(_dev(w.H), w.nocc, rfoe.SP2_ACCEL, w.tol)
+    _check_expansion(w, res, ref)
+    assert res.iterations < res0.iterations
+    with pytest.raises(rfoe.RfoeError) as ei:          # the history of the accelerated run itself is not accepted
+        handle.estimate_homo_lumo()
+    assert ei.value.status == rfoe.ERR_UNSUPPORTED
+
+
 def test_expand_host_entry_point(handle):
     w = rfoe_inputs.make_workload(1, k=192)
     ref = oracle.expand(w.H, w.nocc, tol=w.tol)
