@@ -35,6 +35,20 @@ def test_stats_struct_matches_header():
     assert ctypes.sizeof(rfoe._Stats) == expect
 
 
+def test_header_is_plain_c_and_struct_size_matches_the_binding(tmp_path):
+    """include/rfoe.h compiles as strict C99 (no C++, no torch types) inside a C client that links librfoe.so; the
+    compiler's sizeof(rfoe_stats_t) is the binding's."""
+    import subprocess
+
+    from tests import abi_client_build
+
+    exe = abi_client_build.build(tmp_path)
+    out = subprocess.run([exe, "sizeof"], check=True, capture_output=True, text=True).stdout
+    kv = dict(p.split("=") for p in out.split())
+    assert int(kv["sizeof_stats"]) == ctypes.sizeof(rfoe._Stats)
+    assert int(kv["version"]) == 100 and int(kv["max_steps"]) == rfoe.MAX_STEPS
+
+
 def test_argument_errors_without_gpu():
     L = rfoe.load_library()
     h = ctypes.c_void_p()
