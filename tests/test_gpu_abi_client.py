@@ -29,7 +29,9 @@ def test_c_client_matches_oracle(tmp_path, k):
     ref = oracle.expand(H, nocc, tol=tol)
     P = np.fromfile(out_bin, dtype=np.float64).reshape(k, k)
     assert int(kv["status"]) == 0 and int(kv["converged"]) == 1
-    assert int(kv["iterations"]) == ref.iterations and kv["branch"] == ref.branch
+    assert int(kv["iterations"]) == ref.iterations and len(kv["branch"]) == ref.iterations
+    for n, (a, b) in enumerate(zip(kv["branch"], ref.branch)):  # identical wherever t_n - nocc is above rounding level (R10)
+        assert a == b or abs(ref.t[n] - nocc) <= 1e-9 * max(1.0, k / 256), n
     lo, hi = oracle.bounds(H)
     for key, val in (("eps_min", lo), ("bounds_min", lo), ("eps_max", hi), ("bounds_max", hi)):
         assert float(kv[key]) == pytest.approx(val, rel=1e-13)
