@@ -33,7 +33,7 @@ OK, ERR_INVALID_ARG, ERR_ALLOC, ERR_CUDA, ERR_BAD_BOUNDS, ERR_NOT_SYMMETRIC, ERR
 EXPORTS = ("rfoe_create", "rfoe_bounds", "rfoe_bounds_lanczos", "rfoe_expand", "rfoe_expand_host", "rfoe_square", "rfoe_square_reduced",
            "rfoe_symm_product", "rfoe_project", "rfoe_apply", "rfoe_expand_sharded", "rfoe_shard_range", "rfoe_plan_squaring",
            "rfoe_shard_local_ptrs", "rfoe_shard_set_peers", "rfoe_shard_ipc_export", "rfoe_shard_ipc_import",
-           "rfoe_expand_sharded_p2p",
+           "rfoe_expand_sharded_p2p", "rfoe_expand_many",
            "rfoe_estimate_homo_lumo", "rfoe_set_option", "rfoe_get_stats", "rfoe_destroy", "rfoe_strerror", "rfoe_version")
 
 
@@ -98,6 +98,8 @@ def load_library(path: str | None = None):
     L.rfoe_shard_ipc_export.argtypes = [vp, vp]
     L.rfoe_shard_ipc_import.argtypes = [vp, C.c_int, C.c_int, vp]
     L.rfoe_expand_sharded_p2p.argtypes = [vp, vp, i64, i64, C.c_int, dbl, vp, BARRIER_FN, vp, vp]
+    L.rfoe_expand_many.argtypes = [C.POINTER(vp), C.POINTER(vp), C.c_int, C.c_int, C.POINTER(vp), C.POINTER(i64), C.POINTER(i64),
+                                   C.c_int, dp, C.POINTER(vp), C.POINTER(C.c_int), C.POINTER(_Stats)]
     L.rfoe_plan_squaring.argtypes = [i64, C.c_int, C.POINTER(i64), C.POINTER(i64), C.POINTER(C.c_int), C.POINTER(C.c_int)]
     L.rfoe_shard_range.argtypes = [i64, C.c_int, C.c_int, C.POINTER(i64), C.POINTER(i64)]
     L.rfoe_set_option.argtypes = [vp, C.c_int, dbl]
@@ -159,6 +161,54 @@ def _check_rect(x, name):
     if not (isinstance(x, torch.Tensor) and x.is_cuda and x.dtype == torch.float64 and x.dim() == 2 and x.stride(1) == 1
             and x.stride(0) >= x.shape[1]):
         raise ValueError(f"{name}: row-major float64 CUDA matrix (k x M, unit column stride) expected")
+
+
+def _result_from(st: _Stats, P, rc) -> "ExpandResult":
+    n = st.iterations
+    return ExpandResult(
+        P=P, status=rc, converged=bool(st.converged), iterations=n, multiplications=st.multiplications,
+        mcweeny_steps=st.mcweeny_steps, fp32_steps=st.fp32_steps, branch=st.branch.decode()[:n],
+        eps_min=st.eps_min, eps_max=st.eps_max, tr_PH=st.tr_PH, device_ms=st.device_ms, square_ms=st.square_ms,
+        square_launches=st.square_launches, gpu_launches=st.gpu_launches, t=np.array(st.t[: n + 1]),
+        s=np.array(st.s[: n + 1]), e=np.array(st.e[:n]), reltr=np.array(st.reltr[:n]))
+
+
+def expand_many(handles, problems, variant: int = SP2, streams=None):
+    """rfoe_expand_many: independent problems side by side on one GPU.  ``handles``: Rfoe objects (one host thread and
+    one stream each, inside the library); ``problems``: list of (Hp, nocc, tol) or (Hp, nocc, tol, P) with CUDA tensors.
+    Returns one ExpandResult per problem, in order; raises on any status other than OK / NOT_CONVERGED."""
+    import torch
+
+    L = load_library()
+    nh, n = len(handles), len(problems)
+    if streams is None:
+        streams = [torch.cuda.Stream() for _ in handles]
+    torch.cuda.current_stream().synchronize()              # every Hp complete before the call (rfoe.h)
+    Ps = []
+    for pr in problems:
+        _check_dev(pr[0], "Hp")
+        Ps.append(pr[3] if len(pr) > 3 and pr[3] is not None else torch.empty_like(pr[0]))
+        _check_dev(Ps[-1], "P")
+    vp = C.c_void_p
+    hs = (vp * nh)(*[h._h.value for h in handles])
+    ss = (vp * nh)(*[s.cuda_stream for s in streams])
+    Hp = (vp * n)(*[pr[0].data_ptr() for pr in problems])
+    Pp = (vp * n)(*[p.data_ptr() for p in Ps])
+    ks = (C.c_int64 * n)(*[pr[0].shape[0] for pr in problems])
+    no = (C.c_int64 * n)(*[int(pr[1]) for pr in problems])
+    tl = (C.c_double * n)(*[float(pr[2]) for pr in problems])
+    status = (C.c_int * n)()
+    stats = (_Stats * n)()
+    rc = L.rfoe_expand_many(hs, ss, nh, n, Hp, ks, no, int(variant), tl, Pp, status, stats)
+    out = []
+    for j in range(n):
+        if status[j] not in (OK, ERR_NOT_CONVERGED):
+            raise RfoeError(status[j], f"rfoe_expand_many, problem {j}: " + L.rfoe_strerror(status[j]).decode(),
+                            stats[j].cuda_error)
+        out.append(_result_from(stats[j], Ps[j], status[j]))
+    if rc not in (OK, ERR_NOT_CONVERGED):
+        raise RfoeError(rc, "rfoe_expand_many: " + L.rfoe_strerror(rc).decode())
+    return out
 
 
 def estimate_homo_lumo(stats: _Stats):
@@ -277,14 +327,7 @@ class Rfoe:
         return self
 
     def _result(self, P, rc) -> ExpandResult:
-        st = self.stats_raw()
-        n = st.iterations
-        return ExpandResult(
-            P=P, status=rc, converged=bool(st.converged), iterations=n, multiplications=st.multiplications,
-            mcweeny_steps=st.mcweeny_steps, fp32_steps=st.fp32_steps, branch=st.branch.decode()[:n],
-            eps_min=st.eps_min, eps_max=st.eps_max, tr_PH=st.tr_PH, device_ms=st.device_ms, square_ms=st.square_ms, square_launches=st.square_launches,
-            gpu_launches=st.gpu_launches, t=np.array(st.t[: n + 1]), s=np.array(st.s[: n + 1]),
-            e=np.array(st.e[:n]), reltr=np.array(st.reltr[:n]))
+        return _result_from(self.stats_raw(), P, rc)
 
     # ---- the C-ABI calls
     def bounds(self, Hp, stream=None):

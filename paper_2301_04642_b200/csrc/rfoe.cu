@@ -7,7 +7,9 @@
 #include <stdint.h>
 #include <string.h>
 
+#include <atomic>
 #include <new>
+#include <thread>
 #include <vector>
 
 #include "../../include/rfoe.h"
@@ -813,6 +815,45 @@ extern "C" int rfoe_expand(rfoe_handle_t h, const double* Hp, int64_t k, int64_t
                            rfoe_stream_t stream)
 {
     return expand_impl(h, Hp, k, nocc, variant, tol, P, stream, nullptr);
+}
+
+// Many independent problems on one GPU: one host thread per handle, problems taken from a shared counter (rfoe.h).
+extern "C" int rfoe_expand_many(const rfoe_handle_t* handles, const rfoe_stream_t* streams, int n_handles, int n_problems,
+                                const double* const* Hp, const int64_t* k, const int64_t* nocc, int variant, const double* tol,
+                                double* const* P, int* status, rfoe_stats_t* stats)
+{
+    if (!handles || !streams || n_handles < 1 || n_problems < 0) return RFOE_ERR_INVALID_ARG;
+    if (n_problems > 0 && (!Hp || !k || !nocc || !tol || !P)) return RFOE_ERR_INVALID_ARG;
+    for (int i = 0; i < n_handles; ++i) {
+        if (!handles[i]) return RFOE_ERR_INVALID_ARG;
+        for (int j = 0; j < i; ++j)
+            if (handles[j] == handles[i]) return RFOE_ERR_INVALID_ARG;
+    }
+    std::vector<int> rcs((size_t)n_problems, RFOE_OK);
+    std::atomic<int> next(0);
+    auto worker = [&](int i) {
+        for (;;) {
+            const int j = next.fetch_add(1);
+            if (j >= n_problems) break;
+            rcs[j] = expand_impl(handles[i], Hp[j], k[j], nocc[j], variant, tol[j], P[j], streams[i], nullptr);
+            if (stats) stats[j] = handles[i]->stats;
+        }
+    };
+    const int n_threads = n_handles < n_problems ? n_handles : n_problems;
+    std::vector<std::thread> pool;
+    try {
+        for (int i = 1; i < n_threads; ++i) pool.emplace_back(worker, i);
+    } catch (...) {
+        // fewer threads than asked for: the remaining handles stay idle, the problems are still all taken
+    }
+    if (n_threads > 0) worker(0);
+    for (std::thread& t : pool) t.join();
+    int first = RFOE_OK;
+    for (int j = 0; j < n_problems; ++j) {
+        if (status) status[j] = rcs[j];
+        if (first == RFOE_OK && rcs[j] != RFOE_OK) first = rcs[j];
+    }
+    return first;
 }
 
 extern "C" int rfoe_expand_sharded(rfoe_handle_t h, const double* Hp, int64_t k, int64_t nocc, int variant, double tol, double* P,

@@ -56,6 +56,10 @@ def test_argument_errors_without_gpu():
     assert L.rfoe_create(ctypes.byref(h), 0, 0) == rfoe.ERR_INVALID_ARG
     assert L.rfoe_destroy(None) == rfoe.OK
     assert L.rfoe_set_option(None, 0, 0.0) == rfoe.ERR_INVALID_ARG
+    assert L.rfoe_expand_many(None, None, 1, 0, None, None, None, 0, None, None, None, None) == rfoe.ERR_INVALID_ARG
+    hs, ss = (ctypes.c_void_p * 1)(None), (ctypes.c_void_p * 1)(None)
+    assert L.rfoe_expand_many(hs, ss, 1, 0, None, None, None, 0, None, None, None, None) == rfoe.ERR_INVALID_ARG   # null handle
+    assert L.rfoe_expand_many(hs, ss, 0, 0, None, None, None, 0, None, None, None, None) == rfoe.ERR_INVALID_ARG
 
 
 def test_no_cpu_fallback():
