@@ -336,6 +336,8 @@ def run_ours(args) -> int:
         if world == 1 and not shard:
             line["hbm_kernels"] = hbm_report(h, H, stream)
             line["lanczos_bounds"] = lanczos_report(h, rfoe, w, H, P, stream, ms_total / args.steps)
+        if world == 1 and not shard and not args.no_many:
+            line["many_small_problems"] = many_report(rfoe, rfoe_inputs, local)
         if want_reduced:
             line["reduced_precision"] = reduced_report(h, rfoe, w, H, P, stream, ms_total / args.steps)
         if world == 1 and not args.no_subspace and k <= 16384:   # 59 GB of basis + generator temporaries: not beside config 5
@@ -353,6 +355,45 @@ def run_ours(args) -> int:
     if dist.is_initialized():
         dist.destroy_process_group()
     return 0
+
+
+def many_report(rfoe, rfoe_inputs, local):
+    """Reported separately ("throughput over independent H^p (k-points, spins)"): BASELINE configs 1 and 2 are too
+    small to fill the chip one at a time; rfoe_expand_many runs independent copies side by side on one GPU (one handle,
+    stream and host thread each).  Wall-clock rate of a batch after one warm batch, against the lone-handle rate."""
+    import time
+
+    import torch
+
+    out = {}
+    for c, n_handles, n_problems in ((1, 16, 128), (2, 4, 32)):
+        w = rfoe_inputs.make_workload(c)
+        H = torch.from_numpy(w.H).cuda(local)
+        m = (w.k + TILE - 1) // TILE
+        rates = {}
+        for nh in (1, n_handles):
+            handles = [rfoe.Rfoe(w.k, device=local) for _ in range(nh)]
+            streams = [torch.cuda.Stream() for _ in range(nh)]
+            Ps = [torch.empty_like(H) for _ in range(n_problems)]
+            probs = [(H, w.nocc, w.tol, Ps[j]) for j in range(n_problems)]
+            rfoe.expand_many(handles, probs, rfoe.SP2, streams)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            res = rfoe.expand_many(handles, probs, rfoe.SP2, streams)
+            torch.cuda.synchronize()
+            dt = time.perf_counter() - t0
+            rates[nh] = n_problems / dt
+            its = res[0].iterations
+            for hh in handles:
+                hh.close()
+            del Ps, probs, res
+        out[f"config{c}_k{w.k}"] = {
+            "handles": n_handles, "problems": n_problems, "squarings_per_expansion": its,
+            "expansions_per_s": rates[n_handles], "expansions_per_s_one_handle": rates[1],
+            "speedup": rates[n_handles] / rates[1],
+            "tflops_executed": rates[n_handles] * its * executed_flops_per_squaring(w.k) / 1e12,
+            "timing": "host wall clock around one rfoe_expand_many batch (device idle before and after)"}
+    return out
 
 
 def hbm_report(h, H, stream):
@@ -516,6 +557,7 @@ def main() -> int:
     ap.add_argument("--shard", nargs="?", const="p2p", default=None, choices=["p2p", "allgather"],
                     help="N > 1: shard ONE expansion over the ranks (strong scaling) instead of independent replicas; p2p (default): "
                          "epilogue stores to all ranks' memory over NVLink + one barrier per step; allgather: NCCL all-gather per step")
+    ap.add_argument("--no-many", action="store_true", help="skip the separately reported many-small-problems run")
     ap.add_argument("--no-subspace", action="store_true", help="skip the separately reported Rayleigh-Ritz / apply steps")
     ap.add_argument("--only-subspace", action="store_true", help="run only the Rayleigh-Ritz / apply chain (ncu captures)")
     ap.add_argument("--subspace-k", type=int, default=4096)
