@@ -112,6 +112,88 @@ def test_fullsize_config5():
         f.write(repr(r) + "\n")
 
 
+@pytest.mark.slow
+@pytest.mark.parametrize("c", [3] + ([4] if os.environ.get("RFOE_FULL_ORACLE_16384") == "1" else []))
+def test_full_oracle_expansion_every_element(c):
+    """"run the full oracle once for k=8192 and 16384 (budget it)".  The WHOLE naive oracle expansion
+    (2 k^3 per squaring, host cores, minutes to hours) against the GPU expansion on the same bytes: every element of P,
+    the iteration count, the branch string, the band energy and the per-step history, at the north_star tolerances.
+    k=16384 only with RFOE_FULL_ORACLE_16384=1 (about two hours of host time)."""
+    import time
+
+    w = rfoe_inputs.make_workload(c, device="cuda")
+    k, nocc = w.k, w.nocc
+    Hn = w.H.cpu().numpy()
+    with rfoe.Rfoe(k) as h:
+        res = h.expand(w.H, nocc, rfoe.SP2, w.tol)
+    P = res.P.cpu().numpy()
+    del res.P
+    w.H = w.Q = None
+    torch.cuda.empty_cache()
+    t0 = time.perf_counter()
+    ref = oracle.expand(Hn, nocc, tol=w.tol)
+    oracle_s = time.perf_counter() - t0
+    assert ref.converged and res.converged and res.iterations == ref.iterations
+    decided = np.abs(ref.t[: ref.iterations] - nocc) > 1e-9 * k / 256
+    assert all(a == b for a, b, d in zip(res.branch, ref.branch, decided) if d), (res.branch, ref.branch)
+    dP = float(np.linalg.norm(P - ref.P) / math.sqrt(k))
+    dmax = float(np.abs(P - ref.P).max())
+    dE = abs(res.tr_PH - ref.tr_PH) / abs(ref.tr_PH)
+    assert dP <= 1e-10 and dE <= 1e-11, (dP, dE)
+    assert res.eps_min == pytest.approx(ref.emin, rel=1e-13) and res.eps_max == pytest.approx(ref.emax, rel=1e-13)
+    assert np.allclose(res.t, ref.t, rtol=0, atol=1e-8 * k / 256)
+    assert np.allclose(res.s, ref.s, rtol=0, atol=1e-8 * k / 256)
+    live = ref.e > 1e3 * EPS * k                       # above the rounding floor of e_n
+    assert np.allclose(res.e[live], ref.e[live], rtol=1e-6)
+    out = dict(config=c, k=k, iterations=ref.iterations, branch=ref.branch, dP=dP, max_abs_dP=dmax, dE=dE,
+               oracle_seconds=oracle_s, oracle_threads=os.cpu_count(), gpu_ms=res.device_ms,
+               oracle_tflops=ref.iterations * float(k) * k * (k + 1) / oracle_s / 1e12)
+    print(out)
+    os.makedirs("gpurun_out", exist_ok=True)
+    with open(f"gpurun_out/full_oracle_config{c}.txt", "w") as f:
+        f.write(repr(out) + "\n")
+
+
+@pytest.mark.slow
+def test_headline_size_first_steps_every_element():
+    """k=16384 (config 4, the size bench.py times): the whole naive oracle expansion would take hours of host time, so the
+    first m = 5 recursion steps are run on both sides (T-RFOE style: RFOE_OPT_MAX_ITER = m, tol = 0) and
+    EVERY element of X_m is compared, with the scalars of every step; both SP2 branches occur in these steps."""
+    import time
+
+    m = 5
+    w = rfoe_inputs.make_workload(4, device="cuda")
+    k, nocc = w.k, w.nocc
+    Hn = w.H.cpu().numpy()
+    with rfoe.Rfoe(k) as h:
+        h.configure(max_iter=m)
+        res = h.expand(w.H, nocc, rfoe.SP2, 0.0)
+    assert res.status == rfoe.ERR_NOT_CONVERGED and res.iterations == m
+    X = res.P.cpu().numpy()
+    del res.P
+    w.H = w.Q = None
+    torch.cuda.empty_cache()
+    t0 = time.perf_counter()
+    ref = oracle.expand(Hn, nocc, tol=0.0, max_iter=m)
+    oracle_s = time.perf_counter() - t0
+    assert ref.iterations == m and res.branch == ref.branch and len(set(ref.branch)) == 2
+    xmax = float(np.abs(ref.P).max())
+    dmax = float(np.abs(X - ref.P).max())
+    dF = float(np.linalg.norm(X - ref.P) / math.sqrt(k))
+    # m products of k terms each, errors carried through x^2 / 2x - x^2 (derivative <= 2): a generous rounding bound
+    assert dmax <= (2.0 ** m) * 8 * k * EPS * xmax, (dmax, xmax)
+    assert dF <= 1e-10
+    assert np.allclose(res.t, ref.t, rtol=1e-12, atol=0) and np.allclose(res.s, ref.s, rtol=1e-12, atol=0)
+    assert np.allclose(res.e, ref.e, rtol=1e-9, atol=0)
+    assert abs(res.tr_PH - ref.tr_PH) <= 1e-11 * abs(ref.tr_PH)
+    out = dict(k=k, steps=m, branch=ref.branch, max_abs_diff=dmax, frob_diff_per_sqrt_k=dF, oracle_seconds=oracle_s,
+               oracle_seconds_per_squaring=oracle_s / m, oracle_threads=os.cpu_count(), gpu_ms=res.device_ms)
+    print(out)
+    os.makedirs("gpurun_out", exist_ok=True)
+    with open("gpurun_out/first_steps_k16384.txt", "w") as f:
+        f.write(repr(out) + "\n")
+
+
 def _run_fullsize_mixed(c):
     """Reduced-precision path (A8) at full size with the paper's schedule (FP32 steps from the start until
     RelTr <= 5e-4).  The oracle's FP32 loop cannot run here; properties that hold at any
