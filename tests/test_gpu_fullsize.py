@@ -113,8 +113,9 @@ def test_fullsize_config5():
 
 
 @pytest.mark.slow
+@pytest.mark.parametrize("variant", ["sp2", "accel"])
 @pytest.mark.parametrize("c", [3] + ([4] if os.environ.get("RFOE_FULL_ORACLE_16384") == "1" else []))
-def test_full_oracle_expansion_every_element(c):
+def test_full_oracle_expansion_every_element(c, variant):
     """"run the full oracle once for k=8192 and 16384 (budget it)".  The WHOLE naive oracle expansion
     (2 k^3 per squaring, host cores, minutes to hours) against the GPU expansion on the same bytes: every element of P,
     the iteration count, the branch string, the band energy and the per-step history, at the north_star tolerances.
@@ -124,14 +125,21 @@ def test_full_oracle_expansion_every_element(c):
     w = rfoe_inputs.make_workload(c, device="cuda")
     k, nocc = w.k, w.nocc
     Hn = w.H.cpu().numpy()
+    accel = variant == "accel"          # A-Z-RFOE with the generator's HOMO / LUMO: about half the squarings
+    homo, lumo = float(w.lam[:nocc].max()), float(w.lam[nocc:].min())
     with rfoe.Rfoe(k) as h:
-        res = h.expand(w.H, nocc, rfoe.SP2, w.tol)
+        if accel:
+            h.configure(homo=homo, lumo=lumo)
+        res = h.expand(w.H, nocc, rfoe.SP2_ACCEL if accel else rfoe.SP2, w.tol)
     P = res.P.cpu().numpy()
     del res.P
     w.H = w.Q = None
     torch.cuda.empty_cache()
     t0 = time.perf_counter()
-    ref = oracle.expand(Hn, nocc, tol=w.tol)
+    if accel:
+        ref = oracle.expand(Hn, nocc, variant=oracle.SP2_ACCEL, tol=w.tol, homo=homo, lumo=lumo)
+    else:
+        ref = oracle.expand(Hn, nocc, tol=w.tol)
     oracle_s = time.perf_counter() - t0
     assert ref.converged and res.converged and res.iterations == ref.iterations
     decided = np.abs(ref.t[: ref.iterations] - nocc) > 1e-9 * k / 256
@@ -145,12 +153,12 @@ def test_full_oracle_expansion_every_element(c):
     assert np.allclose(res.s, ref.s, rtol=0, atol=1e-8 * k / 256)
     live = ref.e > 1e3 * EPS * k                       # above the rounding floor of e_n
     assert np.allclose(res.e[live], ref.e[live], rtol=1e-6)
-    out = dict(config=c, k=k, iterations=ref.iterations, branch=ref.branch, dP=dP, max_abs_dP=dmax, dE=dE,
+    out = dict(config=c, variant=variant, k=k, iterations=ref.iterations, branch=ref.branch, dP=dP, max_abs_dP=dmax, dE=dE,
                oracle_seconds=oracle_s, oracle_threads=os.cpu_count(), gpu_ms=res.device_ms,
                oracle_tflops=ref.iterations * float(k) * k * (k + 1) / oracle_s / 1e12)
     print(out)
     os.makedirs("gpurun_out", exist_ok=True)
-    with open(f"gpurun_out/full_oracle_config{c}.txt", "w") as f:
+    with open(f"gpurun_out/full_oracle_config{c}_{variant}.txt", "w") as f:
         f.write(repr(out) + "\n")
 
 

@@ -250,6 +250,23 @@ def test_expand_config2_full(handle):
     _check_expansion(w, res, ref)
 
 
+def test_expand_config2_full_mcweeny_and_accelerated(handle):
+    """BASELINE config 2 at its full size (k=2048, nocc=1536) in the other two FP64 variants it names / the paper's best
+    performer: McWeeny-style tail (reading R11) and A-Z-RFOE against the whole oracle run."""
+    w = rfoe_inputs.make_workload(2)
+    H = _dev(w.H)
+    ref = oracle.expand(w.H, w.nocc, variant=oracle.MCWEENY, tol=w.tol)
+    res = handle.expand(H, w.nocc, rfoe.MCWEENY, w.tol)
+    assert res.mcweeny_steps == ref.mcweeny_steps >= 1 and res.multiplications == ref.multiplications
+    _check_expansion(w, res, ref)
+    homo, lumo = float(w.lam[: w.nocc].max()), float(w.lam[w.nocc:].min())
+    ref = oracle.expand(w.H, w.nocc, variant=oracle.SP2_ACCEL, tol=w.tol, homo=homo, lumo=lumo)
+    handle.configure(homo=homo, lumo=lumo)
+    res = handle.expand(H, w.nocc, rfoe.SP2_ACCEL, w.tol)
+    assert res.iterations <= 24
+    _check_expansion(w, res, ref)
+
+
 # ------------------------------------------------------------------ errors and degenerate inputs
 def test_error_paths(handle):
     w = rfoe_inputs.make_workload(1, k=64)
