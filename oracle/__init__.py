@@ -6,8 +6,10 @@ see that file's header for the passages of PAPER.md it follows and for its pins)
 legs may import this package; it imports nothing from ``paper_2301_04642_b200``.
 
 Parity status: every function is pinned by tests/test_oracle_pins.py (estimate_homo_lumo: by
-tests/test_oracle_homo_lumo_pins.py) except the exact bit patterns of the iterates X_n ("parity unpinned" for
-bits -- the paper prints no worked example).
+tests/test_oracle_homo_lumo_pins.py; project / apply / density: tests/test_oracle_subspace_pins.py; bounds_lanczos:
+tests/test_oracle_lanczos_pins.py), including the FP32 product (bit for bit against a numpy.float32 loop), the
+mixed schedule's phase switches, the sign rule outside [0,1] and T-RFOE against the exact Fermi-Dirac matrix.
+"Parity unpinned": only the exact bit patterns of the iterates X_n (the paper prints no worked example).
 """
 from __future__ import annotations
 
@@ -22,7 +24,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "rfoe_oracle.c")
 _LIB = os.path.join(_HERE, "librfoe_oracle.so")
 
-SP2, MCWEENY, SP2_MIXED, SP2_ACCEL = 0, 1, 2, 3
+SP2, MCWEENY, SP2_MIXED, SP2_ACCEL, TRUNC, TRUNC_MIXED = 0, 1, 2, 3, 4, 5
 RULE_A, RULE_B = 0, 1
 MAX_STEPS = 256
 
@@ -80,6 +82,8 @@ def lib():
             f.restype = None
         L.rfoe_oracle_bounds_lanczos.argtypes = [dp, C.c_int64, C.c_int32, dp, dp, dp, dp]
         L.rfoe_oracle_bounds_lanczos.restype = C.c_int
+        L.rfoe_oracle_square_f32.argtypes = [dp, C.c_int64, dp, C.POINTER(C.c_float), C.POINTER(C.c_float)]
+        L.rfoe_oracle_square_f32.restype = None
         L.rfoe_oracle_is_symmetric.argtypes = [dp, C.c_int64]
         L.rfoe_oracle_is_symmetric.restype = C.c_int
         L.rfoe_oracle_expand.argtypes = [dp, C.c_int64, C.c_int64, C.POINTER(_Run), dp]
@@ -142,6 +146,18 @@ def matmul(A, B, literal: bool = False) -> np.ndarray:
     return Y
 
 
+def square_f32(X) -> np.ndarray:
+    """The FP32 step's product: X rounded to binary32, binary32 products and sums, l ascending."""
+    X = _sq(X)
+    k = X.shape[0]
+    Y = np.empty_like(X)
+    xf = np.empty(k * k, dtype=np.float32)
+    yf = np.empty(k * k, dtype=np.float32)
+    fp = C.POINTER(C.c_float)
+    lib().rfoe_oracle_square_f32(_p(X), k, _p(Y), xf.ctypes.data_as(fp), yf.ctypes.data_as(fp))
+    return Y
+
+
 def is_symmetric(X) -> bool:
     X = _sq(X)
     return bool(lib().rfoe_oracle_is_symmetric(_p(X), X.shape[0]))
@@ -168,7 +184,9 @@ class OracleResult:
 def expand(H, nocc: int, *, variant: int = SP2, tol: float = 1e-12, stop_rule: int = RULE_A, max_iter: int = 100,
            bounds_override=None, mixed_head: float = 0.0, mixed_reltr: float = 5e-4,
            homo: float = 0.0, lumo: float = 0.0) -> OracleResult:
-    """The whole expansion (O1-O5): Gershgorin -> affine map -> trace-steered recursion -> P."""
+    """The whole expansion (O1-O5): Gershgorin -> affine map -> trace-steered recursion -> P.
+    variant TRUNC / TRUNC_MIXED (T-RFOE, PAPER.md:47-52): exactly ``max_iter`` = m steps, no convergence test;
+    ``converged`` then means "G_m delivered"."""
     H = _sq(H)
     k = H.shape[0]
     run = _Run()

@@ -14,8 +14,10 @@
  *   - RelTr = trace change relative to the previous iterate PAPER.md:64, 92 (sec. III.A, IV)
  *   - mixed precision: FP32 steps far from convergence,
  *     FP64 afterwards, switch tied to RelTr
- *   - truncated expansion G_m (T-RFOE): stop after m steps  PAPER.md:47-52 (sec. II.B.3, Eq. 2)
- *   - accelerated (shifted/scaled) SP2 from HOMO/LUMO       PAPER.md:43    (sec. II.B.2)
+ *   - truncated expansion G_m (T-RFOE): exactly m steps, no
+ *     convergence test (variants ORC_TRUNC, ORC_TRUNC_MIXED) PAPER.md:47-52 (sec. II.B.3, Eq. 2)
+ *   - accelerated (shifted/scaled) SP2 from HOMO/LUMO, in
+ *     the unexpanded form "shift and scale, then SP2"       PAPER.md:43    (sec. II.B.2)
  *   - D = theta(mu I - H): a projector, eigenvalues 0/1     PAPER.md:27    (sec. II.A)
  * Where the paper is silent the readings R1..R16 of DESIGN.md are taken (initial affine map with
  * Gershgorin bounds, tie rule, stop rules A and B, the McWeeny-style switch).
@@ -30,7 +32,9 @@
  * Pins (tests/test_oracle_pins.py, -m "not gpu"): Jacobi-eigendecomposition projector on tiny
  * inputs; construction-exact projector Q_occ Q_occ^T; diagonal-H closed form (scalar recursion);
  * per-step invariants; scalar eigenvalue-space model for branch strings and iteration counts;
- * the paper's printed iteration counts on the paper's matrix.
+ * the paper's printed iteration counts on the paper's matrix; the FP32 product
+ * bit-for-bit against a numpy.float32 loop; the mixed schedule's phase switches and the out-of-range behaviour of
+ * the sign rule on diagonal matrices worked by hand; T-RFOE against the exact Fermi-Dirac matrix.
  * Rayleigh-Ritz / apply / density (NEXT-4): pinned by an invariant-subspace construction against an
  * explicit eigendecomposition (numpy eigh and the Jacobi projector), sum rho = N_occ, and closed forms.
  * Not pinned: the exact bit patterns of X_n (the paper prints no worked example) -- "parity
@@ -43,7 +47,7 @@
 
 #define ORACLE_MAX_STEPS 256
 
-enum { ORC_SP2 = 0, ORC_MCWEENY = 1, ORC_SP2_MIXED = 2, ORC_SP2_ACCEL = 3 };
+enum { ORC_SP2 = 0, ORC_MCWEENY = 1, ORC_SP2_MIXED = 2, ORC_SP2_ACCEL = 3, ORC_TRUNC = 4, ORC_TRUNC_MIXED = 5 };
 enum { ORC_RULE_A = 0, ORC_RULE_B = 1 };
 
 typedef struct {
@@ -326,8 +330,11 @@ void rfoe_oracle_density(const double* Psi, const double* Y, int64_t k, int64_t 
         for (int64_t m = 0; m < M; ++m) rho[m] = rho[m] + Psi[i * ld + m] * Y[i * ld + m];
 }
 
-/* FP32 step of the mixed variant: X rounded to float, float products, float accumulation */
-static void square_f32(const double* X, int64_t k, double* Y, float* xf, float* yf)
+/* ---- FP32 step of the mixed variants ("far away from RFOE convergence ... the floating point
+ * operations can be performed in single precision (FP32)"): X rounded to float, every product and every sum a
+ * separate IEEE binary32 operation, l ascending.  Pinned bit-for-bit against a numpy.float32 triple loop
+ * (tests/test_oracle_pins.py::test_square_f32_bits).  xf, yf: caller-provided k*k float scratch. */
+void rfoe_oracle_square_f32(const double* X, int64_t k, double* Y, float* xf, float* yf)
 {
     for (int64_t i = 0; i < k * k; ++i) xf[i] = (float)X[i];
 #pragma omp parallel for schedule(dynamic, 4)
@@ -355,27 +362,70 @@ int rfoe_oracle_is_symmetric(const double* X, int64_t k)
     return 1;
 }
 
+/* ---- the sign of PAPER.md:39 ----------------------------------------------------------------------------
+ * "The +/- sign is chosen to adjust the trace of X_{n+1} in each projection such that it converges to N_occ":
+ * of the two candidate next iterates, take the one whose trace lands nearer N_occ; a tie takes the "+" sign
+ * (2X - X^2; readings R4, R5).  For a spectrum inside [0,1] this is "X^2 iff Tr X_n > N_occ" (pinned by
+ * test_step_invariants); when rounding has pushed an eigenvalue outside [0,1] it is the branch that maps it back
+ * (pinned by test_sign_rule_repairs_out_of_range_eigenvalue).  Returns 1 for the squaring-type candidate. */
+static int nearer_nocc(double trace_if_squared, double trace_if_other, double nocc)
+{
+    return fabs(trace_if_squared - nocc) < fabs(trace_if_other - nocc);
+}
+
+/* A-Z-RFOE: "shifting and scaling of the SP2 projection polynomials ... based on HOMO ... and LUMO
+ * ... eigenvalues".  Reading R-ACC, written UNEXPANDED, i.e. as the paper's words say -- first shift
+ * and scale, then apply the SP2 polynomial:
+ *     squaring type:   Y = (1 - a) I + a X,  X' = Y^2,          a = 2 / (2 - lumo_img)
+ *     other type:      Y = a X,              X' = 2 Y - Y^2,    a = 2 / (1 + homo_img)
+ * lumo_img / homo_img are the images of the LUMO / HOMO eigenvalue under all maps applied so far. */
+static void shift_scale(const double* X, int64_t k, double a, double shift, double* Y)
+{
+    for (int64_t i = 0; i < k; ++i)
+        for (int64_t j = 0; j < k; ++j) {
+            double v = a * X[i * k + j];
+            Y[i * k + j] = (i == j) ? shift + v : v;
+        }
+}
+static double poly_squaring(double x, double a) { double y = (1.0 - a) + a * x; return y * y; }
+static double poly_other(double x, double a) { double y = a * x; return 2.0 * y - y * y; }
+
 /* ---- O4/O5: the expansion ---------------------------------------------------------------- */
-/* returns 0 on success (converged or max_iter reached; see run->converged), <0 on bad arguments */
+/* returns 0 on success (converged, truncated as asked, or max_iter reached; see run->converged),
+ * -1 bad arguments, -2 H not bitwise symmetric, -3 empty bounds, -4 out of memory,
+ * -5 accelerated variant: HOMO / LUMO estimates not inside the spectral bounds (emin <= homo < lumo <= emax) */
 int rfoe_oracle_expand(const double* H, int64_t k, int64_t nocc, oracle_run_t* run, double* P)
 {
     if (!H || !P || !run || k < 1 || nocc < 0 || nocc > k) return -1;
     if (run->max_iter < 0 || run->max_iter > ORACLE_MAX_STEPS) return -1;
+    if (run->variant < ORC_SP2 || run->variant > ORC_TRUNC_MIXED) return -1;
     if (!rfoe_oracle_is_symmetric(H, k)) return -2;
+
+    const int accel = (run->variant == ORC_SP2_ACCEL);
+    const int mixed = (run->variant == ORC_SP2_MIXED || run->variant == ORC_TRUNC_MIXED);
+    /* T-RFOE (Eq. 2): G_m = F_m(...F_0(H)...), "an intermediate function generated in Z-RFOE that
+     * is obtained before the convergence": exactly max_iter = m steps, no convergence test */
+    const int truncated = (run->variant == ORC_TRUNC || run->variant == ORC_TRUNC_MIXED);
 
     double emin, emax;
     if (run->use_bounds) { emin = run->emin; emax = run->emax; }
     else rfoe_oracle_bounds(H, k, &emin, &emax);
     run->emin = emin; run->emax = emax;
     if (!(emax > emin)) return -3;
+    if (accel && !(emin <= run->homo && run->homo < run->lumo && run->lumo <= emax)) return -5;
 
     const size_t n2 = (size_t)k * (size_t)k;
+    int rc = 0;
     double* X = (double*)malloc(n2 * sizeof(double));
     double* Y = (double*)malloc(n2 * sizeof(double));
-    double* Z = (run->variant == ORC_MCWEENY) ? (double*)malloc(n2 * sizeof(double)) : NULL;
-    float *xf = NULL, *yf = NULL;
-    if (run->variant == ORC_SP2_MIXED) { xf = (float*)malloc(n2 * sizeof(float)); yf = (float*)malloc(n2 * sizeof(float)); }
-    if (!X || !Y) return -4;
+    double* Z = (run->variant == ORC_MCWEENY || accel) ? (double*)malloc(n2 * sizeof(double)) : NULL;
+    double* W = accel ? (double*)malloc(n2 * sizeof(double)) : NULL;
+    float* xf = mixed ? (float*)malloc(n2 * sizeof(float)) : NULL;
+    float* yf = mixed ? (float*)malloc(n2 * sizeof(float)) : NULL;
+    if (!X || !Y || ((run->variant == ORC_MCWEENY || accel) && !Z) || (accel && !W) || (mixed && (!xf || !yf))) {
+        rc = -4;
+        goto cleanup;
+    }
 
     rfoe_oracle_affine(H, k, emin, emax, X);
     double t = rfoe_oracle_trace(X, k), s = rfoe_oracle_sumsq(X, k);
@@ -384,39 +434,28 @@ int rfoe_oracle_expand(const double* H, int64_t k, int64_t nocc, oracle_run_t* r
     run->converged = 0;
     memset(run->branch, 0, sizeof(run->branch));
 
-    /* accelerated SP2 (reading R-ACC): images of LUMO (beta, near 0) and HOMO (bbar,
-     * near 1) under the same maps steer a shift-and-scale of each SP2 polynomial. */
-    double beta = 0.0, bbar = 1.0;
-    if (run->variant == ORC_SP2_ACCEL) {
-        beta = (emax - run->lumo) / (emax - emin);
-        bbar = (emax - run->homo) / (emax - emin);
+    double lumo_img = 0.0, homo_img = 1.0;     /* X0 = (emax I - H) / (emax - emin): occupied -> near 1 */
+    if (accel) {
+        lumo_img = (emax - run->lumo) / (emax - emin);
+        homo_img = (emax - run->homo) / (emax - emin);
     }
     int mcweeny_phase = 0;
-    int mixed_phase = (run->variant == ORC_SP2_MIXED) ? (run->mixed_head > 0.0 ? 0 : 1) : 2;  /* 0 FP64 head, 1 FP32, 2 FP64 */
+    int mixed_phase = mixed ? (run->mixed_head > 0.0 ? 0 : 1) : 2;  /* 0 FP64 head, 1 FP32, 2 FP64 */
     double reltr_prev = INFINITY;
 
     for (int n = 0; n < run->max_iter; ++n) {
-        /* "The +/- sign is chosen to adjust the trace of X_{n+1} ... such that it converges to N_occ"
-         * (PAPER.md:39): take the branch whose RESULTING trace is nearer N_occ; tie -> L (R4, R5).
-         * Tr X^2 = s and Tr(2X - X^2) = 2t - s are known before the product.  For a spectrum
-         * inside [0,1] (t - s >= 0) this is exactly "S iff t > N_occ"; it differs only when rounding noise has
-         * pushed eigenvalues outside [0,1], where it picks the branch that maps them back. */
-        double trS = s, trL = 2.0 * t - s;
-        if (run->variant == ORC_SP2_ACCEL) {
-            const double aS = 2.0 / (2.0 - beta), aL = 2.0 / (1.0 + bbar);
-            trS = aS * aS * s + 2.0 * aS * (1.0 - aS) * t + (1.0 - aS) * (1.0 - aS) * (double)k;
-            trL = 2.0 * aL * t - aL * aL * s;
-        }
-        const int sq = (fabs(trS - (double)nocc) < fabs(trL - (double)nocc));
+        /* mixed schedule: FP32 steps "far away from RFOE convergence", "the number of initial FP32
+         * iterations is linked to RelTr"; optional FP64 head while Tr X - Tr X^2 is still large (reading R-MIX) */
         if (mixed_phase == 0 && (t - s) < run->mixed_head) mixed_phase = 1;
-        if (mixed_phase == 1 && reltr_prev <= run->mixed_reltr) mixed_phase = 2;   /* PAPER.md:66, 92 */
+        if (mixed_phase == 1 && reltr_prev <= run->mixed_reltr) mixed_phase = 2;
         const int fp32 = (mixed_phase == 1);
         if (run->variant == ORC_MCWEENY && !mcweeny_phase)
             if ((t - s) < 3.0 / 16.0 && fabs(t - (double)nocc) < 0.5) mcweeny_phase = 1;   /* R11 */
 
-        if (fp32) square_f32(X, k, Y, xf, yf); else rfoe_oracle_square(X, k, Y);
+        /* Y = X_n^2 (every variant: e_n = ||X_n^2 - X_n||_F is measured on the step's input) */
+        if (fp32) rfoe_oracle_square_f32(X, k, Y, xf, yf); else rfoe_oracle_square(X, k, Y);
         run->multiplications++;
-        double e = sqrt(sumsq_diff(Y, X, k));
+        const double e = sqrt(sumsq_diff(Y, X, k));
 
         if (mcweeny_phase) {
             /* X' = 3 X^2 - 2 X^3, X^3 = (X^2) X as a second naive product */
@@ -431,28 +470,28 @@ int rfoe_oracle_expand(const double* H, int64_t k, int64_t nocc, oracle_run_t* r
                 }
             run->branch[n] = 'M';
             run->mcweeny_steps++;
-        } else if (run->variant == ORC_SP2_ACCEL) {
-            /* S-type: X' = ((1-a) I + a X)^2 = a^2 X^2 + 2a(1-a) X + (1-a)^2 I,  a = 2/(2-beta)
-             * L-type: X' = 2 a X - a^2 X^2,                                      a = 2/(1+bbar) */
-            if (sq) {
-                const double a = 2.0 / (2.0 - beta);
-                const double c2 = a * a, c1 = 2.0 * a * (1.0 - a), c0 = (1.0 - a) * (1.0 - a);
-                for (int64_t i = 0; i < k; ++i)
-                    for (int64_t j = 0; j < k; ++j) {
-                        double v = c2 * Y[i * k + j] + c1 * X[i * k + j];
-                        X[i * k + j] = (i == j) ? v + c0 : v;
-                    }
-                double u = (1.0 - a) + a * beta; beta = u * u;
-                u = (1.0 - a) + a * bbar; bbar = u * u;
+        } else if (accel) {
+            /* both shifted-and-scaled candidates are formed (O(k^2)); their resulting traces follow from
+             * Tr(A^2) = ||A||_F^2 for symmetric A; the chosen one is squared by the naive product.
+             * (The product X_n^2 above only serves e_n here: the method needs one product per step and one is counted.) */
+            const double aS = 2.0 / (2.0 - lumo_img), aO = 2.0 / (1.0 + homo_img);
+            shift_scale(X, k, aS, 1.0 - aS, Z);                       /* Z = (1 - aS) I + aS X */
+            shift_scale(X, k, aO, 0.0, W);                            /* W = aO X              */
+            const double trace_if_squared = rfoe_oracle_sumsq(Z, k);                             /* Tr Z^2       */
+            const double trace_if_other = 2.0 * rfoe_oracle_trace(W, k) - rfoe_oracle_sumsq(W, k); /* Tr(2W - W^2) */
+            if (nearer_nocc(trace_if_squared, trace_if_other, (double)nocc)) {
+                rfoe_oracle_square(Z, k, X);
+                lumo_img = poly_squaring(lumo_img, aS);
+                homo_img = poly_squaring(homo_img, aS);
+                run->branch[n] = 'S';
             } else {
-                const double a = 2.0 / (1.0 + bbar);
-                const double c2 = -(a * a), c1 = 2.0 * a;
-                for (size_t q = 0; q < n2; ++q) X[q] = c2 * Y[q] + c1 * X[q];
-                beta = 2.0 * a * beta - a * a * beta * beta;
-                bbar = 2.0 * a * bbar - a * a * bbar * bbar;
+                rfoe_oracle_square(W, k, Y);
+                for (size_t q = 0; q < n2; ++q) X[q] = 2.0 * W[q] - Y[q];
+                lumo_img = poly_other(lumo_img, aO);
+                homo_img = poly_other(homo_img, aO);
+                run->branch[n] = 'L';
             }
-            run->branch[n] = sq ? 'S' : 'L';
-        } else if (sq) {
+        } else if (nearer_nocc(s, 2.0 * t - s, (double)nocc)) {       /* Tr X^2 = s, Tr(2X - X^2) = 2t - s */
             memcpy(X, Y, n2 * sizeof(double));
             run->branch[n] = fp32 ? 's' : 'S';
         } else {
@@ -468,21 +507,25 @@ int rfoe_oracle_expand(const double* H, int64_t k, int64_t nocc, oracle_run_t* r
         t = t1; s = s1; reltr_prev = reltr;
         run->iterations = n + 1;
         /* mixed: an FP32 step never terminates the expansion (its e, RelTr sit on the FP32 floor) */
-        if (!fp32) {
+        if (!fp32 && !truncated) {
             if (run->stop_rule == ORC_RULE_A ? (e <= run->tol) : (reltr <= run->tol)) { run->converged = 1; break; }
         }
     }
+    if (truncated) run->converged = (run->iterations == run->max_iter);   /* G_m delivered as asked */
 
     memcpy(P, X, n2 * sizeof(double));
-    double acc = 0.0;
-    for (int64_t i = 0; i < k; ++i) {
-        double r = 0.0;
-        for (int64_t j = 0; j < k; ++j) r = r + P[i * k + j] * H[i * k + j];
-        acc = acc + r;
+    {
+        double acc = 0.0;
+        for (int64_t i = 0; i < k; ++i) {
+            double r = 0.0;
+            for (int64_t j = 0; j < k; ++j) r = r + P[i * k + j] * H[i * k + j];
+            acc = acc + r;
+        }
+        run->tr_PH = acc;
     }
-    run->tr_PH = acc;
-    free(X); free(Y); free(Z); free(xf); free(yf);
-    return 0;
+cleanup:
+    free(X); free(Y); free(Z); free(W); free(xf); free(yf);
+    return rc;
 }
 
 int rfoe_oracle_sizeof_run(void) { return (int)sizeof(oracle_run_t); }

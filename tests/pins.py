@@ -108,4 +108,21 @@ def scalar_sp2_accel(lam, nocc: int, emin: float, emax: float, homo: float, lumo
 
 
 def fermi_dirac(lam, mu: float, beta: float):
-    return 1.0 / (np.exp(beta * (np.asarray(lam) - mu)) + 1.0)
+    """Occupancies of the finite-temperature density matrix D = [exp(beta (H - mu I)) + I]^-1,
+    in the overflow-free form (1 - tanh(z/2)) / 2."""
+    return 0.5 * (1.0 - np.tanh(0.5 * beta * (np.asarray(lam, dtype=np.float64) - mu)))
+
+
+def fit_fermi_dirac(lam, occ, mu0: float):
+    """Least-squares (mu, beta) of the Fermi-Dirac function to occupancies ``occ`` at eigenvalues ``lam``
+    (scipy.optimize.least_squares on (mu, log beta) from several starting betas).  Returns (mu, beta)."""
+    from scipy.optimize import least_squares
+
+    lam = np.asarray(lam, dtype=np.float64)
+    best = None
+    for b0 in (10.0, 1e2, 1e3, 1e4, 1e5):
+        r = least_squares(lambda p: fermi_dirac(lam, p[0], math.exp(p[1])) - occ, [mu0, math.log(b0)],
+                          xtol=1e-15, ftol=1e-15, gtol=1e-15)
+        if best is None or r.cost < best.cost:
+            best = r
+    return float(best.x[0]), float(math.exp(best.x[1]))

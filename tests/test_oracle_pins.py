@@ -275,3 +275,186 @@ def test_bad_arguments():
         oracle.expand(np.array([[1.0, 2.0], [3.0, 4.0]]), 1)          # not symmetric
     with pytest.raises(RuntimeError):
         oracle.expand(np.eye(3), 1)                                   # emax == emin
+
+
+# ---------------------------------------------------------------- the FP32 product, bit for bit
+def test_square_f32_bits():
+    """The mixed variants' FP32 step: X rounded to binary32, every product and sum a binary32
+    operation, l ascending -- against a literal numpy.float32 triple loop, bit for bit.  A double-accumulating
+    (or FMA-contracting) version must fail: the test first checks that such versions differ on these inputs."""
+    rng = np.random.default_rng(123)
+    for k in (1, 2, 5, 8):
+        X = rng.standard_normal((k, k))
+        X = X + X.T
+        xf = X.astype(np.float32)
+        ref = np.zeros((k, k), dtype=np.float32)
+        dbl = np.zeros((k, k))
+        for i in range(k):
+            for j in range(k):
+                acc = np.float32(0.0)
+                accd = 0.0
+                for l in range(k):
+                    acc = np.float32(acc + np.float32(xf[i, l] * xf[l, j]))
+                    accd = accd + float(xf[i, l]) * float(xf[l, j])
+                ref[i, j] = acc
+                dbl[i, j] = accd
+        Y = oracle.square_f32(X)
+        assert np.array_equal(Y, ref.astype(np.float64))
+        assert oracle.is_symmetric(Y)
+        if k >= 5:
+            assert not np.array_equal(ref.astype(np.float64), dbl.astype(np.float32).astype(np.float64))
+            assert not np.array_equal(Y, oracle.square(X))
+
+
+# ---------------------------------------------------------------- mixed schedule: where the phases switch
+def test_mixed_phase_switch_on_diagonal():
+    """FP32 steps until RelTr <= mixed_reltr, FP64 afterwards; optional FP64 head while
+    Tr X - Tr X^2 >= mixed_head (reading R-MIX).  On a diagonal H the matrix run is the scalar recursion, so the
+    positions of the lower-case (FP32) steps follow from the plain FP64 scalar model's history (pins.scalar_sp2,
+    which knows nothing about phases): the FP32 phase starts at the first step n with t_n - s_n < head and the
+    last FP32 step is the first one whose RelTr <= switch.  Thresholds sit far from any t_n - s_n / RelTr value."""
+    rng = np.random.default_rng(31)
+    k, nocc = 40, 17
+    lam = np.sort(np.concatenate([rng.uniform(-1.0, -0.1, nocc), rng.uniform(0.1, 1.5, k - nocc)]))
+    H = np.diag(lam)
+    lo, hi = -4.0, 5.0
+    m = pins.scalar_sp2(lam, nocc, lo, hi, tol=1e-12)
+    gap = m["t"][:-1] - m["s"][:-1]                       # t_n - s_n, the quantity the head watches
+    reltr = np.abs(np.diff(m["t"])) / np.abs(m["t"][:-1])
+    n_steps = m["iterations"]
+    for head, switch in [(0.0, 5e-4), (1.8, 5e-4), (0.5, 1e-6), (0.0, 0.0)]:
+        # thresholds must not sit within 5 % of any history value, else FP32 noise could move the switch
+        assert head == 0.0 or all(abs(g - head) > 0.05 * head for g in gap)
+        assert switch == 0.0 or all(abs(r - switch) > 0.05 * switch for r in reltr)
+        first = 0 if head == 0.0 else int(np.argmax(gap < head))
+        if switch == 0.0:
+            expected = None                              # leaves FP32 only once the trace stops moving at all
+        else:
+            last = next(n for n in range(first, n_steps) if reltr[n] <= switch)
+            expected = "".join(ch.lower() if first <= n <= last else ch for n, ch in enumerate(m["branch"]))
+        r = oracle.expand(H, nocc, variant=oracle.SP2_MIXED, tol=1e-12, bounds_override=(lo, hi),
+                          mixed_head=head, mixed_reltr=switch, max_iter=60)
+        if expected is None:
+            nf = r.fp32_steps
+            assert r.branch[:nf].islower() and r.branch[nf:].isupper() and nf >= n_steps - 4
+            assert r.reltr[nf - 1] == 0.0 and np.all(r.reltr[: nf - 1] > 0.0)
+            continue
+        assert r.converged and r.branch == expected, (head, switch, r.branch, expected)
+        assert r.fp32_steps == last - first + 1
+        # FP32 steps leave FP32-level, not FP64-level, agreement with the FP64 model; FP64 steps then repair it
+        assert np.allclose(np.diag(r.P), (lam < 0).astype(float), atol=1e-12)
+    # the FP32 steps really are FP32: after one FP32 step every diagonal entry is a binary32 number
+    r1 = oracle.expand(H, nocc, variant=oracle.TRUNC_MIXED, max_iter=1, bounds_override=(lo, hi), mixed_reltr=0.0)
+    d = np.diag(r1.P)
+    x0 = ((hi - lam) / (hi - lo)).astype(np.float32)
+    sq = (x0 * x0).astype(np.float64)
+    want = sq if r1.branch == "s" else 2.0 * ((hi - lam) / (hi - lo)) - sq
+    assert r1.branch in ("s", "l") and np.array_equal(d, want)
+
+
+# ---------------------------------------------------------------- sign rule outside [0,1]
+def test_sign_rule_repairs_out_of_range_eigenvalue():
+    """PAPER.md:39: "the +/- sign is chosen to adjust the trace of X_{n+1} ... such that it converges to N_occ".
+    Worked by hand on a diagonal X_0 (bounds override (0,1), so X_0 = I - H):
+      * one eigenvalue at 1 + d, d = 1e-7 (as rounding noise of an FP32 phase leaves it), the rest at 0/1:
+        t = N + d, Tr X^2 = N + 2d + d^2, Tr(2X - X^2) = N - d^2 -> the "+" branch 2X - X^2 lands nearer N_occ and maps
+        1 + d to 1 - d^2; the naive "X^2 iff t > N_occ" would square it to 1 + 2d and double the excess every step.
+      * mirror case, one eigenvalue at -d: t = N - d, Tr X^2 = N + d^2, Tr(2X - X^2) = N - 2d - d^2 -> X^2, mapping -d to d^2."""
+    d = 1e-7
+    for x0, first, fixed in [(np.array([1.0 + d, 1.0, 0.0, 0.0]), "L", 1.0 - d * d),
+                             (np.array([1.0, 1.0, -d, 0.0]), "S", d * d)]:
+        nocc = 2
+        H = np.diag(1.0 - x0)
+        r = oracle.expand(H, nocc, tol=1e-13, bounds_override=(0.0, 1.0), max_iter=20)
+        assert r.branch[0] == first, r.branch
+        assert r.t[0] == pytest.approx(float(x0.sum()), abs=1e-15)
+        one = oracle.expand(H, nocc, variant=oracle.TRUNC, max_iter=1, bounds_override=(0.0, 1.0))
+        i = int(np.argmax(np.abs(x0 * (1 - x0))))          # the out-of-range entry
+        assert np.diag(one.P)[i] == pytest.approx(fixed, abs=1e-20 if fixed < 1e-3 else 1e-15)
+        assert r.converged and r.iterations <= 3
+        assert np.all(np.diag(r.P) >= 0.0) and np.all(np.diag(r.P) <= 1.0)
+        assert np.allclose(np.diag(r.P), [1, 1, 0, 0], atol=1e-13)
+
+
+# ---------------------------------------------------------------- A-Z-RFOE: unexpanded form, step by step
+def test_accelerated_unexpanded_form_traces():
+    """A-Z-RFOE (reading R-ACC) step by step in eigenvalue space: X_n = Q diag(x_n) Q^T, so Tr X_n is the
+    sum of the shifted-and-scaled SP2 polynomial applied to each eigenvalue (pins.scalar_sp2_accel applies
+    ((1-a) + a x)^2 and 2(ax) - (ax)^2 literally).  A dropped shift, a wrong alpha or a swapped HOMO/LUMO image
+    changes t_1 already."""
+    w = _tiny(28, 11, 41)
+    homo, lumo = w.lam[: w.nocc].max(), w.lam[w.nocc:].min()
+    r = oracle.expand(w.H, w.nocc, variant=oracle.SP2_ACCEL, tol=1e-12, homo=homo, lumo=lumo)
+    x = (r.emax - w.lam) / (r.emax - r.emin)
+    beta, bbar = (r.emax - lumo) / (r.emax - r.emin), (r.emax - homo) / (r.emax - r.emin)
+    for n, ch in enumerate(r.branch[:8]):
+        aS, aL = 2.0 / (2.0 - beta), 2.0 / (1.0 + bbar)
+        cand = {"S": ((1.0 - aS) + aS * x) ** 2, "L": 2.0 * (aL * x) - (aL * x) ** 2}
+        # the branch taken is the one whose trace (summing the candidate's eigenvalues) is nearer N_occ
+        assert abs(cand[ch].sum() - w.nocc) <= abs(cand["L" if ch == "S" else "S"].sum() - w.nocc)
+        f = (lambda v, a=aS: ((1.0 - a) + a * v) ** 2) if ch == "S" else (lambda v, a=aL: 2.0 * (a * v) - (a * v) ** 2)
+        x, beta, bbar = f(x), f(beta), f(bbar)
+        assert r.t[n + 1] == pytest.approx(x.sum(), abs=1e-11)
+        assert r.s[n + 1] == pytest.approx((x * x).sum(), abs=1e-11)
+        # HOMO / LUMO images stay the edges of the gap in the mapped spectrum
+        assert beta == pytest.approx(x[w.nocc:].max(), abs=1e-12) and bbar == pytest.approx(x[: w.nocc].min(), abs=1e-12)
+    # estimates outside the spectral bounds are refused (alpha would leave (0, 2))
+    with pytest.raises(RuntimeError):
+        oracle.expand(w.H, w.nocc, variant=oracle.SP2_ACCEL, homo=r.emin - 1.0, lumo=lumo)
+    with pytest.raises(RuntimeError):
+        oracle.expand(w.H, w.nocc, variant=oracle.SP2_ACCEL, homo=lumo, lumo=homo)
+
+
+# ---------------------------------------------------------------- T-RFOE against the exact Fermi-Dirac matrix
+def test_truncated_variant_runs_exactly_m_steps():
+    w = _tiny(32, 12, 17, lo=(-1.0, -0.02), hi=(0.02, 1.0))
+    for m_steps in (1, 5, 9):
+        r = oracle.expand(w.H, w.nocc, variant=oracle.TRUNC, max_iter=m_steps)
+        old = oracle.expand(w.H, w.nocc, tol=0.0, max_iter=m_steps)          # the same arithmetic by the SP2 route
+        assert r.converged and r.iterations == m_steps and not old.converged
+        assert np.array_equal(r.P, old.P) and r.branch == old.branch
+    # even when the expansion has long converged, T-RFOE keeps going to m (no convergence test)
+    r = oracle.expand(w.H, w.nocc, variant=oracle.TRUNC, max_iter=70)
+    assert r.iterations == 70 and r.converged
+
+
+@pytest.mark.parametrize("k", [96, 256])
+def test_truncated_expansion_vs_fermi_dirac(k):
+    """D = [exp(beta (H - mu I)) + I]^-1;  PAPER.md:47-52 (Eq. 2): the truncated G_m(H) "serves as a
+    smeared function" standing in for it, more steps m <-> higher beta;  PAPER.md:86: the paper's matrix with 85 %
+    of the states occupied;  PAPER.md:92: eps1 ~ 1e-3 against the exact Fermi-Dirac density matrix, "around 30"
+    T-RFOE iterations at 500 K.  The paper gives no m <-> beta relation (reading R-TRUNC): for each m the pair
+    (mu, beta) is fitted to the occupancies of G_m by least squares and the paper's error metrics
+    are taken against D_FD = V f(lambda) V^T built from numpy's eigendecomposition."""
+    H = rfoe_inputs.paper_matrix(k)
+    nocc = round(0.85 * k)
+    lam, V = np.linalg.eigh(H)
+    mu0 = 0.5 * (lam[nocc - 1] + lam[nocc])
+    betas, eps1s = [], []
+    for m_steps in (12, 16, 20, 24, 28, 32, 36):
+        r = oracle.expand(H, nocc, variant=oracle.TRUNC, max_iter=m_steps)
+        assert r.iterations == m_steps
+        occ = np.einsum("ij,ij->j", V, r.P @ V)                      # v_i^T G_m v_i
+        assert np.linalg.norm(r.P - (V * occ[None, :]) @ V.T) <= 1e-10   # G_m is a function of H
+        assert occ.min() > -1e-9 and occ.max() < 1 + 1e-9
+        assert np.all(np.diff(occ) <= 1e-9)                          # monotone in energy, like f_FD
+        mu, beta = pins.fit_fermi_dirac(lam, occ, mu0)
+        f = pins.fermi_dirac(lam, mu, beta)
+        D = (V * f[None, :]) @ V.T
+        eps1 = np.linalg.norm(r.P - D) / np.linalg.norm(D)
+        eps2 = abs(r.tr_PH - float(np.sum(f * lam))) / abs(float(np.sum(f * lam)))
+        assert eps1 <= 5e-3 and eps2 <= 5e-3, (m_steps, eps1, eps2)   # paper: eps1 ~ 1e-3
+        assert lam[0] < mu < lam[-1]
+        betas.append(beta)
+        eps1s.append(eps1)
+    assert all(b1 > b0 for b0, b1 in zip(betas, betas[1:]))          # more steps <-> lower temperature (PAPER.md:52)
+    assert betas[-1] / betas[0] > 30
+    assert max(eps1s) >= 1e-4                                        # a smeared stand-in, not the Fermi function itself
+    # "around 30" iterations at 500 K (golden value 3): with the matrix read in Hartree, beta(500 K) = 1 / (k_B T) =
+    # 631.6; the m whose fitted beta is nearest lies within +-25 % of 30 (m runs in steps of 4 here)
+    with open(os.path.join(GOLDEN, "paper_iteration_counts.txt")) as fh:
+        t_iters = int(fh.read().split("VALUES:")[1].split()[2])
+    assert t_iters == 30
+    beta_500K = 1.0 / (3.166811563e-6 * 500.0)
+    m_near = (12, 16, 20, 24, 28, 32, 36)[int(np.argmin(np.abs(np.log(np.array(betas) / beta_500K))))]
+    assert abs(m_near - t_iters) <= 0.25 * t_iters, (m_near, betas)
