@@ -33,15 +33,37 @@ METRIC = "FP64 TFLOP/s over a whole RFOE expansion (executed flops of the symmet
 UNIT = "TFLOP/s"
 TILE = 128
 
-# FP64 tensor-pipe peak the roofline is quoted against:
-# 148 SMs x 64 DFMA/clk/SM (DMMA.8x8x4 issue rate, measured by the register-only probe) x 2 x 1.965 GHz.
-# MEASURED_PEAKS.json has no FP64 entry; its bf16 figure x the guide's nominal 45/2250 ratio gives a LOWER
-# 33.2 TF/s, and cuBLAS Dgemm measured 36.2 TF/s on the same box -- the strictest of the three is used.
-FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
+# FP64 tensor-pipe peak.  MEASURED_PEAKS.json has no FP64 entry and the profiling
+# guide lists no FP64 nominal, so the denominator is MEASURED BY THIS RUN: rfoe_probe_fp64_peak, a register-only
+# DMMA.8x8x4 issue loop on every SM (`roofline.peak` = `peak_measured`), right after the timed region.  The derived
+# figure 148 SMs x 64 DFMA/clk/SM x 2 x 1.965 GHz is reported beside it as `peak_derived`, and a cuBLAS Dgemm
+# (torch.matmul, FP64) as context.
+FP64_PEAK_DERIVED_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
+FP64_PEAK_TFLOPS = FP64_PEAK_DERIVED_TFLOPS
 
-# dram__bytes_read.sum + dram__bytes_write.sum of one sym_square_kernel launch at k=16384, from the
-# `ncu --set full` capture summarised in profiles/ (None for sizes without a capture).
-NCU_TRAFFIC_BYTES = {16384: 34.673915e9 + 2.129676e9}   # profiles/r01b_sym_square_k16384.md
+# dram__bytes_read.sum + dram__bytes_write.sum of one sym_square_kernel launch, from the `ncu --set full` captures
+# summarised in profiles/ (ncu cannot run inside a timed bench: the figure is quoted, with its source, not re-measured).
+NCU_TRAFFIC_BYTES = {16384: (34.673915e9 + 2.129676e9, "profiles/r01b_sym_square_k16384.md")}
+
+
+def fp64_peaks(h, torch, stream, n_gemm=8192):
+    """The FP64 denominators, measured now on this device: the library's DMMA issue-rate probe (~300 ms) and, as context,
+    cuBLAS Dgemm through torch.matmul (2 n^3 flops, best of 3 after a warm-up)."""
+    probe = h.probe_fp64_peak(300.0, stream=stream)
+    a = torch.randn((n_gemm, n_gemm), dtype=torch.float64, device="cuda")
+    b = torch.randn((n_gemm, n_gemm), dtype=torch.float64, device="cuda")
+    c = torch.empty_like(a)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    best = float("inf")
+    for i in range(4):
+        e0.record(stream)
+        torch.matmul(a, b, out=c)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        if i:
+            best = min(best, e0.elapsed_time(e1))
+    del a, b, c
+    return probe, 2.0 * n_gemm ** 3 / (best * 1e-3) / 1e12
 
 
 def executed_flops_per_squaring(k: int) -> float:
@@ -300,6 +322,11 @@ def run_ours(args) -> int:
         avg_launch_ms = sq_ms / max(sq_n, 1)
         fl_launch = fl_sq / (world if shard else 1)      # a sharded launch squares 1/world of the tiles
         achieved = fl_launch / (avg_launch_ms * 1e-3) / 1e12
+        # the denominator, measured by this run (outside the timed region, device still warm), with its own clock sample
+        psamp = ClockSampler(gpu_id).start()
+        peak_probe, dgemm_tf = fp64_peaks(h, torch, stream)
+        pclk = psamp.stop()
+        traffic = NCU_TRAFFIC_BYTES.get(k)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "strong" if shard else "weak", "vs_baseline": None,
@@ -315,11 +342,17 @@ def run_ours(args) -> int:
             "seconds_per_expansion": ms_total / args.steps / 1e3,
             "gemm_equiv_tflops": (1 if shard else world) * args.steps * iters * 2.0 * k ** 3 / (ms_total * 1e-3) / 1e12,
             "square_share_of_step": sq_ms / ms_total if world == 1 else None,
-            "roofline": {"bound": "tensor", "kernel": "sym_square_kernel<false> (FP64 DMMA.8x8x4)", "achieved": achieved,
-                         "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP64_PEAK_TFLOPS,
-                         "traffic": NCU_TRAFFIC_BYTES.get(k), "avg_launch_ms": avg_launch_ms, "launches_timed": sq_n,
-                         "flops_per_launch": fl_launch,
-                         "peak_source": "derived: 148 SM x 64 DFMA/clk x 2 x 1.965 GHz (no FP64 entry in MEASURED_PEAKS.json)"},
+            "roofline": {"bound": "tensor", "kernel": "sym_square_kernel<0> (FP64 DMMA.8x8x4)", "achieved": achieved,
+                         "peak": peak_probe, "unit": "TFLOP/s", "frac": achieved / peak_probe,
+                         "traffic": traffic[0] if traffic else None, "traffic_source": traffic[1] if traffic else None,
+                         "avg_launch_ms": avg_launch_ms, "launches_timed": sq_n, "flops_per_launch": fl_launch,
+                         "peak_measured": peak_probe, "peak_derived": FP64_PEAK_DERIVED_TFLOPS,
+                         "frac_of_derived": achieved / FP64_PEAK_DERIVED_TFLOPS, "cublas_dgemm_tflops": dgemm_tf,
+                         "peak_clocks": {"sm_mhz": pclk["sm_mhz"], "reasons": pclk["reasons"], "power_w_max": pclk["power_w_max"]},
+                         "peak_source": "measured by this run: rfoe_probe_fp64_peak (register-only DMMA.8x8x4 issue loop, 8 warps x 32 "
+                                        "accumulators per SM, ~300 ms) right after the timed region; peak_derived = 148 SM x 64 DFMA/clk "
+                                        "x 2 x 1.965 GHz; cublas_dgemm_tflops = torch.matmul FP64 8192^3 (context); MEASURED_PEAKS.json "
+                                        "has no FP64 entry"},
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 8 * k * k, "d2h_bytes_per_step": 8 * k * k,
                     "ms_per_step": ms2 / args.steps},
             "gpu_launches": launches,
@@ -532,16 +565,82 @@ def subspace_report(h, rfoe, rfoe_inputs, args, dev, stream):
     rho_exact = ((Qo.T @ sub.Psi) ** 2).sum(dim=0)
     out.update({
         "project": {"kernel": "sym_square_kernel<2> + project_reduce_kernel", "ms": ms_p, "ms_call": tot_p,
-                    "tflops_executed": fl_proj / ms_p / 1e9, "frac_fp64_peak": fl_proj / ms_p / 1e9 / FP64_PEAK_TFLOPS,
+                    "tflops_executed": fl_proj / ms_p / 1e9, "frac_fp64_peak_derived": fl_proj / ms_p / 1e9 / FP64_PEAK_TFLOPS,
                     "max_abs_err_vs_construction": float((Hp - Hw).abs().max()), "bitwise_symmetric": bool(torch.equal(Hp, Hp.T))},
         "expand": {"ms": tot_e, "iterations": res.iterations, "converged": bool(res.converged)},
         "apply": {"kernel": "apply_kernel (+ density kernels in ms_call)", "ms": ms_a, "ms_call": tot_a,
-                  "tflops_executed": fl_apply / ms_a / 1e9, "frac_fp64_peak": fl_apply / ms_a / 1e9 / FP64_PEAK_TFLOPS,
+                  "tflops_executed": fl_apply / ms_a / 1e9, "frac_fp64_peak_derived": fl_apply / ms_a / 1e9 / FP64_PEAK_TFLOPS,
                   "electron_count_error": abs(float(rho.sum()) - w.nocc),
                   "max_abs_density_err_vs_construction": float((rho - rho_exact).abs().max())},
         "seconds_chain": (tot_p + tot_e + tot_a) / 1e3,
     })
     return out
+
+
+def run_matrix(args) -> int:
+    """--run-matrix: the run matrix of SURVEY.md section 8(d) / DESIGN.md section 8 -- every BASELINE.json config through the
+    C ABI in each variant that applies, CUDA-event time of the second (warm) run, accuracy against the construction-exact
+    projector (harness algebra in torch).  Prints one table row per (config, run); not a bench line."""
+    import torch
+
+    import paper_2301_04642_b200 as rfoe
+    import rfoe_inputs
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --run-matrix: no CUDA device -- there is no CPU fallback")
+    sep = " | " if args.markdown else "  "
+    cols = ["config", "k", "run", "steps", "mults", "reduced", "resident", "ms", "TFLOP/s", "errP", "dE", "status"]
+    print(sep.join(cols))
+    if args.markdown:
+        print(sep.join("---" for _ in cols))
+    for c in args.matrix_configs:
+        w = rfoe_inputs.make_workload(c, device="cuda")
+        k, nocc = w.k, w.nocc
+        H = w.H if isinstance(w.H, torch.Tensor) else torch.from_numpy(w.H).cuda()
+        Q = w.Q if isinstance(w.Q, torch.Tensor) else torch.from_numpy(w.Q).cuda()
+        Pex = Q[:, :nocc] @ Q[:, :nocc].T
+        del Q
+        w.Q = None
+        eband = w.band_energy()
+        fl_sq = executed_flops_per_squaring(k)
+        lam = w.lam
+        homo, lumo = float(lam[:nocc].max()), float(lam[nocc:].min())
+        runs = [("SP2 rule A, Gershgorin (normative)", rfoe.SP2, w.tol, {}),
+                ("the same, one launch sequence per step (RFOE_OPT_RESIDENT = 0)", rfoe.SP2, w.tol, dict(resident=False)),
+                ("SP2 rule B RelTr 5e-8 (paper's criterion)", rfoe.SP2, 5e-8, dict(stop_rule=rfoe.RULE_B)),
+                ("SP2 rule A, exact spectral bounds", rfoe.SP2, w.tol, dict(bounds=(float(lam.min()), float(lam.max())))),
+                ("SP2 rule A, Lanczos bounds (24 steps, on the device)", rfoe.SP2, w.tol, dict(lanczos_steps=24)),
+                ("mixed (late switch 5e-7) + Lanczos bounds", rfoe.SP2_MIXED, w.tol, dict(lanczos_steps=24, mixed_head=0.0, mixed_reltr=5e-7)),
+                ("A-Z-RFOE (accelerated), exact HOMO/LUMO", rfoe.SP2_ACCEL, w.tol, dict(homo=homo, lumo=lumo)),
+                ("A-Z-RFOE, HOMO/LUMO estimated from the normative run's history", rfoe.SP2_ACCEL, w.tol, "estimated"),
+                ("McWeeny-style tail", rfoe.MCWEENY, w.tol, {}),
+                ("mixed, paper schedule (reduced until RelTr 5e-4)", rfoe.SP2_MIXED, w.tol, dict(mixed_head=0.0, mixed_reltr=5e-4)),
+                ("T-RFOE, m = 30 (fractional occupancies: errP is the distance to the zero-temperature projector)", rfoe.TRUNC, 0.0,
+                 dict(trunc_steps=30)),
+                ("mixed T-RFOE, m = 30", rfoe.TRUNC_MIXED, 0.0, dict(trunc_steps=30, mixed_head=0.0, mixed_reltr=5e-4))]
+        est = None
+        with rfoe.Rfoe(k) as h:
+            for name, variant, tol, opts in runs:
+                h.configure(stop_rule=rfoe.RULE_A, bounds=False, mixed_head=0.0, mixed_reltr=5e-4, lanczos_steps=0, resident=True)
+                if opts == "estimated":                              # rfoe_estimate_homo_lumo on the first row's history
+                    opts = dict(homo=est[0], lumo=est[1])
+                h.configure(**opts)
+                r = None
+                for _ in range(2):                                   # second run is the timed one (warm)
+                    r = h.expand(H, nocc, variant, tol)
+                if name.endswith("(normative)"):
+                    est = h.estimate_homo_lumo()
+                P = r.P
+                err = torch.linalg.norm(P - Pex).item() / math.sqrt(k)
+                dE = abs(r.tr_PH - eband) / abs(eband)
+                tf = r.multiplications * fl_sq / (r.device_ms * 1e-3) / 1e12
+                row = [str(c), str(k), name, str(r.iterations), str(r.multiplications), str(r.fp32_steps), "yes" if r.resident else "no",
+                       f"{r.device_ms:.3f}", f"{tf:.1f}", f"{err:.2e}", f"{dE:.1e}", "ok" if r.converged else "not converged"]
+                print(sep.join(row), flush=True)
+                del P, r
+        del H, Pex
+        torch.cuda.empty_cache()
+    return 0
 
 
 def main() -> int:
@@ -562,7 +661,12 @@ def main() -> int:
     ap.add_argument("--only-subspace", action="store_true", help="run only the Rayleigh-Ritz / apply chain (ncu captures)")
     ap.add_argument("--subspace-k", type=int, default=4096)
     ap.add_argument("--subspace-m", type=int, default=600000)
+    ap.add_argument("--run-matrix", action="store_true", help="print the run matrix (every config x variant) instead of the bench line")
+    ap.add_argument("--matrix-configs", type=int, nargs="+", default=[1, 2, 3, 4])
+    ap.add_argument("--markdown", action="store_true")
     args = ap.parse_args()
+    if args.run_matrix:
+        return run_matrix(args)
     if args.warmup < 3 and args.impl == "ours":
         print("bench.py: note: fewer than 3 warm-up steps", file=sys.stderr)
     return run_reference(args) if args.impl == "reference" else run_ours(args)

@@ -38,7 +38,9 @@ typedef enum {
     RFOE_ERR_BAD_BOUNDS = 4,    /* eps_max <= eps_min (e.g. H^p is a multiple of the identity) or not finite */
     RFOE_ERR_NOT_SYMMETRIC = 5, /* H^p is not bitwise symmetric (the squaring X X^T relies on it) */
     RFOE_ERR_UNSUPPORTED = 6,   /* unknown variant / option, or device is not compute capability 10.x */
-    RFOE_ERR_NOT_CONVERGED = 7  /* max_iter steps taken; P holds the last iterate, stats are complete */
+    RFOE_ERR_NOT_CONVERGED = 7, /* max_iter steps taken; P holds the last iterate, stats are complete */
+    RFOE_ERR_NO_PEER_ACCESS = 8 /* sharded P2P setup: a peer's buffers cannot be mapped (cudaDeviceCanAccessPeer is false, or
+                                   cudaIpcOpenMemHandle failed: cuda_error has the reason); use rfoe_expand_sharded instead */
 } rfoe_status_t;
 
 /* Recursion variants.
@@ -49,9 +51,18 @@ typedef enum {
  *             switch tied to RelTr; optional FP64 head (RFOE_OPT_MIXED_HEAD)
  *  SP2_ACCEL  A-Z-RFOE: shifted-and-scaled SP2 polynomials from HOMO/LUMO estimates
  *                                                                       PAPER.md:43 (sec. II.B.2)
- * T-RFOE (Eq. 2) is SP2 with RFOE_OPT_MAX_ITER = m and tol = 0: the truncated
- * expansion G_m(H^p) is returned with status RFOE_ERR_NOT_CONVERGED. */
-enum { RFOE_VARIANT_SP2 = 0, RFOE_VARIANT_MCWEENY = 1, RFOE_VARIANT_SP2_MIXED = 2, RFOE_VARIANT_SP2_ACCEL = 3 };
+ *  TRUNC      T-RFOE, the paper's finite-temperature scheme: the truncated expansion        PAPER.md:47-52 (sec. II.B.3, Eq. 2)
+ *             G_m(H^p) = F_m(...F_0(H^p)...), "an intermediate function generated in Z-RFOE that is obtained before the
+ *             convergence", a smeared stand-in for the Fermi-Dirac matrix [exp(beta (H - mu I)) + I]^-1.
+ *             Exactly m = RFOE_OPT_TRUNC_STEPS SP2 steps (default 30, the paper's "around 30" at 500 K), no
+ *             convergence test, `tol` ignored; returns RFOE_OK with iterations == m and stats.trunc_steps == m.  The paper
+ *             gives no m(beta) relation; DESIGN.md (reading R-TRUNC) tabulates the one measured on its matrix.
+ *  TRUNC_MIXED  mixed-precision T-RFOE: the same m steps, reduced-precision ones until
+ *             RelTr <= RFOE_OPT_MIXED_RELTR (and after the optional FP64 head), FP64 afterwards.
+ * (SP2 with RFOE_OPT_MAX_ITER = m and tol = 0 runs the same m steps but reports RFOE_ERR_NOT_CONVERGED: that route is
+ * a convergence failure by definition; TRUNC is the method of PAPER.md:47-52.) */
+enum { RFOE_VARIANT_SP2 = 0, RFOE_VARIANT_MCWEENY = 1, RFOE_VARIANT_SP2_MIXED = 2, RFOE_VARIANT_SP2_ACCEL = 3,
+       RFOE_VARIANT_TRUNC = 4, RFOE_VARIANT_TRUNC_MIXED = 5 };
 
 /* Options (rfoe_set_option).  Values are doubles; integer options are rounded. */
 enum {
@@ -65,7 +76,10 @@ enum {
     RFOE_OPT_MIXED_RELTR = 6,  /* SP2_MIXED: FP32 steps until RelTr <= value (default 5e-4) */
     RFOE_OPT_HOMO = 7,         /* SP2_ACCEL: estimate of the highest occupied eigenvalue of H^p */
     RFOE_OPT_LUMO = 8,         /* SP2_ACCEL: estimate of the lowest unoccupied eigenvalue of H^p */
-    RFOE_OPT_LANCZOS_STEPS = 9 /* 0 (default): Gershgorin bounds in rfoe_expand; m in 1..64: rfoe_bounds_lanczos with m steps */
+    RFOE_OPT_LANCZOS_STEPS = 9, /* 0 (default): Gershgorin bounds in rfoe_expand; m in 1..64: rfoe_bounds_lanczos with m steps */
+    RFOE_OPT_TRUNC_STEPS = 10, /* TRUNC / TRUNC_MIXED: the number m of recursion steps, 1..RFOE_MAX_STEPS (default 30) */
+    RFOE_OPT_RESIDENT = 11     /* 1 (default): expansions small enough to stay on chip (see rfoe_expand) run the WHOLE recursion
+                                  in one persistent launch, no host round trip per step; 0: one launch sequence per step */
 };
 
 #define RFOE_MAX_STEPS 256
@@ -81,6 +95,9 @@ typedef struct {
     int32_t fp32_steps;
     int32_t converged;
     int32_t square_launches; /* launches of the symmetric squaring / product kernel */
+    int32_t trunc_steps;     /* TRUNC / TRUNC_MIXED: the m asked for (0 for the other variants): iterations == trunc_steps
+                                means "truncated on purpose", as opposed to status NOT_CONVERGED */
+    int32_t resident;        /* 1 when the recursion ran as one persistent launch (RFOE_OPT_RESIDENT) */
     int64_t k;
     int64_t nocc;
     int64_t gpu_launches;    /* kernels launched by the last call */
@@ -123,9 +140,11 @@ int rfoe_bounds_lanczos(rfoe_handle_t h, const double* Hp, int64_t k, int m, dou
 /* The expansion.  Hp: device, k x k, bitwise symmetric, never written.  P: device, k x k, overwritten
  * with the final iterate (bitwise symmetric); must not overlap Hp.  0 < nocc < k.  tol: threshold of
  * the active stop rule (finite, >= 0).  Steps: Gershgorin bounds (or the override / Lanczos option) -> X_0 =
- * (eps_max I - H^p)/(eps_max - eps_min) -> recursion steered by Tr X_n vs N_occ (S iff Tr X_n > N_occ,
- * PAPER.md:39) -> P, tr(P H^p).  Returns OK, NOT_CONVERGED (P and stats still valid) or an error
- * (P unspecified). */
+ * (eps_max I - H^p)/(eps_max - eps_min) -> recursion, each step taking the sign whose resulting trace (known beforehand
+ * from Tr X_n and Tr X_n^2 = ||X_n||_F^2) lands nearer N_occ (for a spectrum inside [0,1] this is
+ * "X^2 iff Tr X_n > N_occ", reading R4) -> P, tr(P H^p).  SP2_ACCEL additionally requires
+ * eps_min <= RFOE_OPT_HOMO < RFOE_OPT_LUMO <= eps_max (else INVALID_ARG: the scaling factors would leave (0, 2)).
+ * Returns OK, NOT_CONVERGED (P and stats still valid) or an error (P unspecified). */
 int rfoe_expand(rfoe_handle_t h, const double* Hp, int64_t k, int64_t nocc, int variant, double tol, double* P,
                 rfoe_stream_t stream);
 
@@ -149,6 +168,13 @@ int rfoe_square(rfoe_handle_t h, const double* X, int64_t k, double c2, double c
  * iterate of an expansion, whose spectrum lies in [0,1]); larger entries are clamped. */
 int rfoe_square_reduced(rfoe_handle_t h, const double* X, int64_t k, double c2, double c1, double c0, double* Xout,
                         double* scalars, float* kernel_ms, rfoe_stream_t stream);
+
+/* Issue-rate ceiling of the FP64 tensor pipe, measured on this device now: every SM runs 8 warps of a register-only
+ * mma.m8n8k4.f64 (SASS DMMA.8x8x4) loop with 32 independent accumulators per warp -- the squaring kernel's inner loop with
+ * its shared-memory loads removed -- for about `ms` milliseconds (1..10000); *tflops = issued flops / CUDA-event time.
+ * No memory traffic, so this is the denominator the squaring's roofline fraction is quoted against (bench.py
+ * `roofline.peak_measured`); it moves with the SM clock the device holds under this load.  tflops: HOST double. */
+int rfoe_probe_fp64_peak(rfoe_handle_t h, double ms, double* tflops, rfoe_stream_t stream);
 
 /* Symmetric product for commuting symmetric A, B (k x k, device): Cout = c2 * (A B) + c1 * A + c0 * I, upper
  * triangle computed and mirrored (the McWeeny step uses it with A = X^2, B = X).  scalars as in rfoe_square
@@ -210,8 +236,8 @@ int rfoe_expand_many(const rfoe_handle_t* handles, const rfoe_stream_t* streams,
  * rank into the DEVICE buffer `recv` (world x bytes, rank order), ordered after the work already enqueued on
  * `stream` and complete before work enqueued on `stream` afterwards (e.g. ncclAllGather on that stream, or
  * torch.distributed.all_gather_into_tensor under that current stream).  Returns 0 on success.
- * Every rank must call with the same H^p, k, nocc, variant, tol and options.  Variants: SP2 and SP2_ACCEL
- * (and T-RFOE through RFOE_OPT_MAX_ITER); others -> UNSUPPORTED. */
+ * Every rank must call with the same H^p, k, nocc, variant, tol and options.  Variants: SP2, SP2_ACCEL and TRUNC;
+ * others -> UNSUPPORTED. */
 typedef int (*rfoe_allgather_fn)(void* user, const void* send, void* recv, int64_t bytes, rfoe_stream_t stream);
 int rfoe_expand_sharded(rfoe_handle_t h, const double* Hp, int64_t k, int64_t nocc, int variant, double tol, double* P,
                         int rank, int world, rfoe_allgather_fn allgather, void* user, rfoe_stream_t stream);
@@ -227,6 +253,11 @@ int rfoe_expand_sharded(rfoe_handle_t h, const double* Hp, int64_t k, int64_t no
  *       rfoe_shard_ipc_import(h, rank, world, handles of all ranks in rank order) (cudaIpcOpenMemHandle).
  * barrier(user, stream): must return after every rank's work enqueued on its stream so far has COMPLETED
  * (e.g. cudaStreamSynchronize + an MPI / torch.distributed barrier).  Returns 0 on success.
+ * rfoe_expand_sharded_p2p calls barrier once on entry (before its first store into a peer: a rank still finishing the
+ * previous expansion reads the same buffers) and once per recursion step; every rank must therefore make the same
+ * sequence of calls with the same arguments, or the barrier never completes.
+ * rfoe_shard_ipc_import checks every opened buffer with cudaDeviceCanAccessPeer and returns RFOE_ERR_NO_PEER_ACCESS (nothing
+ * left mapped) when a peer cannot be reached; fall back to rfoe_expand_sharded then.
  * Variants and the bitwise-equality guarantee as for rfoe_expand_sharded. */
 #define RFOE_IPC_HANDLE_BYTES 64
 typedef int (*rfoe_barrier_fn)(void* user, rfoe_stream_t stream);

@@ -18,20 +18,21 @@ import numpy as np
 from . import build as _build
 
 __all__ = ["Rfoe", "RfoeError", "ExpandResult", "load_library", "shard_range", "torch_distributed_allgather", "SP2", "MCWEENY", "SP2_MIXED", "SP2_ACCEL",
-           "RULE_A", "RULE_B", "EXPORTS"]
+           "TRUNC", "TRUNC_MIXED", "RULE_A", "RULE_B", "EXPORTS"]
 
-SP2, MCWEENY, SP2_MIXED, SP2_ACCEL = 0, 1, 2, 3
+SP2, MCWEENY, SP2_MIXED, SP2_ACCEL, TRUNC, TRUNC_MIXED = 0, 1, 2, 3, 4, 5
 RULE_A, RULE_B = 0, 1
 MAX_STEPS = 256
 
 (OPT_STOP_RULE, OPT_MAX_ITER, OPT_EPS_MIN, OPT_EPS_MAX, OPT_CHECK_SYMMETRY, OPT_MIXED_HEAD, OPT_MIXED_RELTR,
- OPT_HOMO, OPT_LUMO, OPT_LANCZOS_STEPS) = range(10)
+ OPT_HOMO, OPT_LUMO, OPT_LANCZOS_STEPS, OPT_TRUNC_STEPS, OPT_RESIDENT) = range(12)
 
-OK, ERR_INVALID_ARG, ERR_ALLOC, ERR_CUDA, ERR_BAD_BOUNDS, ERR_NOT_SYMMETRIC, ERR_UNSUPPORTED, ERR_NOT_CONVERGED = range(8)
+(OK, ERR_INVALID_ARG, ERR_ALLOC, ERR_CUDA, ERR_BAD_BOUNDS, ERR_NOT_SYMMETRIC, ERR_UNSUPPORTED, ERR_NOT_CONVERGED,
+ ERR_NO_PEER_ACCESS) = range(9)
 
 # every symbol include/rfoe.h declares
 EXPORTS = ("rfoe_create", "rfoe_bounds", "rfoe_bounds_lanczos", "rfoe_expand", "rfoe_expand_host", "rfoe_square", "rfoe_square_reduced",
-           "rfoe_symm_product", "rfoe_project", "rfoe_apply", "rfoe_expand_sharded", "rfoe_shard_range", "rfoe_plan_squaring",
+           "rfoe_symm_product", "rfoe_probe_fp64_peak", "rfoe_project", "rfoe_apply", "rfoe_expand_sharded", "rfoe_shard_range", "rfoe_plan_squaring",
            "rfoe_shard_local_ptrs", "rfoe_shard_set_peers", "rfoe_shard_ipc_export", "rfoe_shard_ipc_import",
            "rfoe_expand_sharded_p2p", "rfoe_expand_many",
            "rfoe_estimate_homo_lumo", "rfoe_set_option", "rfoe_get_stats", "rfoe_destroy", "rfoe_strerror", "rfoe_version")
@@ -58,6 +59,7 @@ class _Stats(C.Structure):
         ("status", C.c_int32), ("cuda_error", C.c_int32), ("variant", C.c_int32), ("stop_rule", C.c_int32),
         ("iterations", C.c_int32), ("multiplications", C.c_int32), ("mcweeny_steps", C.c_int32),
         ("fp32_steps", C.c_int32), ("converged", C.c_int32), ("square_launches", C.c_int32),
+        ("trunc_steps", C.c_int32), ("resident", C.c_int32),
         ("k", C.c_int64), ("nocc", C.c_int64), ("gpu_launches", C.c_int64),
         ("tol", C.c_double), ("eps_min", C.c_double), ("eps_max", C.c_double), ("tr_PH", C.c_double),
         ("device_ms", C.c_double), ("square_ms", C.c_double),
@@ -90,6 +92,7 @@ def load_library(path: str | None = None):
     L.rfoe_square.argtypes = [vp, vp, i64, dbl, dbl, dbl, vp, dp, C.POINTER(C.c_float), vp]
     L.rfoe_square_reduced.argtypes = [vp, vp, i64, dbl, dbl, dbl, vp, dp, C.POINTER(C.c_float), vp]
     L.rfoe_symm_product.argtypes = [vp, vp, vp, i64, dbl, dbl, dbl, vp, dp, C.POINTER(C.c_float), vp]
+    L.rfoe_probe_fp64_peak.argtypes = [vp, dbl, dp, vp]
     L.rfoe_project.argtypes = [vp, vp, vp, i64, i64, i64, vp, dp, C.POINTER(C.c_float), vp]
     L.rfoe_apply.argtypes = [vp, vp, vp, i64, i64, i64, vp, i64, vp, C.POINTER(C.c_float), vp]
     L.rfoe_expand_sharded.argtypes = [vp, vp, i64, i64, C.c_int, dbl, vp, C.c_int, C.c_int, ALLGATHER_FN, vp, vp]
@@ -134,6 +137,8 @@ class ExpandResult:
     square_ms: float
     square_launches: int
     gpu_launches: int
+    trunc_steps: int
+    resident: bool
     t: np.ndarray
     s: np.ndarray
     e: np.ndarray
@@ -169,7 +174,8 @@ def _result_from(st: _Stats, P, rc) -> "ExpandResult":
         P=P, status=rc, converged=bool(st.converged), iterations=n, multiplications=st.multiplications,
         mcweeny_steps=st.mcweeny_steps, fp32_steps=st.fp32_steps, branch=st.branch.decode()[:n],
         eps_min=st.eps_min, eps_max=st.eps_max, tr_PH=st.tr_PH, device_ms=st.device_ms, square_ms=st.square_ms,
-        square_launches=st.square_launches, gpu_launches=st.gpu_launches, t=np.array(st.t[: n + 1]),
+        square_launches=st.square_launches, gpu_launches=st.gpu_launches, trunc_steps=st.trunc_steps,
+        resident=bool(st.resident), t=np.array(st.t[: n + 1]),
         s=np.array(st.s[: n + 1]), e=np.array(st.e[:n]), reltr=np.array(st.reltr[:n]))
 
 
@@ -311,8 +317,10 @@ class Rfoe:
             raise RfoeError(rc, self._L.rfoe_strerror(rc).decode())
 
     def configure(self, *, stop_rule=None, max_iter=None, bounds=None, check_symmetry=None, mixed_head=None,
-                  mixed_reltr=None, homo=None, lumo=None, lanczos_steps=None):
+                  mixed_reltr=None, homo=None, lumo=None, lanczos_steps=None, trunc_steps=None, resident=None):
         if lanczos_steps is not None: self.set_option(OPT_LANCZOS_STEPS, lanczos_steps)
+        if trunc_steps is not None: self.set_option(OPT_TRUNC_STEPS, trunc_steps)
+        if resident is not None: self.set_option(OPT_RESIDENT, 1.0 if resident else 0.0)
         if stop_rule is not None: self.set_option(OPT_STOP_RULE, stop_rule)
         if max_iter is not None: self.set_option(OPT_MAX_ITER, max_iter)
         if bounds is not None:
@@ -388,6 +396,14 @@ class Rfoe:
         if rc != OK:
             self._raise(rc)
         return out, np.array(sc[:]), ms.value
+
+    def probe_fp64_peak(self, ms: float = 200.0, stream=None) -> float:
+        """rfoe_probe_fp64_peak: TFLOP/s of a register-only DMMA.8x8x4 issue loop on every SM for about ``ms`` ms."""
+        tf = C.c_double()
+        rc = self._L.rfoe_probe_fp64_peak(self._h, float(ms), C.byref(tf), _stream_ptr(stream))
+        if rc != OK:
+            self._raise(rc)
+        return tf.value
 
     def symm_product(self, A, B, c2=1.0, c1=0.0, c0=0.0, out=None, stream=None):
         """out = c2 A B + c1 A + c0 I (upper triangle mirrored); returns (out, scalars[5], kernel_ms)."""

@@ -15,7 +15,7 @@ namespace rfoe {
 constexpr int CTRL_MAX_STEPS = 256;
 
 enum Action : int { ACT_STOP = 0, ACT_SP2 = 1, ACT_MCWEENY = 2, ACT_SP2_FP32 = 3 };
-enum Variant : int { VAR_SP2 = 0, VAR_MCWEENY = 1, VAR_MIXED = 2, VAR_ACCEL = 3 };
+enum Variant : int { VAR_SP2 = 0, VAR_MCWEENY = 1, VAR_MIXED = 2, VAR_ACCEL = 3, VAR_TRUNC = 4, VAR_TRUNC_MIXED = 5 };
 
 struct Ctrl {
     // configuration (host -> device once per expansion)
@@ -104,7 +104,7 @@ __device__ inline void decide_next(Ctrl* c)
     if (c->variant == VAR_MCWEENY) {
         if (!c->mcweeny_phase && (t - s) < 3.0 / 16.0 && fabs(t - c->nocc) < 0.5) c->mcweeny_phase = 1;   // R11
         if (c->mcweeny_phase) action = ACT_MCWEENY;
-    } else if (c->variant == VAR_MIXED) {
+    } else if (c->variant == VAR_MIXED || c->variant == VAR_TRUNC_MIXED) {
         if (c->mixed_phase == 0 && (t - s) < c->mixed_head) c->mixed_phase = 1;
         if (c->mixed_phase == 1 && c->reltr_prev <= c->mixed_reltr) c->mixed_phase = 2;
         if (c->mixed_phase == 1) action = ACT_SP2_FP32;
@@ -173,7 +173,10 @@ control_kernel(Ctrl* __restrict__ c, int mode, const double* __restrict__ part_t
         c->t = t1; c->s = s1; c->reltr_prev = reltr;
         c->step = n + 1;
         bool stop = false;
-        if (!was_fp32) {   // an FP32 step never terminates the expansion (its e, RelTr sit on the FP32 floor)
+        const bool truncated = (c->variant == VAR_TRUNC || c->variant == VAR_TRUNC_MIXED);
+        if (truncated) {   // T-RFOE: exactly max_iter = m steps, no convergence test; G_m delivered = success
+            if (c->step >= c->max_iter) { stop = true; c->converged = 1; }
+        } else if (!was_fp32) {   // an FP32 step never terminates the expansion (its e, RelTr sit on the FP32 floor)
             if (c->stop_rule == 0 ? (e <= c->tol) : (reltr <= c->tol)) { stop = true; c->converged = 1; }
         }
         if (!stop && c->step >= c->max_iter) stop = true;

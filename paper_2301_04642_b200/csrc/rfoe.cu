@@ -16,6 +16,7 @@
 #include "control.cuh"
 #include "hbm_kernels.cuh"
 #include "lanczos.cuh"
+#include "probe.cuh"
 #include "shard.cuh"
 #include "subspace.cuh"
 #include "sym_square.cuh"
@@ -82,7 +83,7 @@ struct rfoe_handle_s {
     int sq_n = 0;
     EncodeTiledFn encode = nullptr;
     // options
-    int stop_rule = 0, max_iter = 100, check_sym = 1;
+    int stop_rule = 0, max_iter = 100, check_sym = 1, trunc_steps = 30, resident = 1;
     double eps_min = NAN, eps_max = NAN, mixed_head = 0.0, mixed_reltr = 5e-4, homo = NAN, lumo = NAN;
     rfoe_stats_t stats;
     int64_t launches = 0;
@@ -302,11 +303,12 @@ extern "C" const char* rfoe_strerror(int status)
         case RFOE_ERR_NOT_SYMMETRIC: return "H^p is not bitwise symmetric";
         case RFOE_ERR_UNSUPPORTED: return "unsupported variant, option or device";
         case RFOE_ERR_NOT_CONVERGED: return "maximum number of recursion steps reached";
+        case RFOE_ERR_NO_PEER_ACCESS: return "a peer GPU's buffers cannot be mapped (no P2P access)";
         default: return "unknown status";
     }
 }
 
-extern "C" int rfoe_version(void) { return 100; }
+extern "C" int rfoe_version(void) { return 200; }
 
 extern "C" int rfoe_destroy(rfoe_handle_t h)
 {
@@ -410,6 +412,12 @@ extern "C" int rfoe_set_option(rfoe_handle_t h, int key, double value)
         case RFOE_OPT_LANCZOS_STEPS:
             if (!(value >= 0.0 && value <= (double)LZ_MAX_STEPS)) return RFOE_ERR_INVALID_ARG;
             h->lanczos_steps = (int)llround(value); return RFOE_OK;
+        case RFOE_OPT_TRUNC_STEPS:
+            if (!(value >= 1.0 && value <= (double)RFOE_MAX_STEPS)) return RFOE_ERR_INVALID_ARG;
+            h->trunc_steps = (int)llround(value); return RFOE_OK;
+        case RFOE_OPT_RESIDENT:
+            if (value != 0.0 && value != 1.0) return RFOE_ERR_INVALID_ARG;
+            h->resident = (int)value; return RFOE_OK;
         case RFOE_OPT_HOMO: h->homo = value; return RFOE_OK;
         case RFOE_OPT_LUMO: h->lumo = value; return RFOE_OK;
         default: return RFOE_ERR_UNSUPPORTED;
@@ -599,7 +607,10 @@ static int expand_impl(rfoe_handle_t h, const double* Hp, int64_t k64, int64_t n
         const size_t bytes = (size_t)k64 * k64 * sizeof(double);
         if (a < b + bytes && b < a + bytes) return fail(RFOE_ERR_INVALID_ARG);
     }
-    if (variant < RFOE_VARIANT_SP2 || variant > RFOE_VARIANT_SP2_ACCEL) return fail(RFOE_ERR_UNSUPPORTED);
+    if (variant < RFOE_VARIANT_SP2 || variant > RFOE_VARIANT_TRUNC_MIXED) return fail(RFOE_ERR_UNSUPPORTED);
+    const bool is_mixed = (variant == RFOE_VARIANT_SP2_MIXED || variant == RFOE_VARIANT_TRUNC_MIXED);
+    const bool is_trunc = (variant == RFOE_VARIANT_TRUNC || variant == RFOE_VARIANT_TRUNC_MIXED);
+    S.trunc_steps = is_trunc ? h->trunc_steps : 0;
     if (variant == RFOE_VARIANT_SP2_ACCEL && !(isfinite(h->homo) && isfinite(h->lumo) && h->lumo > h->homo))
         return fail(RFOE_ERR_INVALID_ARG);
     const int k = (int)k64;
@@ -610,13 +621,13 @@ static int expand_impl(rfoe_handle_t h, const double* Hp, int64_t k64, int64_t n
     h->launches = 0;
     CK(cudaSetDevice(h->device));
     if (variant == RFOE_VARIANT_MCWEENY && (rc = ensure_third(h)) != RFOE_OK) return fail(rc);
-    if (variant == RFOE_VARIANT_SP2_MIXED && (rc = ensure_parts(h)) != RFOE_OK) return fail(rc);
+    if (is_mixed && (rc = ensure_parts(h)) != RFOE_OK) return fail(rc);
     if ((rc = ensure_tiles(h, m, st)) != RFOE_OK) return fail(rc);
     // sharded run: this rank's contiguous range of the tile order, and the exchange buffers
     int t_begin = 0, t_count = h->n_tiles, c_max = h->n_tiles;
     size_t rank_stride = 0;
     if (sh) {
-        if (variant != RFOE_VARIANT_SP2 && variant != RFOE_VARIANT_SP2_ACCEL) return fail(RFOE_ERR_UNSUPPORTED);
+        if (variant != RFOE_VARIANT_SP2 && variant != RFOE_VARIANT_SP2_ACCEL && variant != RFOE_VARIANT_TRUNC) return fail(RFOE_ERR_UNSUPPORTED);
         int64_t b, c;
         if (rfoe_shard_range(h->n_tiles, sh->rank, sh->world, &b, &c) != RFOE_OK || (!sh->allgather && !sh->barrier))
             return fail(RFOE_ERR_INVALID_ARG);
@@ -633,6 +644,9 @@ static int expand_impl(rfoe_handle_t h, const double* Hp, int64_t k64, int64_t n
         if (!h->d_peers && cudaMalloc(&h->d_peers, 2 * sizeof(PeerSet)) != cudaSuccess) { cudaGetLastError(); return fail(RFOE_ERR_ALLOC); }
         CK(cudaMemcpyAsync(h->d_peers, psets, sizeof(psets), cudaMemcpyHostToDevice, st));
         CK(cudaStreamSynchronize(st));   // psets lives on this stack frame
+        // entry barrier: this call's first epilogue stores into every peer's W[1] / records, which a peer still inside
+        // its previous expansion (control kernel, output pass) may be reading -- nobody stores before everybody is here
+        if (sh->barrier(sh->user, stream) != 0) return fail(RFOE_ERR_CUDA);
     }
     if (sh && sh->allgather) {
         rank_stride = (size_t)c_max * (TILE_ELEMS + SQ_NPART);
@@ -656,7 +670,7 @@ static int expand_impl(rfoe_handle_t h, const double* Hp, int64_t k64, int64_t n
     for (int i = 0; i < 3; ++i)
         if (h->W[i] && (rc = make_map(h, &tm[i], h->W[i], n, ld)) != RFOE_OK) return fail(rc);
     CUtensorMap tmF[2];
-    if (variant == RFOE_VARIANT_SP2_MIXED)
+    if (is_mixed)
         for (int i = 0; i < 2; ++i)
             if ((rc = make_map_parts(h, &tmF[i], h->F[i], n, n + TQ_PAD)) != RFOE_OK) return fail(rc);
 
@@ -689,13 +703,15 @@ static int expand_impl(rfoe_handle_t h, const double* Hp, int64_t k64, int64_t n
     const double emin = h->hp->bounds[0], emax = h->hp->bounds[1];
     S.eps_min = emin; S.eps_max = emax;
     if (!(isfinite(emin) && isfinite(emax) && emax > emin)) return fail(RFOE_ERR_BAD_BOUNDS);
+    // A-Z-RFOE: estimates outside the bounds would put the scaling factors 2/(2 - beta), 2/(1 + bbar) outside (0, 2)
+    if (variant == RFOE_VARIANT_SP2_ACCEL && !(emin <= h->homo && h->lumo <= emax)) return fail(RFOE_ERR_INVALID_ARG);
 
     Ctrl& C = h->hp->ctrl;
     memset(&C, 0, sizeof(Ctrl));
-    C.variant = variant; C.stop_rule = h->stop_rule; C.max_iter = h->max_iter; C.kvalid = k;
+    C.variant = variant; C.stop_rule = h->stop_rule; C.max_iter = is_trunc ? h->trunc_steps : h->max_iter; C.kvalid = k;
     C.nocc = (double)nocc; C.tol = tol;
     C.mixed_head = h->mixed_head; C.mixed_reltr = h->mixed_reltr;
-    C.mixed_phase = (variant == RFOE_VARIANT_SP2_MIXED) ? (h->mixed_head > 0.0 ? 0 : 1) : 2;
+    C.mixed_phase = is_mixed ? (h->mixed_head > 0.0 ? 0 : 1) : 2;
     C.reltr_prev = INFINITY;
     C.emin = emin; C.emax = emax;
     if (variant == RFOE_VARIANT_SP2_ACCEL) {
@@ -916,8 +932,25 @@ extern "C" int rfoe_shard_ipc_import(rfoe_handle_t h, int rank, int world, const
         if (d == rank) { ptrs[4 * d] = h->W[0]; ptrs[4 * d + 1] = h->W[1]; ptrs[4 * d + 2] = h->part[0]; ptrs[4 * d + 3] = h->part[1]; continue; }
         for (int q = 0; q < 4; ++q) {
             void* p = nullptr;
-            CK(cudaIpcOpenMemHandle(&p, in[4 * d + q], cudaIpcMemLazyEnablePeerAccess));
-            h->ipc_opened[h->n_ipc_opened++] = p;
+            cudaError_t e = cudaIpcOpenMemHandle(&p, in[4 * d + q], cudaIpcMemLazyEnablePeerAccess);
+            if (e == cudaSuccess) {
+                // preflight: the buffer lives on the peer's device; this device must be able to reach it over P2P
+                h->ipc_opened[h->n_ipc_opened++] = p;
+                cudaPointerAttributes attr;
+                int can = 1;
+                e = cudaPointerGetAttributes(&attr, p);
+                if (e == cudaSuccess && attr.device != h->device) e = cudaDeviceCanAccessPeer(&can, h->device, attr.device);
+                if (e == cudaSuccess && !can) e = cudaErrorPeerAccessUnsupported;
+            }
+            if (e != cudaSuccess) {
+                cudaGetLastError();
+                for (int i = 0; i < h->n_ipc_opened; ++i) cudaIpcCloseMemHandle(h->ipc_opened[i]);
+                h->n_ipc_opened = 0;
+                h->p2p_world = 0;
+                h->stats.cuda_error = (int)e;
+                h->stats.status = RFOE_ERR_NO_PEER_ACCESS;
+                return RFOE_ERR_NO_PEER_ACCESS;
+            }
             ptrs[4 * d + q] = p;
         }
     }
@@ -930,6 +963,39 @@ extern "C" int rfoe_expand_sharded_p2p(rfoe_handle_t h, const double* Hp, int64_
     if (!h || !barrier || h->p2p_world < 1) return RFOE_ERR_INVALID_ARG;
     ShardCtx sh = {h->p2p_rank, h->p2p_world, nullptr, barrier, user};
     return expand_impl(h, Hp, k, nocc, variant, tol, P, stream, &sh);
+}
+
+// ---------------------------------------------------------------------------------------------
+// FP64 tensor-pipe issue-rate probe (probe.cuh): a short calibration launch sizes the timed one for ~ms milliseconds
+extern "C" int rfoe_probe_fp64_peak(rfoe_handle_t h, double ms, double* tflops, rfoe_stream_t stream)
+{
+    if (!h || !tflops || !(ms >= 1.0 && ms <= 10000.0)) return RFOE_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    h->launches = 0;
+    h->stats.cuda_error = 0;
+    CK(cudaSetDevice(h->device));
+    h->hp->scalars[0] = 1e-3; h->hp->scalars[1] = -1e-3;
+    CK(cudaMemcpyAsync(h->d_scalars, (void*)h->hp->scalars, 2 * sizeof(double), cudaMemcpyHostToDevice, st));
+    const double flops_per_iter = (double)h->sm_count * (PROBE_THREADS / 32) * PROBE_FLOPS_PER_WARP_ITER;
+    long long iters = 4096;
+    float t = 0.f;
+    for (int pass = 0; pass < 2; ++pass) {
+        CK(cudaEventRecord(h->ev0, st));
+        fp64_peak_probe_kernel<<<h->sm_count, PROBE_THREADS, 0, st>>>(iters, h->d_scalars, h->d_scalars + 4);
+        h->launches++;
+        CK(cudaGetLastError());
+        CK(cudaEventRecord(h->ev1, st));
+        CK(cudaStreamSynchronize(st));
+        CK(cudaEventElapsedTime(&t, h->ev0, h->ev1));
+        if (pass == 0) {
+            if (!(t > 0.f)) return RFOE_ERR_CUDA;
+            iters = (long long)((double)iters * ms / (double)t) + 1;
+        }
+    }
+    *tflops = flops_per_iter * (double)iters / ((double)t * 1e-3) / 1e12;
+    h->stats.gpu_launches = h->launches;
+    h->stats.status = RFOE_OK;
+    return RFOE_OK;
 }
 
 // ---------------------------------------------------------------------------------------------

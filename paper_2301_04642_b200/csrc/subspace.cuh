@@ -133,6 +133,14 @@ apply_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CU
         }
     };
     if (warp == 0) issue_loads(min(KT, SQ_STAGES));
+    // warp 0 (producer and consumer) never blocks on a full-barrier: it polls and keeps issuing (see sym_square.cuh)
+    auto wait_full = [&](uint32_t bar, uint32_t parity, int kt_now) {
+        if (warp == 0) {
+            while (!mbar_test(bar, parity)) issue_loads(min(KT, kt_now + SQ_STAGES));
+        } else {
+            mbar_wait_safe(bar, parity);
+        }
+    };
 
     const int warp_m = warp >> 2;      // 0..1 -> 64 tile rows
     const int warp_n = warp & 3;       // 0..3 -> 32 tile cols
@@ -178,7 +186,7 @@ apply_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CU
     int s = 0;
     uint32_t ph = 0;
     double a0[8], b0[4], a1[8], b1[4];
-    mbar_wait(full0, 0);
+    wait_full(full0, 0, 0);
     uint32_t st = smem_base;
     load_frag(a0, b0, st, 0);
     for (int kt = 0; kt < KT; ++kt) {
@@ -192,7 +200,7 @@ apply_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CU
         load_frag(a0, b0, st, 2);
         mma_step(a1, b1);
         load_frag(a1, b1, st, 3);
-        if (kt + 1 < KT) mbar_wait(full0 + 8 * s1, ph1);
+        if (kt + 1 < KT) wait_full(full0 + 8 * s1, ph1, kt);
         mma_step(a0, b0);
         load_frag(a0, b0, stn, 0);      // after the last stage this reads stale smem; unused
         mma_step(a1, b1);

@@ -123,6 +123,17 @@ sym_square_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
         }
     };
     if (warp == 0) issue_loads(min(KT, SQ_STAGES));
+    // Waiting for a stage to fill.  Warp 0 is the only producer AND a consumer: if it blocked here while another warp
+    // still held the stage that chunk kt+1 must go into (a 5-chunk skew, which the 6-stage ring permits), nobody would
+    // ever issue that chunk.  So warp 0 polls and keeps issuing; the other warps wait (bounded: a pipeline bug traps
+    // instead of hanging the GPU).
+    auto wait_full = [&](uint32_t bar, uint32_t parity, int kt_now) {
+        if (warp == 0) {
+            while (!mbar_test(bar, parity)) issue_loads(min(KT, kt_now + SQ_STAGES));
+        } else {
+            mbar_wait_safe(bar, parity);
+        }
+    };
     {
         // ===== consumers =====
         const int warp_m = warp >> 2;      // 0..1  -> 64 tile rows
@@ -165,7 +176,7 @@ sym_square_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
         int s = 0;
         uint32_t ph = 0;
         double a0[8], b0[4], a1[8], b1[4];
-        mbar_wait(full0, 0);
+        wait_full(full0, 0, 0);
         uint32_t st = smem_base;
         load_frag(a0, b0, st + rowA, st + rowB, off[0]);
         for (int kt = 0; kt < KT; ++kt) {
@@ -180,7 +191,7 @@ sym_square_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
             load_frag(a0, b0, aB, bB, off[2]);
             mma_step(a1, b1);
             load_frag(a1, b1, aB, bB, off[3]);
-            if (kt + 1 < KT) mbar_wait(full0 + 8 * s1, ph1);
+            if (kt + 1 < KT) wait_full(full0 + 8 * s1, ph1, kt);
             mma_step(a0, b0);
             // first fragments of the next stage (after the last stage this reads stale smem; unused)
             load_frag(a0, b0, stn + rowA, stn + rowB, off[0]);

@@ -129,6 +129,7 @@ def _check_expansion(w, res, ref, *, ptol=1e-10, etol=1e-11, inv=1.0):
     decided = np.abs(ref.t[: ref.iterations] - w.nocc) > 1e-9 * max(1.0, k / 256)
     assert all(a == b for a, b, d in zip(res.branch, ref.branch, decided) if d), (res.branch, ref.branch)
     assert np.linalg.norm(P - ref.P) / math.sqrt(k) <= ptol
+    assert np.abs(P - ref.P).max() <= ptol / 10.0            # every element, not only the norm (measured: 1e-15 .. 3e-14)
     assert abs(res.tr_PH - ref.tr_PH) / abs(ref.tr_PH) <= etol
     assert np.array_equal(P, P.T)
     assert abs(res.eps_min - ref.emin) <= 1e-12 * abs(ref.emin) and abs(res.eps_max - ref.emax) <= 1e-12 * abs(ref.emax)
@@ -183,14 +184,64 @@ def test_expand_bounds_override_and_truncated(handle):
         res = handle.expand(_dev(w.H), w.nocc, rfoe.SP2, w.tol)
         _check_expansion(w, res, ref)
         assert res.iterations < 30
-        # T-RFOE: truncated expansion G_m
+        # the MAX_ITER route: m steps of SP2 with an unreachable tolerance is a convergence FAILURE by definition
         handle.configure(max_iter=7)
         ref = oracle.expand(w.H, w.nocc, tol=0.0, max_iter=7, bounds_override=(lo, hi))
         res = handle.expand(_dev(w.H), w.nocc, rfoe.SP2, 0.0)
-        assert res.status == rfoe.ERR_NOT_CONVERGED and res.iterations == 7
+        assert res.status == rfoe.ERR_NOT_CONVERGED and res.iterations == 7 and res.trunc_steps == 0
         _check_expansion(w, res, ref)
+        # T-RFOE proper (Eq. 2): RFOE_VARIANT_TRUNC with m steps delivers G_m and reports success
+        handle.configure(max_iter=100, trunc_steps=7)
+        ref = oracle.expand(w.H, w.nocc, variant=oracle.TRUNC, max_iter=7, bounds_override=(lo, hi))
+        res2 = handle.expand(_dev(w.H), w.nocc, rfoe.TRUNC, 0.0)
+        assert res2.status == rfoe.OK and res2.converged and res2.iterations == 7 and res2.trunc_steps == 7
+        _check_expansion(w, res2, ref)
+        assert torch.equal(res2.P, res.P)
     finally:
-        handle.configure(bounds=False, max_iter=100)
+        handle.configure(bounds=False, max_iter=100, trunc_steps=30)
+
+
+@pytest.mark.parametrize("k", [384, 2048])
+def test_truncated_paper_matrix_vs_oracle_and_fermi_dirac(k):
+    """T-RFOE as the paper runs it: its synthetic H^p, 85 % of the states occupied, m = 30 steps.
+    Against the whole oracle (every element of G_m, same branch string), and against the exact Fermi-Dirac density
+    matrix D = [exp(beta (H - mu)) + I]^-1 with (mu, beta) fitted to the occupancies (reading R-TRUNC):
+    eps1 at the paper's order (~1e-3), eps2 small."""
+    H = rfoe_inputs.paper_matrix(k)
+    nocc = round(0.85 * k)
+    m_steps = 30
+    ref = oracle.expand(H, nocc, variant=oracle.TRUNC, max_iter=m_steps)
+    with rfoe.Rfoe(k) as h:
+        h.configure(trunc_steps=m_steps)
+        res = h.expand(_dev(H), nocc, rfoe.TRUNC, 0.0)
+        assert res.status == rfoe.OK and res.iterations == m_steps == res.trunc_steps and res.branch == ref.branch
+        G = res.P.cpu().numpy()
+        assert np.linalg.norm(G - ref.P) / math.sqrt(k) <= 1e-10 and np.abs(G - ref.P).max() <= 1e-11
+        assert abs(res.tr_PH - ref.tr_PH) <= 1e-11 * abs(ref.tr_PH)
+        assert np.allclose(res.t, ref.t, rtol=1e-12, atol=0) and np.allclose(res.s, ref.s, rtol=1e-12, atol=0)
+        lam, V = np.linalg.eigh(H)
+        occ = np.einsum("ij,ij->j", V, G @ V)
+        mu, beta = pins.fit_fermi_dirac(lam, occ, 0.5 * (lam[nocc - 1] + lam[nocc]))
+        f = pins.fermi_dirac(lam, mu, beta)
+        D = (V * f[None, :]) @ V.T
+        eps1 = np.linalg.norm(G - D) / np.linalg.norm(D)
+        eps2 = abs(res.tr_PH - float(np.sum(f * lam))) / abs(float(np.sum(f * lam)))
+        frac = int(np.sum((occ > 1e-3) & (occ < 1 - 1e-3)))
+        print(f"T-RFOE k={k} m={m_steps}: beta={beta:.4g} mu={mu:.5f} eps1={eps1:.2e} eps2={eps2:.2e} fractional={frac}")
+        assert eps1 <= 5e-3 and eps2 <= 5e-3 and frac >= 3
+        # mixed-precision T-RFOE (PAPER.md:66, 92, 128): same m, reduced-precision steps until RelTr <= 5e-4
+        h.configure(mixed_head=0.0, mixed_reltr=5e-4)
+        mx = h.expand(_dev(H), nocc, rfoe.TRUNC_MIXED, 0.0)
+        refm = oracle.expand(H, nocc, variant=oracle.TRUNC_MIXED, max_iter=m_steps, mixed_head=0.0, mixed_reltr=5e-4)
+        assert mx.status == rfoe.OK and mx.iterations == m_steps and mx.fp32_steps == refm.fp32_steps >= 5
+        assert [c.islower() for c in mx.branch] == [c.islower() for c in refm.branch]
+        Gm = mx.P.cpu().numpy()
+        e1m = np.linalg.norm(Gm - G) / np.linalg.norm(G)
+        e1o = np.linalg.norm(refm.P - ref.P) / np.linalg.norm(ref.P)
+        print(f"  mixed: fp32 steps {mx.fp32_steps}, eps1 vs FP64 G_m: kernel {e1m:.2e}, oracle FP32 loop {e1o:.2e}")
+        # FP32-level agreement with the FP64 G_m; the kernel's reduced step is not worse than the oracle's plain FP32 loop
+        assert e1m <= 1e-4 and e1m <= 3.0 * e1o + 1e-7
+        assert np.linalg.norm(Gm - D) / np.linalg.norm(D) <= 5e-3
 
 
 def test_expand_mcweeny(handle):
@@ -210,6 +261,14 @@ def test_expand_accelerated(handle):
     _check_expansion(w, res, ref)
     plain = handle.expand(_dev(w.H), w.nocc, rfoe.SP2, w.tol)
     assert res.iterations < plain.iterations
+    # estimates outside the spectral bounds are refused on both sides (the scaling factors would leave (0, 2))
+    handle.configure(homo=res.eps_min - 1.0, lumo=lumo)
+    with pytest.raises(rfoe.RfoeError) as ei:
+        handle.expand(_dev(w.H), w.nocc, rfoe.SP2_ACCEL, w.tol)
+    assert ei.value.status == rfoe.ERR_INVALID_ARG
+    with pytest.raises(RuntimeError):
+        oracle.expand(w.H, w.nocc, variant=oracle.SP2_ACCEL, tol=w.tol, homo=res.eps_min - 1.0, lumo=lumo)
+    handle.configure(homo=homo, lumo=lumo)
 
 
 @pytest.mark.parametrize("c,k", [(1, 256), (2, 333), (4, 450)])
@@ -367,8 +426,43 @@ def test_expand_mixed_paper_schedule(handle):
     assert res.converged and res.iterations == ref.iterations and res.fp32_steps == ref.fp32_steps
     assert abs(np.trace(P) - w.nocc) <= 1e-9
     err = np.linalg.norm(P - w.exact_projector()) / math.sqrt(w.k)
-    assert err <= 2e-4
+    err_oracle = np.linalg.norm(ref.P - w.exact_projector()) / math.sqrt(w.k)
+    print(f"paper schedule k={w.k}: errP kernel {err:.2e}, oracle FP32 loop {err_oracle:.2e}, fp32 steps {res.fp32_steps}")
+    # the oracle's plain FP32 loop on the same input sets the scale (a few 1e-5 here, R-MIX): the kernel's reduced step
+    # (FP16 parts, exact products) must not be worse than it, and both stay FP32-sized
+    assert err <= 1.5 * err_oracle + 1e-7 and err <= 2e-4
     assert abs(res.tr_PH - w.band_energy()) / abs(w.band_energy()) <= 1e-7
+
+
+def test_expand_mixed_paper_matrix_eps1():
+    """mixed-precision Z-RFOE reaches eps1 ~ 1e-7, eps2 ~ 1e-9 on the paper's matrix (PAPER.md:86,
+    N_occ = 0.9 k) with FP32 steps until RelTr <= 5e-4.  Stop rule A here, so that the FP32 damage is not hidden behind
+    the RelTr 5e-8 stop; D_ref from an eigendecomposition, as in the paper."""
+    k = 1024
+    H = rfoe_inputs.paper_matrix(k)
+    nocc = round(0.9 * k)
+    lam, V = np.linalg.eigh(H)
+    Dref = V[:, :nocc] @ V[:, :nocc].T
+    eband = float(lam[:nocc].sum())
+    with rfoe.Rfoe(k) as h:
+        h.configure(mixed_head=0.0, mixed_reltr=5e-4)
+        r64 = h.expand(_dev(H), nocc, rfoe.SP2, 4e-12)
+        mx = h.expand(_dev(H), nocc, rfoe.SP2_MIXED, 4e-12)
+    assert r64.converged and mx.converged and mx.fp32_steps >= 10
+    e64 = np.linalg.norm(r64.P.cpu().numpy() - Dref) / math.sqrt(nocc)
+    e1 = np.linalg.norm(mx.P.cpu().numpy() - Dref) / math.sqrt(nocc)
+    e2 = abs(mx.tr_PH - eband) / abs(eband)
+    print(f"paper matrix k={k}: eps1 fp64 {e64:.2e}, mixed {e1:.2e}, eps2 mixed {e2:.2e}, fp32 steps {mx.fp32_steps}/{mx.iterations}")
+    assert e64 <= 1e-9
+    assert e1 <= 2e-6 and e2 <= 1e-8          # paper: ~1e-7 / ~1e-9; a regression of the reduced kernel by 10x fails this
+
+
+def test_probe_fp64_peak(handle):
+    """rfoe_probe_fp64_peak: register-only DMMA issue loop; B200's FP64 tensor pipe is 128 flop/clk/SM (37.2 TFLOP/s at
+    1965 MHz on 148 SMs), and no clock this part runs at takes it below 20."""
+    tf = handle.probe_fp64_peak(50.0)
+    print(f"FP64 DMMA issue-rate probe: {tf:.2f} TFLOP/s")
+    assert 20.0 < tf < 40.0
 
 
 def test_expand_mixed_truncated(handle):
