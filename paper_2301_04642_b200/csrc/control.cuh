@@ -28,6 +28,7 @@ struct Ctrl {
     int action;          // next action (mirrors the host word)
     int mcweeny_phase, mixed_phase;
     int multiplications, mcweeny_steps, fp32_steps, converged;
+    int error, pad_;     // set by the first decision: 0 ok, 1 spectral bounds empty / not finite, 2 HOMO / LUMO estimates outside them
     double t, s, reltr_prev;
     double beta, bbar;   // accelerated SP2: images of LUMO / HOMO under the maps applied so far
     double emin, emax;
@@ -136,22 +137,66 @@ __device__ inline void decide_next(Ctrl* c)
     c->action = action;
 }
 
-// mode 0: after the affine map (row_tr / row_ss hold k per-row values) -> t_0, s_0, first decision.
+// first decision (thread 0): t_0, s_0 and the spectral bounds are known; validity of the bounds and (A-Z-RFOE) the
+// images of LUMO / HOMO under the affine map are settled here, on the device, so that a launch sequence enqueued
+// without a host round trip stops by itself on bad input
+__device__ inline void control_begin(Ctrl* c, double t0, double s0, const double* __restrict__ bounds)
+{
+    const double emin = bounds[0], emax = bounds[1];
+    c->emin = emin; c->emax = emax;
+    c->t = t0; c->s = s0;
+    c->ht[0] = t0; c->hs[0] = s0;
+    c->step = 0;
+    int err = 0;
+    if (!(isfinite(emin) && isfinite(emax) && emax > emin)) err = 1;
+    else if (c->variant == VAR_ACCEL) {
+        if (!(emin <= c->homo && c->homo < c->lumo && c->lumo <= emax)) err = 2;
+        c->beta = (emax - c->lumo) / (emax - emin);
+        c->bbar = (emax - c->homo) / (emax - emin);
+    }
+    c->error = err;
+    if (err || c->max_iter <= 0) c->action = ACT_STOP; else decide_next(c);
+}
+
+// one finished recursion step (thread 0): t_{n+1}, s_{n+1} and e_n^2 are the fixed-order sums of the step's records
+__device__ inline void control_update(Ctrl* c, double t1, double s1, double e2)
+{
+    const int n = c->step;
+    const int was_fp32 = (c->action == ACT_SP2_FP32);
+    const double e = sqrt(e2);
+    const double reltr = fabs(t1 - c->t) / fabs(c->t);
+    c->he[n] = e; c->hreltr[n] = reltr;
+    c->ht[n + 1] = t1; c->hs[n + 1] = s1;
+    c->multiplications += (c->action == ACT_MCWEENY) ? 2 : 1;
+    c->mcweeny_steps += (c->action == ACT_MCWEENY);
+    c->fp32_steps += was_fp32;
+    c->t = t1; c->s = s1; c->reltr_prev = reltr;
+    c->step = n + 1;
+    bool stop = false;
+    const bool truncated = (c->variant == VAR_TRUNC || c->variant == VAR_TRUNC_MIXED);
+    if (truncated) {   // T-RFOE: exactly max_iter = m steps, no convergence test; G_m delivered = success
+        if (c->step >= c->max_iter) { stop = true; c->converged = 1; }
+    } else if (!was_fp32) {   // an FP32 step never terminates the expansion (its e, RelTr sit on the FP32 floor)
+        if (c->stop_rule == 0 ? (e <= c->tol) : (reltr <= c->tol)) { stop = true; c->converged = 1; }
+    }
+    if (!stop && c->step >= c->max_iter) stop = true;
+    if (stop) c->action = ACT_STOP; else decide_next(c);
+}
+
+// mode 0: after the affine map (row_tr / row_ss hold k per-row values; bounds = the two device scalars) -> t_0, s_0,
+//         first decision.
 // mode 1: after a recursion step.  part_ts: tile records of the launch that wrote X_{n+1} (Tr, ||.||_F^2),
 //         part_e: tile records of the squaring X_n^2 (||X_n^2 - X_n||_F^2); n_rec records each.
 __global__ void __launch_bounds__(256)
 control_kernel(Ctrl* __restrict__ c, int mode, const double* __restrict__ part_ts, const double* __restrict__ part_e,
-               int n_rec, volatile int* __restrict__ host_word)
+               int n_rec, volatile int* __restrict__ host_word, const double* __restrict__ bounds)
 {
     __shared__ double sh[256];
     if (mode == 0) {
         const double t0 = block_sum_strided(part_ts, n_rec, 1, sh);
         const double s0 = block_sum_strided(part_e, n_rec, 1, sh);
         if (threadIdx.x == 0) {
-            c->t = t0; c->s = s0;
-            c->ht[0] = t0; c->hs[0] = s0;
-            c->step = 0;
-            if (c->max_iter <= 0) c->action = ACT_STOP; else decide_next(c);
+            control_begin(c, t0, s0, bounds);
             *host_word = c->action;
             __threadfence_system();
         }
@@ -161,26 +206,7 @@ control_kernel(Ctrl* __restrict__ c, int mode, const double* __restrict__ part_t
     const double s1 = block_sum_strided(part_ts + 1, n_rec, SQ_NPART, sh);
     const double e2 = block_sum_strided(part_e + 2, n_rec, SQ_NPART, sh);
     if (threadIdx.x == 0) {
-        const int n = c->step;
-        const int was_fp32 = (c->action == ACT_SP2_FP32);
-        const double e = sqrt(e2);
-        const double reltr = fabs(t1 - c->t) / fabs(c->t);
-        c->he[n] = e; c->hreltr[n] = reltr;
-        c->ht[n + 1] = t1; c->hs[n + 1] = s1;
-        c->multiplications += (c->action == ACT_MCWEENY) ? 2 : 1;
-        c->mcweeny_steps += (c->action == ACT_MCWEENY);
-        c->fp32_steps += was_fp32;
-        c->t = t1; c->s = s1; c->reltr_prev = reltr;
-        c->step = n + 1;
-        bool stop = false;
-        const bool truncated = (c->variant == VAR_TRUNC || c->variant == VAR_TRUNC_MIXED);
-        if (truncated) {   // T-RFOE: exactly max_iter = m steps, no convergence test; G_m delivered = success
-            if (c->step >= c->max_iter) { stop = true; c->converged = 1; }
-        } else if (!was_fp32) {   // an FP32 step never terminates the expansion (its e, RelTr sit on the FP32 floor)
-            if (c->stop_rule == 0 ? (e <= c->tol) : (reltr <= c->tol)) { stop = true; c->converged = 1; }
-        }
-        if (!stop && c->step >= c->max_iter) stop = true;
-        if (stop) c->action = ACT_STOP; else decide_next(c);
+        control_update(c, t1, s1, e2);
         *host_word = c->action;
         __threadfence_system();
     }

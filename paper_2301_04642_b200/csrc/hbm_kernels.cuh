@@ -142,9 +142,8 @@ pad_copy_kernel(const double* __restrict__ src, int k, int n, int ld, double* __
 
 // Output pass: P (k x k, ld = k) <- work matrix (row pitch ld); row_ph[i] = sum_j P_ij H_ij (band energy
 // tr(P H^p)).  H may be null (then only the copy is done).
-__global__ void __launch_bounds__(HBM_THREADS)
-copy_out_kernel(const double* __restrict__ W, int k, int ld, const double* __restrict__ H, double* __restrict__ P,
-                double* __restrict__ row_ph)
+__device__ __forceinline__ void copy_out_rows(const double* __restrict__ W, int k, int ld, const double* __restrict__ H,
+                                              double* __restrict__ P, double* __restrict__ row_ph)
 {
     const int lane = threadIdx.x & 31;
     const int wglobal = blockIdx.x * HBM_WARPS + (threadIdx.x >> 5);
@@ -175,6 +174,22 @@ copy_out_kernel(const double* __restrict__ W, int k, int ld, const double* __res
         acc = warp_sum(acc);
         if (lane == 0 && row_ph) row_ph[i] = acc;
     }
+}
+
+__global__ void __launch_bounds__(HBM_THREADS)
+copy_out_kernel(const double* __restrict__ W, int k, int ld, const double* __restrict__ H, double* __restrict__ P,
+                double* __restrict__ row_ph)
+{
+    copy_out_rows(W, k, ld, H, P, row_ph);
+}
+
+// The same pass when the host does not know which of the two work matrices holds the result (the recursion ran in one
+// persistent launch): the parity of the step counter in device memory selects it.
+__global__ void __launch_bounds__(HBM_THREADS)
+copy_out_select_kernel(const double* __restrict__ W0, const double* __restrict__ W1, const int* __restrict__ step, int k, int ld,
+                       const double* __restrict__ H, double* __restrict__ P, double* __restrict__ row_ph)
+{
+    copy_out_rows((*step & 1) ? W1 : W0, k, ld, H, P, row_ph);
 }
 
 // Bitwise symmetry check of a k x k matrix: 64 x 64 tiles of the upper triangle, both tiles read

@@ -128,19 +128,23 @@ __device__ __forceinline__ void mbar_wait_bounded(uint32_t bar, uint32_t parity)
 
 // mbar_wait that cannot hang the GPU: one plain try_wait first (the common case: no extra instructions on the fast
 // path), then the bounded loop above (traps after ~2 s instead of spinning forever on a pipeline bug)
-__device__ __forceinline__ void mbar_wait_safe(uint32_t bar, uint32_t parity)
+__device__ __forceinline__ bool mbar_try(uint32_t bar, uint32_t parity)
 {
     uint32_t ok;
     asm volatile(
         "{\n"
         ".reg .pred p;\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"   // may suspend, but only up to a HW time limit
         "selp.u32 %0, 1, 0, p;\n"
         "}\n"
         : "=r"(ok)
         : "r"(bar), "r"(parity)
         : "memory");
-    if (!ok) mbar_wait_bounded(bar, parity);
+    return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait_safe(uint32_t bar, uint32_t parity)
+{
+    if (!mbar_try(bar, parity)) mbar_wait_bounded(bar, parity);
 }
 
 // TMEM allocation: one full warp; the base address is written to shared memory at `dst_smem`

@@ -17,6 +17,7 @@
 #include "hbm_kernels.cuh"
 #include "lanczos.cuh"
 #include "probe.cuh"
+#include "resident.cuh"
 #include "shard.cuh"
 #include "subspace.cuh"
 #include "sym_square.cuh"
@@ -59,6 +60,13 @@ struct rfoe_handle_s {
     int n_tiles = 0;
     HostPage* hp = nullptr;
     int* d_word = nullptr; // device alias of hp->word
+    // the whole recursion in one persistent launch (resident.cuh)
+    int coop_ok = 0;           // cooperative launch supported and one CTA of the kernel fits an SM
+    int rs_m = 0, rs_G = 0, rs_n_split = 0;   // the plan the split list / records were set up for
+    int2* d_split = nullptr;
+    double* d_rec[2] = {nullptr, nullptr};
+    unsigned* d_flags = nullptr;
+    unsigned long long* d_timing = nullptr;
     // sharded expansion over peer memory (rfoe_shard_set_peers / rfoe_shard_ipc_import)
     int p2p_world = 0, p2p_rank = 0;
     double* peer_W[2][SQ_MAX_PEERS] = {};
@@ -291,6 +299,7 @@ static cudaError_t launch_sp2_range(rfoe_handle_s* h, const CUtensorMap& tm, con
 }
 
 static int ensure_tail_ws(rfoe_handle_s* h, int n_tiles, const TailPlan& plan);
+static int ensure_ws(rfoe_handle_s* h, size_t bytes);
 
 extern "C" const char* rfoe_strerror(int status)
 {
@@ -320,6 +329,7 @@ extern "C" int rfoe_destroy(rfoe_handle_t h)
     for (double* p : h->rows) cudaFree(p);
     cudaFree(h->d_bounds); cudaFree(h->d_scalars); cudaFree(h->d_flag); cudaFree(h->d_ctrl); cudaFree(h->d_tiles);
     cudaFree(h->d_pairs);
+    cudaFree(h->d_split); cudaFree(h->d_rec[0]); cudaFree(h->d_rec[1]); cudaFree(h->d_flags); cudaFree(h->d_timing);
     cudaFree(h->stage_H); cudaFree(h->stage_P); cudaFree(h->ws); cudaFree(h->lz_vec); cudaFree(h->lz_state);
     cudaFree(h->sh_send); cudaFree(h->sh_recv); cudaFree(h->sh_parts);
     for (int i = 0; i < h->n_ipc_opened; ++i) cudaIpcCloseMemHandle(h->ipc_opened[i]);
@@ -365,6 +375,14 @@ extern "C" int rfoe_create(rfoe_handle_t* out, int device, int64_t k_max)
     ok = ok && cudaMalloc(&h->d_ctrl, sizeof(Ctrl)) == cudaSuccess;
     ok = ok && cudaMalloc(&h->d_tiles, nt * sizeof(int2)) == cudaSuccess;
     ok = ok && cudaMalloc(&h->d_pairs, nt * sizeof(int2)) == cudaSuccess;
+    {
+        const size_t mr = (size_t)RS_MAX_N / SQ_BM, nrec = mr * (mr + 1) / 2 + (size_t)RS_BANDS * RS_MAX_SPLIT;
+        ok = ok && cudaMalloc(&h->d_split, RS_MAX_SPLIT * sizeof(int2)) == cudaSuccess;
+        ok = ok && cudaMalloc(&h->d_rec[0], nrec * SQ_NPART * sizeof(double)) == cudaSuccess;
+        ok = ok && cudaMalloc(&h->d_rec[1], nrec * SQ_NPART * sizeof(double)) == cudaSuccess;
+        ok = ok && cudaMalloc(&h->d_flags, 256 * sizeof(unsigned)) == cudaSuccess;
+        ok = ok && cudaMalloc(&h->d_timing, 2 * sizeof(unsigned long long)) == cudaSuccess;
+    }
     ok = ok && cudaHostAlloc((void**)&h->hp, sizeof(HostPage), cudaHostAllocMapped) == cudaSuccess;
     ok = ok && cudaHostGetDevicePointer((void**)&h->d_word, (void*)&h->hp->word, 0) == cudaSuccess;
     ok = ok && cudaEventCreate(&h->ev0) == cudaSuccess && cudaEventCreate(&h->ev1) == cudaSuccess;
@@ -381,10 +399,19 @@ extern "C" int rfoe_create(rfoe_handle_t* out, int device, int64_t k_max)
         cudaFuncSetAttribute(sym_square_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, SQ_SMEM_BYTES) != cudaSuccess ||
         cudaFuncSetAttribute(sym_square_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, SQ_SMEM_BYTES) != cudaSuccess ||
         cudaFuncSetAttribute(sym_square_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, SQ_SMEM_BYTES) != cudaSuccess ||
+        cudaFuncSetAttribute(resident_recursion_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, RS_SMEM_BYTES) != cudaSuccess ||
         cudaFuncSetAttribute(apply_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, AP_SMEM_BYTES) != cudaSuccess ||
         cudaFuncSetAttribute(sym_square_reduced_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TQ_SMEM_BYTES) != cudaSuccess) {
         rfoe_destroy(h);
         return RFOE_ERR_CUDA;
+    }
+    {
+        int coop = 0, per_sm = 0;
+        if (cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, device) == cudaSuccess && coop &&
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, resident_recursion_kernel, SQ_THREADS, RS_SMEM_BYTES) == cudaSuccess &&
+            per_sm >= 1 && h->sm_count <= 256)
+            h->coop_ok = 1;
+        cudaGetLastError();
     }
     *out = h;
     return RFOE_OK;
@@ -592,6 +619,31 @@ extern "C" int rfoe_shard_range(int64_t n_tiles, int rank, int world, int64_t* b
     return RFOE_OK;
 }
 
+// Plan of the persistent recursion (resident.cuh): G CTAs share the n_tiles x KT chunk units of a step evenly; a tile
+// not wholly inside one CTA's range [b U / G, (b+1) U / G) is "split" and finished in the FIX phase.
+static int ensure_resident_plan(rfoe_handle_s* h, int m, int KT, cudaStream_t st)
+{
+    const long long U = (long long)h->n_tiles * KT;
+    const int G = (int)(U < h->sm_count ? U : h->sm_count);
+    if (h->rs_m == m && h->rs_G == G) return RFOE_OK;
+    std::vector<int2> split;
+    int b = 0;
+    for (int t = 0; t < h->n_tiles; ++t) {
+        const long long t0 = (long long)t * KT, t1 = t0 + KT;
+        while ((long long)(b + 1) * U / G <= t0) ++b;          // b: the CTA whose range holds unit t0
+        if ((long long)(b + 1) * U / G < t1) split.push_back(make_int2(t, b));
+    }
+    if ((int)split.size() > RS_MAX_SPLIT) return RFOE_ERR_UNSUPPORTED;
+    h->rs_m = 0;
+    if (!split.empty()) CK(cudaMemcpyAsync(h->d_split, split.data(), split.size() * sizeof(int2), cudaMemcpyHostToDevice, st));
+    const size_t nrec = (size_t)h->n_tiles + (size_t)RS_BANDS * split.size();
+    CK(cudaMemsetAsync(h->d_rec[0], 0, nrec * SQ_NPART * sizeof(double), st));   // the tile records of split tiles stay zero
+    CK(cudaMemsetAsync(h->d_rec[1], 0, nrec * SQ_NPART * sizeof(double), st));
+    CK(cudaStreamSynchronize(st));   // `split` is pageable and dies here
+    h->rs_m = m; h->rs_G = G; h->rs_n_split = (int)split.size();
+    return RFOE_OK;
+}
+
 static int expand_impl(rfoe_handle_t h, const double* Hp, int64_t k64, int64_t nocc, int variant, double tol, double* P,
                        rfoe_stream_t stream, const ShardCtx* sh)
 {
@@ -674,8 +726,16 @@ static int expand_impl(rfoe_handle_t h, const double* Hp, int64_t k64, int64_t n
         for (int i = 0; i < 2; ++i)
             if ((rc = make_map_parts(h, &tmF[i], h->F[i], n, n + TQ_PAD)) != RFOE_OK) return fail(rc);
 
+    // the whole recursion in one persistent launch when the problem is small enough to live on chip (resident.cuh)
+    const bool use_resident = h->resident && h->coop_ok && !sh && n <= RS_MAX_N &&
+                              (variant == RFOE_VARIANT_SP2 || variant == RFOE_VARIANT_SP2_ACCEL || variant == RFOE_VARIANT_TRUNC);
+    if (use_resident) {
+        if ((rc = ensure_resident_plan(h, m, n / SQ_BK, st)) != RFOE_OK) return fail(rc);
+        if ((rc = ensure_ws(h, (size_t)2 * h->rs_G * RS_TILE_ELEMS * sizeof(double))) != RFOE_OK) return fail(rc);
+    }
+
     CK(cudaEventRecord(h->ev0, st));
-    // --- symmetry check, bounds, affine map, first decision -------------------------------------
+    // --- symmetry check, bounds, affine map, first decision: enqueued back to back, validity settled on the device ----
     h->hp->sym_flag = 0;
     if (h->check_sym) {
         CK(cudaMemsetAsync(h->d_flag, 0, sizeof(int), st));
@@ -697,15 +757,6 @@ static int expand_impl(rfoe_handle_t h, const double* Hp, int64_t k64, int64_t n
             return fail(rc);
         CK(cudaMemcpyAsync((void*)h->hp->bounds, h->d_bounds, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
     }
-    // the check of the bounds needs them on the host before X0 is trusted: one sync (also covers sym_flag)
-    CK(cudaStreamSynchronize(st));
-    if (h->check_sym && h->hp->sym_flag) return fail(RFOE_ERR_NOT_SYMMETRIC);
-    const double emin = h->hp->bounds[0], emax = h->hp->bounds[1];
-    S.eps_min = emin; S.eps_max = emax;
-    if (!(isfinite(emin) && isfinite(emax) && emax > emin)) return fail(RFOE_ERR_BAD_BOUNDS);
-    // A-Z-RFOE: estimates outside the bounds would put the scaling factors 2/(2 - beta), 2/(1 + bbar) outside (0, 2)
-    if (variant == RFOE_VARIANT_SP2_ACCEL && !(emin <= h->homo && h->lumo <= emax)) return fail(RFOE_ERR_INVALID_ARG);
-
     Ctrl& C = h->hp->ctrl;
     memset(&C, 0, sizeof(Ctrl));
     C.variant = variant; C.stop_rule = h->stop_rule; C.max_iter = is_trunc ? h->trunc_steps : h->max_iter; C.kvalid = k;
@@ -713,27 +764,82 @@ static int expand_impl(rfoe_handle_t h, const double* Hp, int64_t k64, int64_t n
     C.mixed_head = h->mixed_head; C.mixed_reltr = h->mixed_reltr;
     C.mixed_phase = is_mixed ? (h->mixed_head > 0.0 ? 0 : 1) : 2;
     C.reltr_prev = INFINITY;
-    C.emin = emin; C.emax = emax;
-    if (variant == RFOE_VARIANT_SP2_ACCEL) {
-        C.homo = h->homo; C.lumo = h->lumo;
-        C.beta = (emax - h->lumo) / (emax - emin);
-        C.bbar = (emax - h->homo) / (emax - emin);
-    }
+    if (variant == RFOE_VARIANT_SP2_ACCEL) { C.homo = h->homo; C.lumo = h->lumo; }   // images beta / bbar: control_begin
     CK(cudaMemcpyAsync(h->d_ctrl, &C, sizeof(Ctrl), cudaMemcpyHostToDevice, st));
 
     affine_map_kernel<<<hbm_grid(h, n), HBM_THREADS, 0, st>>>(Hp, k, n, ld, h->d_bounds, h->W[0], h->rows[0], h->rows[1]);
     h->launches++;
     CK(cudaGetLastError());
     h->hp->word = -1;
-    control_kernel<<<1, 256, 0, st>>>(h->d_ctrl, 0, h->rows[0], h->rows[1], k, h->d_word);
+    control_kernel<<<1, 256, 0, st>>>(h->d_ctrl, 0, h->rows[0], h->rows[1], k, h->d_word, h->d_bounds);   // stops by itself on bad bounds
     h->launches++;
     CK(cudaGetLastError());
+    // what the host makes of the prologue's results, once they are here (both paths)
+    auto check_prologue = [&]() -> int {
+        if (h->check_sym && h->hp->sym_flag) return RFOE_ERR_NOT_SYMMETRIC;
+        const double emin = h->hp->bounds[0], emax = h->hp->bounds[1];
+        S.eps_min = emin; S.eps_max = emax;
+        if (!(isfinite(emin) && isfinite(emax) && emax > emin)) return RFOE_ERR_BAD_BOUNDS;
+        // A-Z-RFOE: estimates outside the bounds would put the scaling factors 2/(2 - beta), 2/(1 + bbar) outside (0, 2)
+        if (variant == RFOE_VARIANT_SP2_ACCEL && !(emin <= h->homo && h->lumo <= emax)) return RFOE_ERR_INVALID_ARG;
+        return RFOE_OK;
+    };
+    h->sq_n = 0;
+    int cur = 0;
+
+    if (use_resident) {
+        // --- the recursion without the host: one cooperative launch runs every step, the output pass picks the buffer by
+        //     the parity of the device's step counter, and the host synchronises once, at the end
+        ResidentPlan rp = {};
+        rp.n = n; rp.ld = ld; rp.kvalid = k; rp.KT = n / SQ_BK;
+        rp.n_tiles = h->n_tiles; rp.n_split = h->rs_n_split; rp.G = h->rs_G;
+        rp.U = (long long)h->n_tiles * rp.KT;
+        rp.tile_map = h->d_tiles; rp.split = h->d_split;
+        rp.W0 = h->W[0]; rp.W1 = h->W[1]; rp.ws = h->ws;
+        rp.rec0 = h->d_rec[0]; rp.rec1 = h->d_rec[1];
+        rp.flags = h->d_flags; rp.ctrl = h->d_ctrl; rp.timing = h->d_timing;
+        CK(cudaMemsetAsync(h->d_flags, 0, 256 * sizeof(unsigned), st));
+        CK(cudaMemsetAsync(h->d_timing, 0, 2 * sizeof(unsigned long long), st));
+        void* args[3] = {(void*)&tm[0], (void*)&tm[1], (void*)&rp};
+        CK(cudaLaunchCooperativeKernel((const void*)resident_recursion_kernel, dim3(h->rs_G), dim3(SQ_THREADS), args, RS_SMEM_BYTES, st));
+        h->launches++;
+        copy_out_select_kernel<<<hbm_grid(h, k), HBM_THREADS, 0, st>>>(h->W[0], h->W[1], &h->d_ctrl->step, k, ld, Hp, P, h->rows[0]);
+        h->launches++;
+        CK(cudaGetLastError());
+        sum_rows_kernel<<<1, 256, 0, st>>>(h->rows[0], k, &h->d_ctrl->tr_PH);
+        h->launches++;
+        CK(cudaGetLastError());
+        CK(cudaEventRecord(h->ev1, st));
+        CK(cudaMemcpyAsync(&C, h->d_ctrl, sizeof(Ctrl), cudaMemcpyDeviceToHost, st));
+        CK(cudaMemcpyAsync((void*)h->hp->scalars, h->d_timing, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+        if ((rc = check_prologue()) != RFOE_OK) return fail(rc);
+        float ms = 0.f;
+        CK(cudaEventElapsedTime(&ms, h->ev0, h->ev1));
+        unsigned long long step_ns = 0;
+        memcpy(&step_ns, (const void*)h->hp->scalars, sizeof(step_ns));
+        S.iterations = C.step; S.multiplications = C.multiplications; S.mcweeny_steps = C.mcweeny_steps;
+        S.fp32_steps = C.fp32_steps; S.converged = C.converged; S.tr_PH = C.tr_PH; S.device_ms = ms;
+        S.gpu_launches = h->launches;
+        S.square_launches = C.step;                  // squarings, all inside the one launch
+        S.square_ms = (double)step_ns * 1e-6;        // CTA 0's %globaltimer around the steps
+        S.resident = 1;
+        const int ns = C.step;
+        memcpy(S.t, C.ht, sizeof(double) * (ns + 1));
+        memcpy(S.s, C.hs, sizeof(double) * (ns + 1));
+        memcpy(S.e, C.he, sizeof(double) * ns);
+        memcpy(S.reltr, C.hreltr, sizeof(double) * ns);
+        memcpy(S.branch, C.branch, ns);
+        S.branch[ns] = 0;
+        S.status = C.converged ? RFOE_OK : RFOE_ERR_NOT_CONVERGED;
+        return S.status;
+    }
+
     CK(cudaStreamSynchronize(st));
+    if ((rc = check_prologue()) != RFOE_OK) return fail(rc);
 
     // --- the recursion: one scalar (the action word) crosses to the host per step ----------------
-    int cur = 0;
     int action = h->hp->word;
-    h->sq_n = 0;
     while (action != ACT_STOP) {
         const int nxt = cur ^ 1;
         if (action == ACT_SP2 && sh && sh->barrier) {
@@ -747,7 +853,7 @@ static int expand_impl(rfoe_handle_t h, const double* Hp, int64_t k64, int64_t n
                 h->sq_n++;
             }
             if (sh->barrier(sh->user, stream) != 0) return fail(RFOE_ERR_CUDA);
-            control_kernel<<<1, 256, 0, st>>>(h->d_ctrl, 1, h->part[nxt], h->part[nxt], h->n_tiles, h->d_word);
+            control_kernel<<<1, 256, 0, st>>>(h->d_ctrl, 1, h->part[nxt], h->part[nxt], h->n_tiles, h->d_word, nullptr);
         } else if (action == ACT_SP2 && sh) {
             // this rank's tiles (and their mirrors) -> W[nxt]; pack them with their records; ONE all-gather; unpack
             // the foreign tiles; the records, now in global tile order, feed the same control kernel on every rank
@@ -767,23 +873,23 @@ static int expand_impl(rfoe_handle_t h, const double* Hp, int64_t k64, int64_t n
                                                            h->sh_parts);
             h->launches++;
             CK(cudaGetLastError());
-            control_kernel<<<1, 256, 0, st>>>(h->d_ctrl, 1, h->sh_parts, h->sh_parts, h->n_tiles, h->d_word);
+            control_kernel<<<1, 256, 0, st>>>(h->d_ctrl, 1, h->sh_parts, h->sh_parts, h->n_tiles, h->d_word, nullptr);
         } else if (action == ACT_SP2) {
             CK(cudaEventRecord(h->sq_ev[2 * h->sq_n], st));
             CK(launch_sp2_range(h, tm[cur], h->W[cur], h->W[nxt], n, ld, k, &h->d_ctrl->coef, h->part[0], 0, h->n_tiles, plan, st));
             CK(cudaEventRecord(h->sq_ev[2 * h->sq_n + 1], st));
             h->sq_n++;
-            control_kernel<<<1, 256, 0, st>>>(h->d_ctrl, 1, h->part[0], h->part[0], h->n_tiles, h->d_word);
+            control_kernel<<<1, 256, 0, st>>>(h->d_ctrl, 1, h->part[0], h->part[0], h->n_tiles, h->d_word, nullptr);
         } else if (action == ACT_SP2_FP32) {
             CK(cudaEventRecord(h->sq_ev[2 * h->sq_n], st));
             CK(launch_square_reduced(h, tmF[0], tmF[1], h->W[cur], h->W[nxt], n, ld, k, &h->d_ctrl->t, &h->d_ctrl->coef, h->part[0], st));
             CK(cudaEventRecord(h->sq_ev[2 * h->sq_n + 1], st));
             h->sq_n++;
-            control_kernel<<<1, 256, 0, st>>>(h->d_ctrl, 1, h->part[0], h->part[0], 2 * h->n_pairs, h->d_word);
+            control_kernel<<<1, 256, 0, st>>>(h->d_ctrl, 1, h->part[0], h->part[0], 2 * h->n_pairs, h->d_word, nullptr);
         } else if (action == ACT_MCWEENY) {
             CK(timed_square<false>(h, tm[cur], tm[cur], h->W[cur], h->W[2], n, ld, k, &h->d_ctrl->coef, h->part[0], st));
             CK(timed_square<true>(h, tm[2], tm[cur], h->W[2], h->W[nxt], n, ld, k, &h->d_ctrl->coef_aux, h->part[1], st));
-            control_kernel<<<1, 256, 0, st>>>(h->d_ctrl, 1, h->part[1], h->part[0], h->n_tiles, h->d_word);
+            control_kernel<<<1, 256, 0, st>>>(h->d_ctrl, 1, h->part[1], h->part[0], h->n_tiles, h->d_word, nullptr);
         } else {
             return fail(RFOE_ERR_UNSUPPORTED);
         }

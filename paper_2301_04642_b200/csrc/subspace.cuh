@@ -135,10 +135,11 @@ apply_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CU
     if (warp == 0) issue_loads(min(KT, SQ_STAGES));
     // warp 0 (producer and consumer) never blocks on a full-barrier: it polls and keeps issuing (see sym_square.cuh)
     auto wait_full = [&](uint32_t bar, uint32_t parity, int kt_now) {
+        if (mbar_try(bar, parity)) return;          // the common case, the same instructions for every warp
         if (warp == 0) {
-            while (!mbar_test(bar, parity)) issue_loads(min(KT, kt_now + SQ_STAGES));
+            do { issue_loads(min(KT, kt_now + SQ_STAGES)); } while (!mbar_test(bar, parity));
         } else {
-            mbar_wait_safe(bar, parity);
+            mbar_wait_bounded(bar, parity);
         }
     };
 

@@ -128,10 +128,11 @@ sym_square_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     // ever issue that chunk.  So warp 0 polls and keeps issuing; the other warps wait (bounded: a pipeline bug traps
     // instead of hanging the GPU).
     auto wait_full = [&](uint32_t bar, uint32_t parity, int kt_now) {
+        if (mbar_try(bar, parity)) return;          // the common case, the same instructions for every warp
         if (warp == 0) {
-            while (!mbar_test(bar, parity)) issue_loads(min(KT, kt_now + SQ_STAGES));
+            do { issue_loads(min(KT, kt_now + SQ_STAGES)); } while (!mbar_test(bar, parity));
         } else {
-            mbar_wait_safe(bar, parity);
+            mbar_wait_bounded(bar, parity);
         }
     };
     {

@@ -121,7 +121,7 @@ def test_symm_product_parity(handle, k):
 
 
 # ------------------------------------------------------------------ whole expansions
-def _check_expansion(w, res, ref, *, ptol=1e-10, etol=1e-11, inv=1.0):
+def _check_expansion(w, res, ref, *, ptol=1e-10, etol=1e-11, inv=1.0, projector=True):
     k = w.k
     P = res.P.cpu().numpy() if hasattr(res.P, "cpu") else res.P
     assert res.converged == ref.converged
@@ -138,7 +138,7 @@ def _check_expansion(w, res, ref, *, ptol=1e-10, etol=1e-11, inv=1.0):
     assert np.allclose(res.s, ref.s, rtol=0, atol=1e-9 * k / 256)
     assert np.allclose(res.e[: n - 1], ref.e[: n - 1], rtol=1e-6, atol=1e-11 * k / 256)
     # north_star invariants on the GPU result, and the construction-exact projector (pin P2)
-    if ref.converged:
+    if ref.converged and projector:          # (a truncated expansion G_m is delivered, but it is not a projector)
         # (inv loosens them for stop rule B, which stops at RelTr 5e-8 -- before P is converged to rounding)
         assert abs(np.trace(P) - w.nocc) <= 1e-9 * inv
         assert np.linalg.norm(P @ P - P) <= 1e-10 * k / 256 * inv
@@ -195,7 +195,7 @@ def test_expand_bounds_override_and_truncated(handle):
         ref = oracle.expand(w.H, w.nocc, variant=oracle.TRUNC, max_iter=7, bounds_override=(lo, hi))
         res2 = handle.expand(_dev(w.H), w.nocc, rfoe.TRUNC, 0.0)
         assert res2.status == rfoe.OK and res2.converged and res2.iterations == 7 and res2.trunc_steps == 7
-        _check_expansion(w, res2, ref)
+        _check_expansion(w, res2, ref, projector=False)
         assert torch.equal(res2.P, res.P)
     finally:
         handle.configure(bounds=False, max_iter=100, trunc_steps=30)

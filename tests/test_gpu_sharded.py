@@ -74,6 +74,7 @@ def test_sharded_equals_single_gpu_bitwise(c, k, g):
     w = rfoe_inputs.make_workload(c, k=k)
     H = torch.from_numpy(w.H).cuda()
     with rfoe.Rfoe(k) as h:
+        h.configure(resident=False)      # the sharded run reproduces the bits of the launch-per-step path (same tiles, same order)
         one = h.expand(H, w.nocc, rfoe.SP2, w.tol)
     ref = oracle.expand(w.H, w.nocc, tol=w.tol)
     assert one.iterations == ref.iterations
@@ -91,13 +92,13 @@ def test_sharded_world1_and_accelerated_and_truncated():
     H = torch.from_numpy(w.H).cuda()
     homo, lumo = float(w.lam[: w.nocc].max()), float(w.lam[w.nocc:].min())
     with rfoe.Rfoe(333) as h:
-        h.configure(homo=homo, lumo=lumo)
+        h.configure(homo=homo, lumo=lumo, resident=False)
         one = h.expand(H, w.nocc, rfoe.SP2_ACCEL, w.tol)
     assert torch.equal(_run_sharded(H, w.nocc, rfoe.SP2_ACCEL, w.tol, 1, dict(homo=homo, lumo=lumo))[0].P, one.P)
     for r in _run_sharded(H, w.nocc, rfoe.SP2_ACCEL, w.tol, 2, dict(homo=homo, lumo=lumo)):
         assert r.iterations == one.iterations and torch.equal(r.P, one.P)
     with rfoe.Rfoe(333) as h:                                              # T-RFOE: m = 12 steps, no stop test
-        h.configure(max_iter=12)
+        h.configure(max_iter=12, resident=False)
         trunc = h.expand(H, w.nocc, rfoe.SP2, 0.0)
     for r in _run_sharded(H, w.nocc, rfoe.SP2, 0.0, 3, dict(max_iter=12)):
         assert r.iterations == 12 and not r.converged and torch.equal(r.P, trunc.P)
@@ -160,6 +161,7 @@ def test_p2p_sharded_equals_single_gpu_bitwise(c, k, g):
     w = rfoe_inputs.make_workload(c, k=k)
     H = torch.from_numpy(w.H).cuda()
     with rfoe.Rfoe(k) as h:
+        h.configure(resident=False)
         one = h.expand(H, w.nocc, rfoe.SP2, w.tol)
     for r in _run_p2p_threads(H, w.nocc, rfoe.SP2, w.tol, g):
         assert r.converged and r.iterations == one.iterations and r.branch == one.branch
@@ -182,6 +184,7 @@ def _ipc_worker(rank, world, port, k, c, out):
         torch.cuda.synchronize()
         dist.barrier()
         if rank == 0:
+            h.configure(resident=False)
             one = h.expand(H, w.nocc, rfoe.SP2, w.tol)
             out["single"] = (one.iterations, one.branch)
             out["equal"] = bool(torch.equal(one.P, res.P))
