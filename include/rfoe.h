@@ -105,7 +105,10 @@ typedef struct {
     double eps_min, eps_max; /* the bounds used for X_0 */
     double tr_PH;            /* sum_ij P_ij H^p_ij (band energy) */
     double device_ms;        /* CUDA-event time of the last rfoe_expand on its stream */
-    double square_ms;        /* CUDA-event time summed over its squaring / product kernel launches */
+    double square_ms;        /* CUDA-event time summed over its squaring / product kernel launches (persistent launch: the
+                                steps as timed by CTA 0 with %globaltimer) */
+    double resident_phase_ms[5]; /* persistent launch only, CTA 0's share of the steps: products, first grid barrier (the wait
+                                for the slowest SM included), finishing of split tiles, second barrier, reductions + decision */
     double t[RFOE_MAX_STEPS + 1];   /* t[n] = Tr X_n */
     double s[RFOE_MAX_STEPS + 1];   /* s[n] = ||X_n||_F^2 = Tr X_n^2 */
     double e[RFOE_MAX_STEPS];       /* e[n] = ||X_n^2 - X_n||_F (idempotency error of the step's input) */

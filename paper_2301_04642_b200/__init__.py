@@ -62,7 +62,7 @@ class _Stats(C.Structure):
         ("trunc_steps", C.c_int32), ("resident", C.c_int32),
         ("k", C.c_int64), ("nocc", C.c_int64), ("gpu_launches", C.c_int64),
         ("tol", C.c_double), ("eps_min", C.c_double), ("eps_max", C.c_double), ("tr_PH", C.c_double),
-        ("device_ms", C.c_double), ("square_ms", C.c_double),
+        ("device_ms", C.c_double), ("square_ms", C.c_double), ("resident_phase_ms", C.c_double * 5),
         ("t", C.c_double * (MAX_STEPS + 1)), ("s", C.c_double * (MAX_STEPS + 1)),
         ("e", C.c_double * MAX_STEPS), ("reltr", C.c_double * MAX_STEPS),
         ("branch", C.c_char * (MAX_STEPS + 8)),
@@ -139,6 +139,7 @@ class ExpandResult:
     gpu_launches: int
     trunc_steps: int
     resident: bool
+    resident_phase_ms: tuple
     t: np.ndarray
     s: np.ndarray
     e: np.ndarray
@@ -175,7 +176,7 @@ def _result_from(st: _Stats, P, rc) -> "ExpandResult":
         mcweeny_steps=st.mcweeny_steps, fp32_steps=st.fp32_steps, branch=st.branch.decode()[:n],
         eps_min=st.eps_min, eps_max=st.eps_max, tr_PH=st.tr_PH, device_ms=st.device_ms, square_ms=st.square_ms,
         square_launches=st.square_launches, gpu_launches=st.gpu_launches, trunc_steps=st.trunc_steps,
-        resident=bool(st.resident), t=np.array(st.t[: n + 1]),
+        resident=bool(st.resident), resident_phase_ms=tuple(st.resident_phase_ms), t=np.array(st.t[: n + 1]),
         s=np.array(st.s[: n + 1]), e=np.array(st.e[:n]), reltr=np.array(st.reltr[:n]))
 
 

@@ -1,25 +1,28 @@
 // The whole recursion in ONE persistent launch (rows A3-A6 of DESIGN.md for H^p small enough to stay on chip).
 //
-// A recursion step of a small problem is short -- k=256: 2.5e7 flops, a microsecond of tensor work; k=2048: 250 us --
-// so the launch-per-step path spends its time elsewhere: a host round trip per step (the one scalar of A3), two kernel
-// boundaries, and, for k=2048, 136 tiles on 148 SMs.  Here a cooperative grid of G <= 148 CTAs (one per SM) stays
-// resident for the whole expansion and runs, per step:
+// A recursion step of a small problem is short -- k=2048: 250 us of tensor work, k=1024: 30 us -- so the launch-per-step
+// path spends its time elsewhere: a host round trip per step (the one scalar of A3), two kernel boundaries, and, at
+// k=2048, 136 equal tiles on 148 SMs (one wave, 12 SMs idle).  Here a cooperative grid of G <= 148 CTAs (one per SM)
+// stays resident for the whole expansion and runs, per step:
 //   MM   the step's work is the stream of U = n_tiles x KT "chunk units" (tile, 16-wide slice of the contraction) in
-//        tile order; CTA b takes the contiguous range [b U / G, (b+1) U / G) -- every SM gets the same number of DMMAs
-//        (stream-K).  Units arrive by TMA through the same 6-stage mbarrier ring as sym_square_kernel, which keeps
-//        running across tile boundaries, so there is no pipeline refill between segments.  A tile that lies wholly in
-//        one range gets the fused epilogue of sym_square.cuh straight from registers; the two (at most) partial
-//        segments at the ends of a range go to a workspace as raw accumulators.
-//   --   grid barrier (one flag per CTA, release / acquire, no atomics)
-//   FIX  every split tile is finished in 8 bands of 16 rows spread over all CTAs: its segments are added in ascending
-//        order of the contraction index (fixed order: reproducible bits), then exactly the fused epilogue -- update
-//        c2 C + c1 X + c0 I, mirror (through shared memory, 128-byte runs), the five partial sums.
+//        tile order; CTA b takes a contiguous range of it, all ranges costing the same (stream-K; where a CTA holds
+//        several whole tiles their register epilogues are counted in, as epi_cost units each).  Units arrive by TMA
+//        through the same 6-stage mbarrier ring as sym_square_kernel, which keeps running across tile boundaries: no
+//        pipeline refill between segments.  A tile that lies wholly in one range gets the fused epilogue of
+//        sym_square.cuh straight from registers; the (at most two) partial segments at the ends of a range go to a
+//        workspace as raw accumulators.
+//   --   grid barrier (a flag per CTA, release / acquire, no atomics)
+//   FIX  every split tile is finished in 8 bands of 16 rows, ONE WARP per band, spread over all warps of all CTAs (no
+//        block-level synchronisation, so the L2 round trips of the 8 warps of an SM overlap): its segments are added in
+//        ascending order of the contraction index (fixed order: reproducible bits), then exactly the fused epilogue --
+//        update c2 C + c1 X + c0 I, mirror (through the warp's patch of shared memory: 128-byte runs both ways), the five
+//        partial sums, gathered into one record per CTA.
 //   --   grid barrier
 //   CTL  EVERY CTA sums all records in the same fixed order and takes the step's decision (control_update) on its own
-//        shared-memory copy of the control block: identical inputs, identical code, identical decisions, so there is
-//        no broadcast and no third barrier.  CTA 0 writes the history back at the end.
-// The host is not in the loop at all: it enqueues bounds, affine map, first decision, this kernel and the output pass
-// and synchronises once.  Cross-CTA data (X_n written by other SMs, raw segments, records) is read through L2
+//        shared-memory copy of the control block: identical inputs, identical code, identical decisions -- no broadcast,
+//        no third barrier.  CTA 0 writes the history back at the end.
+// The host is not in the loop: it enqueues bounds, affine map, first decision, this kernel and the output pass, and
+// synchronises once.  Cross-CTA data (X_n written by other SMs, raw segments, records) is read through L2
 // (ld.global.cg / TMA), never through L1, and both sides of every barrier carry a fence.proxy.async because TMA reads
 // what ordinary stores wrote.
 #pragma once
@@ -34,33 +37,26 @@ constexpr int RS_BAND_ROWS = SQ_BM / RS_BANDS;       // 16
 constexpr int RS_TILE_ELEMS = SQ_BM * SQ_BM;
 constexpr int RS_MAX_SPLIT = 1024;
 constexpr int RS_SMEM_BYTES = SQ_SMEM_BYTES;
+constexpr int RS_EPI_COST = 10;                      // a register epilogue in chunk units (~39k cycles / 4096 per chunk)
+constexpr int RS_TW_PITCH = 129;                     // row pitch (doubles) of a warp's 16 x 128 transposition patch
 
 struct ResidentPlan {
     int n, ld, kvalid, KT;        // padded size, row pitch, true size, chunks per tile (n / 16)
-    int n_tiles, n_split, G, pad_;
-    long long U;                  // n_tiles * KT chunk units per step
+    int n_tiles, n_split, G, tile_cost;   // tile_cost = KT + epi_cost (epi_cost = 0 when nearly every tile is split)
+    long long cost_total;         // n_tiles * tile_cost
     const int2* tile_map;         // (I, J) of every upper-triangle tile, the usual order
-    const int2* split;            // per split tile: (tile, first CTA that holds a segment of it)
+    const int4* split;            // per split tile: (tile, first CTA holding a segment of it, number of segments, 0)
     double* W0;                   // the two work matrices (ping-pong by step parity)
     double* W1;
     double* ws;                   // 2 G slots of 128 x 128 raw accumulators (slot 2b: segment that continues a tile, 2b+1: that starts one)
-    double* rec0;                 // records of even / odd steps: n_tiles tile records (split tiles' stay zero) + 8 per split tile
+    double* rec0;                 // records of even / odd steps: n_tiles tile records (split tiles' stay zero) + one per CTA (its FIX bands)
     double* rec1;
     unsigned* flags;              // G grid-barrier flags, zero at launch
     Ctrl* ctrl;
-    unsigned long long* timing;   // [0]: ns CTA 0 spent in the steps (MM + FIX + CTL), for rfoe_stats_t.square_ms
+    unsigned long long* timing;   // CTA 0's %globaltimer, ns: [0] all steps (rfoe_stats_t.square_ms), [1] MM, [2] first barrier, [3] FIX,
+                                  // [4] second barrier, [5] CTL
 };
 
-__device__ __forceinline__ unsigned ld_acquire_gpu_u32(const unsigned* p)
-{
-    unsigned v;
-    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-    return v;
-}
-__device__ __forceinline__ void st_release_gpu_u32(unsigned* p, unsigned v)
-{
-    asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
-}
 __device__ __forceinline__ void fence_proxy_async_all() { asm volatile("fence.proxy.async;" ::: "memory"); }
 __device__ __forceinline__ unsigned long long globaltimer_ns()
 {
@@ -69,132 +65,188 @@ __device__ __forceinline__ unsigned long long globaltimer_ns()
     return t;
 }
 
+__device__ __forceinline__ unsigned ld_volatile_u32(const unsigned* p)
+{
+    unsigned v;
+    asm volatile("ld.volatile.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_volatile_u32(unsigned* p, unsigned v)
+{
+    asm volatile("st.volatile.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
 // All CTAs of the (cooperative, co-resident) grid: everything written before is visible to everybody after.
+// The pattern of cooperative-groups' grid sync with flags instead of an atomic counter: the block barrier orders every
+// thread's writes before thread 0's fence + flag store (release); pollers spin on plain volatile loads (an acquire load
+// would invalidate the whole L1 on every poll) and fence once when their flag has arrived (acquire); the second block
+// barrier hands that to all threads.  Cross-CTA data is then read through L2 only (ld.global.cg / TMA).
 __device__ __forceinline__ void grid_barrier(unsigned* flags, int G, unsigned& epoch)
 {
     ++epoch;
-    fence_proxy_async_all();      // ordinary stores before later TMA (async proxy) reads of the same data
-    __threadfence();
     __syncthreads();
-    if (threadIdx.x == 0) st_release_gpu_u32(flags + blockIdx.x, epoch);
     if ((int)threadIdx.x < G) {
+        if (threadIdx.x == 0) {
+            fence_proxy_async_all();      // ordinary stores before later TMA (async proxy) reads of the same data
+            __threadfence();
+            st_volatile_u32(flags + blockIdx.x, epoch);
+        }
         const long long t0 = clock64();
-        while ((int)(ld_acquire_gpu_u32(flags + threadIdx.x) - epoch) < 0)
+        while ((int)(ld_volatile_u32(flags + threadIdx.x) - epoch) < 0)
             if (clock64() - t0 > 4000000000LL) __trap();      // a lost CTA must not hang the GPU
+        __threadfence();
     }
     __syncthreads();
     fence_proxy_async_all();
 }
 
-// block_sum_strided (control.cuh) reading through L2: the records were written by other SMs during this launch
-__device__ inline double block_sum_strided_cg(const double* __restrict__ p, int n, int stride, double* sh)
+// first chunk unit of CTA b's range (b = G: the end of the stream).  Ranges are equal in COST: chunk units plus
+// epi_cost units per tile epilogue, which sits at the tile's end and is never cut.  (rfoe.cu has the host twin.)
+__device__ __forceinline__ int rs_boundary(const ResidentPlan& p, int b)
 {
-    double v = 0.0;
-    for (int i = threadIdx.x; i < n; i += blockDim.x) v += __ldcg(p + (size_t)i * stride);
-    sh[threadIdx.x] = v;
-    __syncthreads();
-    for (int m = blockDim.x >> 1; m >= 1; m >>= 1) {
-        if ((int)threadIdx.x < m) sh[threadIdx.x] += sh[threadIdx.x + m];
-        __syncthreads();
-    }
-    const double r = sh[0];
-    __syncthreads();
-    return r;
+    const long long c = (long long)b * p.cost_total / p.G;
+    const int tile = (int)(c / p.tile_cost);
+    const int off = (int)(c - (long long)tile * p.tile_cost);
+    return tile * p.KT + min(off, p.KT);
 }
 
-// FIX phase, one band (16 rows) of one split tile: segments added in ascending order, then the fused epilogue.
-// tsm: 16 x 129 doubles of shared memory (the idle operand ring); red: 8 x 5 doubles.
-__device__ __forceinline__ void resident_fixup_band(const ResidentPlan& p, int q, int G, const double* __restrict__ E,
-                                                    double* __restrict__ Out, double* __restrict__ rec, double c2, double c1,
-                                                    double c0, double* tsm, double (*red)[5])
+// three fixed-order sums over the tile records in one pass (Tr X_{n+1}, ||X_{n+1}||_F^2, ||X_n^2 - X_n||_F^2): per thread
+// strided, then a shuffle tree per warp, then the warps in order.  Reads through L2 (written by other SMs this launch).
+__device__ inline void record_sums_cg(const double* __restrict__ rec, int n_rec, double (*sh)[3], double& t1, double& s1, double& e2)
 {
-    const int j = q / RS_BANDS, band = q % RS_BANDS;
-    const int2 sp = p.split[j];
-    const int tile = sp.x;
-    const int2 ij = p.tile_map[tile];
-    const int I = ij.x, J = ij.y;
-    const bool diag = (I == J);
-    const int t = threadIdx.x, warp = t >> 5, lane = t & 31;
-    const int rl = t >> 4;                     // row inside the band
-    const int r = band * RS_BAND_ROWS + rl;    // row inside the tile
-    const int cl = (t & 15) * 8;               // first of this thread's 8 columns
-    const int row = I * SQ_BM + r, col = J * SQ_BM + cl;
-    const int ld = p.ld;
+    double a = 0.0, c = 0.0, e = 0.0;
+    for (int i = threadIdx.x; i < n_rec; i += SQ_THREADS) {
+        const double2 x = __ldcg(reinterpret_cast<const double2*>(rec + (size_t)i * SQ_NPART));
+        const double y = __ldcg(rec + (size_t)i * SQ_NPART + 2);
+        a += x.x; c += x.y; e += y;
+    }
+#pragma unroll
+    for (int m = 16; m >= 1; m >>= 1) {
+        a += __shfl_xor_sync(0xffffffffu, a, m);
+        c += __shfl_xor_sync(0xffffffffu, c, m);
+        e += __shfl_xor_sync(0xffffffffu, e, m);
+    }
+    if ((threadIdx.x & 31) == 0) { sh[threadIdx.x >> 5][0] = a; sh[threadIdx.x >> 5][1] = c; sh[threadIdx.x >> 5][2] = e; }
+    __syncthreads();
+    t1 = s1 = e2 = 0.0;
+#pragma unroll
+    for (int w = 0; w < SQ_CONSUMER_WARPS; ++w) { t1 += sh[w][0]; s1 += sh[w][1]; e2 += sh[w][2]; }
+    __syncthreads();
+}
 
-    double cv[8];
-#pragma unroll
-    for (int u = 0; u < 8; ++u) cv[u] = 0.0;
-    const long long t0u = (long long)tile * p.KT, t1u = t0u + p.KT;
-    for (int bb = sp.y;; ++bb) {
-        const long long rb = (long long)bb * p.U / G, rb1 = (long long)(bb + 1) * p.U / G;
-        const int slot = (rb > t0u) ? 2 * bb : 2 * bb + 1;
-        const double2* src = reinterpret_cast<const double2*>(p.ws + (size_t)slot * RS_TILE_ELEMS + r * SQ_BM + cl);
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            const double2 x = __ldcg(src + i);
-            cv[2 * i] += x.x;
-            cv[2 * i + 1] += x.y;
-        }
-        if (rb1 >= t1u) break;
-    }
-    double ev[8];
-    {
-        const double2* e2p = reinterpret_cast<const double2*>(E + (size_t)row * ld + col);
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            const double2 x = __ldcg(e2p + i);
-            ev[2 * i] = x.x;
-            ev[2 * i + 1] = x.y;
-        }
-    }
+// FIX phase, one band (16 rows) of one split tile, by ONE WARP: segments added in ascending order, then the fused
+// epilogue.  tw: the warp's 16 x RS_TW_PITCH doubles of shared memory (the operand ring is idle in this phase).
+// wsum[5]: the warp's running partial sums of this step in shared memory (Tr Out, ||Out||^2, ||C - X||^2, Tr C, <C, X>).
+// Everything arrives BY VALUE (registers): a reference to the kernel's __grid_constant__ plan would turn every field into
+// a dependent generic load in this out-of-line function (measured: ~12 us of a 23 us phase).
+// meta = (b0 = first CTA holding a segment, nseg, I, J) of the band's tile.
+__device__ __noinline__ void resident_fixup_band(int4 meta, int band, const double* __restrict__ ws, int ld, int kvalid,
+                                                 const double* __restrict__ E, double* __restrict__ Out, double c2, double c1,
+                                                 double c0, double* tw, double* wsum)
+{
+    const int b0 = meta.x, nseg = meta.y;
+    const int I = meta.z, J = meta.w;
+    const bool diag = (I == J);
+    const int lane = threadIdx.x & 31;
+    const int cl = 4 * lane;                                   // this lane's 4 columns of the tile
+    const int col = J * SQ_BM + cl;
+    constexpr int RB = 4;                                      // rows per batch: 8 (nseg + 1) 16-byte loads in flight per lane
     double p_tr = 0.0, p_ss = 0.0, p_err = 0.0, p_trc = 0.0, p_ce = 0.0;
-    double o[8];
+#pragma unroll 1
+    for (int rb = 0; rb < RS_BAND_ROWS; rb += RB) {
+        double cv[RB][4], ev[RB][4];
+        const int r0 = band * RS_BAND_ROWS + rb;               // first tile row of the batch
 #pragma unroll
-    for (int u = 0; u < 8; ++u) {
-        double v = fma(c2, cv[u], c1 * ev[u]);
-        const double d = cv[u] - ev[u];
-        double w = 1.0;
-        if (diag) {
-            const int cc = col + u;
-            w = (cc > row) ? 2.0 : ((cc == row) ? 1.0 : 0.0);
-            if (cc == row) {
-                if (row < p.kvalid) v += c0;
-                p_tr += v;
-                p_trc += cv[u];
+        for (int i = 0; i < RB; ++i) {
+            const double2* e2p = reinterpret_cast<const double2*>(E + (size_t)(I * SQ_BM + r0 + i) * ld + col);
+            const double2 x = __ldcg(e2p), y = __ldcg(e2p + 1);
+            ev[i][0] = x.x; ev[i][1] = x.y; ev[i][2] = y.x; ev[i][3] = y.y;
+        }
+        {
+            // the first holder's segment starts the tile (slot 2b+1); every later one continues it (slot 2b).  The first two
+            // (a split tile has at least two) are fetched together with X_n: one L2 round trip per batch in the common case.
+            const double* src0 = ws + (size_t)(2 * b0 + 1) * RS_TILE_ELEMS + r0 * SQ_BM + cl;
+            const double* src1 = ws + (size_t)(2 * (b0 + 1)) * RS_TILE_ELEMS + r0 * SQ_BM + cl;
+            double cw[RB][4];
+#pragma unroll
+            for (int i = 0; i < RB; ++i) {
+                const double2 x = __ldcg(reinterpret_cast<const double2*>(src0 + i * SQ_BM));
+                const double2 y = __ldcg(reinterpret_cast<const double2*>(src0 + i * SQ_BM + 2));
+                cv[i][0] = x.x; cv[i][1] = x.y; cv[i][2] = y.x; cv[i][3] = y.y;
+            }
+#pragma unroll
+            for (int i = 0; i < RB; ++i) {
+                const double2 x = __ldcg(reinterpret_cast<const double2*>(src1 + i * SQ_BM));
+                const double2 y = __ldcg(reinterpret_cast<const double2*>(src1 + i * SQ_BM + 2));
+                cw[i][0] = x.x; cw[i][1] = x.y; cw[i][2] = y.x; cw[i][3] = y.y;
+            }
+#pragma unroll
+            for (int i = 0; i < RB; ++i)
+#pragma unroll
+                for (int u = 0; u < 4; ++u) cv[i][u] += cw[i][u];
+        }
+        for (int sg = 2; sg < nseg; ++sg) {
+            const double* src = ws + (size_t)(2 * (b0 + sg)) * RS_TILE_ELEMS + r0 * SQ_BM + cl;
+#pragma unroll
+            for (int i = 0; i < RB; ++i) {
+                const double2 x = __ldcg(reinterpret_cast<const double2*>(src + i * SQ_BM));
+                const double2 y = __ldcg(reinterpret_cast<const double2*>(src + i * SQ_BM + 2));
+                cv[i][0] += x.x; cv[i][1] += x.y; cv[i][2] += y.x; cv[i][3] += y.y;
             }
         }
-        o[u] = v;
-        p_ss = fma(w * v, v, p_ss);
-        p_err = fma(w * d, d, p_err);
-        p_ce = fma(w * cv[u], ev[u], p_ce);
+#pragma unroll
+        for (int i = 0; i < RB; ++i) {
+            const int row = I * SQ_BM + r0 + i;
+            double o[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                double v = fma(c2, cv[i][u], c1 * ev[i][u]);
+                const double d = cv[i][u] - ev[i][u];
+                double w = 1.0;
+                if (diag) {
+                    const int cc = col + u;
+                    w = (cc > row) ? 2.0 : ((cc == row) ? 1.0 : 0.0);
+                    if (cc == row) {
+                        if (row < kvalid) v += c0;
+                        p_tr += v;
+                        p_trc += cv[i][u];
+                    }
+                }
+                o[u] = v;
+                p_ss = fma(w * v, v, p_ss);
+                p_err = fma(w * d, d, p_err);
+                p_ce = fma(w * cv[i][u], ev[i][u], p_ce);
+            }
+            if (!diag) {
+                double2* dst = reinterpret_cast<double2*>(Out + (size_t)row * ld + col);
+                dst[0] = make_double2(o[0], o[1]);
+                dst[1] = make_double2(o[2], o[3]);
+            } else {
+#pragma unroll
+                for (int u = 0; u < 4; ++u)
+                    if (col + u >= row) Out[(size_t)row * ld + col + u] = o[u];
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) tw[(rb + i) * RS_TW_PITCH + cl + u] = o[u];
+        }
     }
-    if (!diag) {
-        double2* dst = reinterpret_cast<double2*>(Out + (size_t)row * ld + col);
+    __syncwarp();
+    // mirror: element (row, col) -> (col, row).  Lane = a column cc of the tile: its 16 band rows are 128 contiguous bytes
+    // of row J*128 + cc of the output.
+#pragma unroll 1
+    for (int cc = lane; cc < SQ_BM; cc += 32) {
+        const int mrow = J * SQ_BM + cc;
+        const int mcol = I * SQ_BM + band * RS_BAND_ROWS;
+        double m[RS_BAND_ROWS];
 #pragma unroll
-        for (int i = 0; i < 4; ++i) dst[i] = make_double2(o[2 * i], o[2 * i + 1]);
-    } else {
-#pragma unroll
-        for (int u = 0; u < 8; ++u)
-            if (col + u >= row) Out[(size_t)row * ld + col + u] = o[u];
-    }
-#pragma unroll
-    for (int u = 0; u < 8; ++u) tsm[rl * 129 + cl + u] = o[u];
-    __syncthreads();
-    {
-        // mirror: element (row, col) -> (col, row); thread = (column cc of the tile, 8 of the band's 16 rows): 64-byte runs
-        const int cc = t >> 1, half = t & 1;
-        const int mrow = J * SQ_BM + cc;                                   // row of the mirrored element
-        const int mcol = I * SQ_BM + band * RS_BAND_ROWS + half * 8;       // its first column
-        double m[8];
-#pragma unroll
-        for (int i = 0; i < 8; ++i) m[i] = tsm[(half * 8 + i) * 129 + cc];
+        for (int i = 0; i < RS_BAND_ROWS; ++i) m[i] = tw[i * RS_TW_PITCH + cc];
         if (!diag) {
             double2* dst = reinterpret_cast<double2*>(Out + (size_t)mrow * ld + mcol);
 #pragma unroll
-            for (int i = 0; i < 4; ++i) dst[i] = make_double2(m[2 * i], m[2 * i + 1]);
+            for (int i = 0; i < RS_BAND_ROWS / 2; ++i) dst[i] = make_double2(m[2 * i], m[2 * i + 1]);
         } else {
 #pragma unroll
-            for (int i = 0; i < 8; ++i)
+            for (int i = 0; i < RS_BAND_ROWS; ++i)
                 if (mrow > mcol + i) Out[(size_t)mrow * ld + mcol + i] = m[i];
         }
     }
@@ -207,15 +259,8 @@ __device__ __forceinline__ void resident_fixup_band(const ResidentPlan& p, int q
         p_trc += __shfl_xor_sync(0xffffffffu, p_trc, m);
         p_ce += __shfl_xor_sync(0xffffffffu, p_ce, m);
     }
-    if (lane == 0) { red[warp][0] = p_tr; red[warp][1] = p_ss; red[warp][2] = p_err; red[warp][3] = p_trc; red[warp][4] = p_ce; }
-    __syncthreads();
-    if (t < 5) {
-        double v = 0.0;
-#pragma unroll
-        for (int w = 0; w < SQ_CONSUMER_WARPS; ++w) v += red[w][t];
-        rec[(size_t)(p.n_tiles + j * RS_BANDS + band) * SQ_NPART + t] = v;
-    }
-    __syncthreads();      // tsm and red are reused by the next band
+    if (lane == 0) { wsum[0] += p_tr; wsum[1] += p_ss; wsum[2] += p_err; wsum[3] += p_trc; wsum[4] += p_ce; }
+    __syncwarp();      // tw is reused by this warp's next band
 }
 
 __global__ void __launch_bounds__(SQ_THREADS, 1)
@@ -226,8 +271,9 @@ resident_recursion_kernel(const __grid_constant__ CUtensorMap tm0, const __grid_
     __shared__ __align__(8) uint64_t full_bar[SQ_STAGES];
     __shared__ __align__(8) uint64_t empty_bar[SQ_STAGES];
     __shared__ double red[SQ_CONSUMER_WARPS][5];
-    __shared__ double sh_sum[SQ_THREADS];
+    __shared__ double sh3[SQ_CONSUMER_WARPS][3];
     __shared__ __align__(16) Ctrl cs;      // this CTA's copy of the control block
+    __shared__ int4 fx_meta[SQ_CONSUMER_WARPS];   // FIX: (first CTA, segments, I, J) of each warp's first band (static over the steps)
 
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
@@ -254,10 +300,20 @@ resident_recursion_kernel(const __grid_constant__ CUtensorMap tm0, const __grid_
         int* dst = reinterpret_cast<int*>(&cs);
         for (int i = threadIdx.x; i < (int)(sizeof(Ctrl) / sizeof(int)); i += SQ_THREADS) dst[i] = __ldcg(src + i);
     }
+    if (lane == 0) {
+        const int q0 = b + warp * G;
+        int4 m4 = make_int4(0, 0, 0, 0);
+        if (q0 < p.n_split * RS_BANDS) {
+            const int4 sp = p.split[q0 / RS_BANDS];
+            const int2 ij = p.tile_map[sp.x];
+            m4 = make_int4(sp.y, sp.z, ij.x, ij.y);
+        }
+        fx_meta[warp] = m4;
+    }
     __syncthreads();
 
-    const long long u_begin = (long long)b * p.U / G, u_end = (long long)(b + 1) * p.U / G;
-    const int n_units = (int)(u_end - u_begin);
+    const int u_begin = rs_boundary(p, b), u_end = rs_boundary(p, b + 1);
+    const int n_units = u_end - u_begin;
 
     // ring state: lives across segments AND steps (the mbarrier phases simply keep alternating)
     int ld_s = 0;
@@ -266,7 +322,8 @@ resident_recursion_kernel(const __grid_constant__ CUtensorMap tm0, const __grid_
     int s = 0;
     uint32_t ph = 0;                 // consumers
     unsigned epoch = 0;
-    unsigned long long step_ns = 0;
+    unsigned long long step_ns = 0, ph_ns[5] = {0, 0, 0, 0, 0};
+    const bool timer = (b == 0 && threadIdx.x == 0);
 
     // consumer geometry, as in sym_square_kernel: 2 x 4 warps of 64 x 32 outputs, fragment row m <-> tile row 2m + p
     const int warp_m = warp >> 2, warp_n = warp & 3;
@@ -286,13 +343,13 @@ resident_recursion_kernel(const __grid_constant__ CUtensorMap tm0, const __grid_
         const double* __restrict__ E = cur ? p.W1 : p.W0;
         double* __restrict__ Out = cur ? p.W0 : p.W1;
         double* __restrict__ rec = cur ? p.rec1 : p.rec0;
-        unsigned long long t_start = 0;
-        if (b == 0 && threadIdx.x == 0) t_start = globaltimer_ns();
+        unsigned long long t_start = 0, t_a = 0, t_b = 0;
+        if (timer) t_start = t_a = globaltimer_ns();
 
         // ================= MM: this CTA's range of chunk units =================
         int ld_r = 0;                                   // units of this step already requested
-        int p_tile = (int)(u_begin / KT), p_kt = (int)(u_begin - (long long)p_tile * KT);
-        int2 p_ij = p.tile_map[p_tile];
+        int p_tile = u_begin / KT, p_kt = u_begin - p_tile * KT;
+        int2 p_ij = p.tile_map[n_units > 0 ? p_tile : 0];
         auto issue_loads = [&](int upto) {
             while (ld_r < upto) {
                 if (ld_total >= SQ_STAGES && !mbar_test(empty0 + 8 * ld_s, ld_ph ^ 1u)) break;
@@ -315,20 +372,17 @@ resident_recursion_kernel(const __grid_constant__ CUtensorMap tm0, const __grid_
             }
         };
         int done = 0;                                   // units of this step already consumed
-        auto wait_full = [&](uint32_t bar, uint32_t parity) {
-            if (mbar_try(bar, parity)) return;
-            if (warp == 0) {
-                do { issue_loads(min(n_units, done + SQ_STAGES)); } while (!mbar_test(bar, parity));
-            } else {
-                mbar_wait_bounded(bar, parity);
-            }
+        // warp 0 is producer and consumer: before it blocks on a stage, the load into that stage must have been issued
+        auto ensure_issued = [&](int upto) {
+            issue_loads(min(n_units, done + SQ_STAGES));
+            while (ld_r < min(n_units, upto)) issue_loads(min(n_units, done + SQ_STAGES));
         };
 
-        long long u = u_begin;
+        int u = u_begin;
         while (u < u_end) {
-            const int tile = (int)(u / KT);
-            const int kt0 = (int)(u - (long long)tile * KT);
-            const int len = min(KT - kt0, (int)(u_end - u));
+            const int tile = u / KT;
+            const int kt0 = u - tile * KT;
+            const int len = min(KT - kt0, u_end - u);
             const int2 ij = p.tile_map[tile];
             const int I = ij.x, J = ij.y;
             const bool diag = (I == J);
@@ -352,12 +406,12 @@ resident_recursion_kernel(const __grid_constant__ CUtensorMap tm0, const __grid_
             };
 
             double a0[8], b0[4], a1[8], b1[4];
-            if (warp == 0) issue_loads(min(n_units, done + SQ_STAGES));
-            wait_full(full0 + 8 * s, ph);
+            if (warp == 0) ensure_issued(done + 1);
+            mbar_wait_safe(full0 + 8 * s, ph);
             uint32_t st = smem_base + s * STAGE_BYTES;
             load_frag(a0, b0, st + rowA, st + rowB, off[0]);
             for (int i = 0; i < len; ++i) {
-                if (warp == 0) issue_loads(min(n_units, done + SQ_STAGES));
+                if (warp == 0) ensure_issued(done + 2);
                 const uint32_t aB = st + rowA, bB = st + rowB;
                 int s1 = s + 1;
                 uint32_t ph1 = ph;
@@ -368,7 +422,7 @@ resident_recursion_kernel(const __grid_constant__ CUtensorMap tm0, const __grid_
                 load_frag(a0, b0, aB, bB, off[2]);
                 mma_step(a1, b1);
                 load_frag(a1, b1, aB, bB, off[3]);
-                if (i + 1 < len) wait_full(full0 + 8 * s1, ph1);
+                if (i + 1 < len) mbar_wait_safe(full0 + 8 * s1, ph1);
                 mma_step(a0, b0);
                 load_frag(a0, b0, stn + rowA, stn + rowB, off[0]);      // last chunk of a segment: stale, reloaded below
                 mma_step(a1, b1);
@@ -473,32 +527,57 @@ resident_recursion_kernel(const __grid_constant__ CUtensorMap tm0, const __grid_
             }
             u += len;
         }
+        if (timer) { t_b = globaltimer_ns(); ph_ns[0] += t_b - t_a; t_a = t_b; }
         grid_barrier(p.flags, G, epoch);
+        if (timer) { t_b = globaltimer_ns(); ph_ns[1] += t_b - t_a; t_a = t_b; }
 
-        // ================= FIX: split tiles, in bands over all CTAs =================
+        // ================= FIX: split tiles, a band per warp, over all warps of the grid =================
         {
             const double c2 = cs.coef.c2, c1 = cs.coef.c1, c0 = cs.coef.c0;
-            for (int q = b; q < p.n_split * RS_BANDS; q += G) resident_fixup_band(p, q, G, E, Out, rec, c2, c1, c0, tsm, red);
+            double* tw = tsm + warp * (RS_BAND_ROWS * RS_TW_PITCH);
+            const int n_q = p.n_split * RS_BANDS;
+            if (lane < 5) red[warp][lane] = 0.0;
+            __syncwarp();
+            int4 meta = fx_meta[warp];                          // this warp's first band: looked up once, at kernel start
+            for (int q = b + warp * G; q < n_q; q += SQ_CONSUMER_WARPS * G) {
+                if (q >= SQ_CONSUMER_WARPS * G) {               // further bands of large problems: look up now
+                    const int4 sp = p.split[q / RS_BANDS];
+                    const int2 ij = p.tile_map[sp.x];
+                    meta = make_int4(sp.y, sp.z, ij.x, ij.y);
+                }
+                resident_fixup_band(meta, q % RS_BANDS, p.ws, p.ld, p.kvalid, E, Out, c2, c1, c0, tw, &red[warp][0]);
+            }
+            // this CTA's bands -> ONE record: a warp's bands in order, then the warps in order (fixed by the plan)
+            __syncthreads();
+            if (threadIdx.x < 5) {
+                double v = 0.0;
+#pragma unroll
+                for (int w = 0; w < SQ_CONSUMER_WARPS; ++w) v += red[w][threadIdx.x];
+                rec[(size_t)(p.n_tiles + b) * SQ_NPART + threadIdx.x] = v;
+            }
         }
+        if (timer) { t_b = globaltimer_ns(); ph_ns[2] += t_b - t_a; t_a = t_b; }
         grid_barrier(p.flags, G, epoch);
+        if (timer) { t_b = globaltimer_ns(); ph_ns[3] += t_b - t_a; t_a = t_b; }
 
         // ================= CTL: the same sums, the same decision, in every CTA =================
         {
-            const int n_rec = p.n_tiles + RS_BANDS * p.n_split;
-            const double t1 = block_sum_strided_cg(rec + 0, n_rec, SQ_NPART, sh_sum);
-            const double s1 = block_sum_strided_cg(rec + 1, n_rec, SQ_NPART, sh_sum);
-            const double e2 = block_sum_strided_cg(rec + 2, n_rec, SQ_NPART, sh_sum);
+            double t1, s1, e2;
+            record_sums_cg(rec, p.n_tiles + G, sh3, t1, s1, e2);
             if (threadIdx.x == 0) control_update(&cs, t1, s1, e2);
             __syncthreads();
         }
-        if (b == 0 && threadIdx.x == 0) step_ns += globaltimer_ns() - t_start;
+        if (timer) { t_b = globaltimer_ns(); ph_ns[4] += t_b - t_a; step_ns += t_b - t_start; }
     }
 
     if (b == 0) {
         const int* src = reinterpret_cast<const int*>(&cs);
         int* dst = reinterpret_cast<int*>(p.ctrl);
         for (int i = threadIdx.x; i < (int)(sizeof(Ctrl) / sizeof(int)); i += SQ_THREADS) dst[i] = src[i];
-        if (threadIdx.x == 0) p.timing[0] = step_ns;
+        if (threadIdx.x == 0) {
+            p.timing[0] = step_ns;
+            for (int i = 0; i < 5; ++i) p.timing[1 + i] = ph_ns[i];
+        }
     }
 }
 

@@ -18,6 +18,7 @@
 #include "lanczos.cuh"
 #include "probe.cuh"
 #include "resident.cuh"
+#include "resident_small.cuh"
 #include "shard.cuh"
 #include "subspace.cuh"
 #include "sym_square.cuh"
@@ -62,8 +63,8 @@ struct rfoe_handle_s {
     int* d_word = nullptr; // device alias of hp->word
     // the whole recursion in one persistent launch (resident.cuh)
     int coop_ok = 0;           // cooperative launch supported and one CTA of the kernel fits an SM
-    int rs_m = 0, rs_G = 0, rs_n_split = 0;   // the plan the split list / records were set up for
-    int2* d_split = nullptr;
+    int rs_m = 0, rs_G = 0, rs_n_split = 0, rs_tile_cost = 0;   // the plan the split list / records were set up for
+    int4* d_split = nullptr;
     double* d_rec[2] = {nullptr, nullptr};
     unsigned* d_flags = nullptr;
     unsigned long long* d_timing = nullptr;
@@ -145,11 +146,11 @@ static int ensure_tiles(rfoe_handle_s* h, int m, cudaStream_t st)
     return RFOE_OK;
 }
 
-static int make_map(rfoe_handle_s* h, CUtensorMap* map, double* base, int n, int ld)
+static int make_map(rfoe_handle_s* h, CUtensorMap* map, double* base, int n, int ld, int box_rows = SQ_BM)
 {
     cuuint64_t dims[2] = {(cuuint64_t)n, (cuuint64_t)n};
     cuuint64_t strides[1] = {(cuuint64_t)ld * sizeof(double)};
-    cuuint32_t box[2] = {(cuuint32_t)SQ_BK, (cuuint32_t)SQ_BM};
+    cuuint32_t box[2] = {(cuuint32_t)SQ_BK, (cuuint32_t)box_rows};
     cuuint32_t estr[2] = {1, 1};
     CUresult r = h->encode(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, base, dims, strides, box, estr,
                            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
@@ -376,12 +377,12 @@ extern "C" int rfoe_create(rfoe_handle_t* out, int device, int64_t k_max)
     ok = ok && cudaMalloc(&h->d_tiles, nt * sizeof(int2)) == cudaSuccess;
     ok = ok && cudaMalloc(&h->d_pairs, nt * sizeof(int2)) == cudaSuccess;
     {
-        const size_t mr = (size_t)RS_MAX_N / SQ_BM, nrec = mr * (mr + 1) / 2 + (size_t)RS_BANDS * RS_MAX_SPLIT;
-        ok = ok && cudaMalloc(&h->d_split, RS_MAX_SPLIT * sizeof(int2)) == cudaSuccess;
+        const size_t mr = (size_t)RS_MAX_N / SQ_BM, nrec = mr * (mr + 1) / 2 + 256;
+        ok = ok && cudaMalloc(&h->d_split, RS_MAX_SPLIT * sizeof(int4)) == cudaSuccess;
         ok = ok && cudaMalloc(&h->d_rec[0], nrec * SQ_NPART * sizeof(double)) == cudaSuccess;
         ok = ok && cudaMalloc(&h->d_rec[1], nrec * SQ_NPART * sizeof(double)) == cudaSuccess;
         ok = ok && cudaMalloc(&h->d_flags, 256 * sizeof(unsigned)) == cudaSuccess;
-        ok = ok && cudaMalloc(&h->d_timing, 2 * sizeof(unsigned long long)) == cudaSuccess;
+        ok = ok && cudaMalloc(&h->d_timing, 8 * sizeof(unsigned long long)) == cudaSuccess;
     }
     ok = ok && cudaHostAlloc((void**)&h->hp, sizeof(HostPage), cudaHostAllocMapped) == cudaSuccess;
     ok = ok && cudaHostGetDevicePointer((void**)&h->d_word, (void*)&h->hp->word, 0) == cudaSuccess;
@@ -400,6 +401,7 @@ extern "C" int rfoe_create(rfoe_handle_t* out, int device, int64_t k_max)
         cudaFuncSetAttribute(sym_square_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, SQ_SMEM_BYTES) != cudaSuccess ||
         cudaFuncSetAttribute(sym_square_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, SQ_SMEM_BYTES) != cudaSuccess ||
         cudaFuncSetAttribute(resident_recursion_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, RS_SMEM_BYTES) != cudaSuccess ||
+        cudaFuncSetAttribute(resident_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, RT_SMEM_BYTES) != cudaSuccess ||
         cudaFuncSetAttribute(apply_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, AP_SMEM_BYTES) != cudaSuccess ||
         cudaFuncSetAttribute(sym_square_reduced_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TQ_SMEM_BYTES) != cudaSuccess) {
         rfoe_destroy(h);
@@ -409,7 +411,8 @@ extern "C" int rfoe_create(rfoe_handle_t* out, int device, int64_t k_max)
         int coop = 0, per_sm = 0;
         if (cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, device) == cudaSuccess && coop &&
             cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, resident_recursion_kernel, SQ_THREADS, RS_SMEM_BYTES) == cudaSuccess &&
-            per_sm >= 1 && h->sm_count <= 256)
+            per_sm >= 1 && h->sm_count <= 256 && (RT_MAX_N / RT_BM) * (RT_MAX_N / RT_BM + 1) / 2 <= h->sm_count &&
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, resident_small_kernel, SQ_THREADS, RT_SMEM_BYTES) == cudaSuccess && per_sm >= 1)
             h->coop_ok = 1;
         cudaGetLastError();
     }
@@ -619,28 +622,51 @@ extern "C" int rfoe_shard_range(int64_t n_tiles, int rank, int world, int64_t* b
     return RFOE_OK;
 }
 
-// Plan of the persistent recursion (resident.cuh): G CTAs share the n_tiles x KT chunk units of a step evenly; a tile
-// not wholly inside one CTA's range [b U / G, (b+1) U / G) is "split" and finished in the FIX phase.
+// Plan of the persistent recursion (resident.cuh): G CTAs (one per SM, fewer when there are fewer chunk units than SMs)
+// share the n_tiles x KT chunk units of a step in contiguous ranges of equal cost; a tile not wholly inside one range is
+// "split" and finished in the FIX phase.  host_boundary is the twin of rs_boundary in resident.cuh.
+static int host_boundary(long long cost_total, int tile_cost, int KT, int G, int b)
+{
+    const long long c = (long long)b * cost_total / G;
+    const int tile = (int)(c / tile_cost);
+    const int off = (int)(c - (long long)tile * tile_cost);
+    return tile * KT + (off < KT ? off : KT);
+}
+
 static int ensure_resident_plan(rfoe_handle_s* h, int m, int KT, cudaStream_t st)
 {
     const long long U = (long long)h->n_tiles * KT;
     const int G = (int)(U < h->sm_count ? U : h->sm_count);
     if (h->rs_m == m && h->rs_G == G) return RFOE_OK;
-    std::vector<int2> split;
-    int b = 0;
-    for (int t = 0; t < h->n_tiles; ++t) {
-        const long long t0 = (long long)t * KT, t1 = t0 + KT;
-        while ((long long)(b + 1) * U / G <= t0) ++b;          // b: the CTA whose range holds unit t0
-        if ((long long)(b + 1) * U / G < t1) split.push_back(make_int2(t, b));
+    // register epilogues are counted into the ranges only where a CTA holds several whole tiles; where nearly every tile
+    // is split (FIX finishes those) the ranges are equal in chunk units
+    int tile_cost = (U / G >= 2LL * KT) ? KT + RS_EPI_COST : KT;
+    std::vector<int4> split;
+    for (int attempt = 0; attempt < 2; ++attempt) {
+        const long long total = (long long)h->n_tiles * tile_cost;
+        bool empty = false;
+        for (int b = 0; b < G && !empty; ++b) empty = host_boundary(total, tile_cost, KT, G, b + 1) <= host_boundary(total, tile_cost, KT, G, b);
+        if (empty && tile_cost != KT) { tile_cost = KT; continue; }      // (cannot happen with ranges >= 2 tiles; belt and braces)
+        split.clear();
+        int b = 0;
+        for (int t = 0; t < h->n_tiles; ++t) {
+            const int t0 = t * KT, t1 = t0 + KT;
+            while (host_boundary(total, tile_cost, KT, G, b + 1) <= t0) ++b;          // b: the CTA whose range holds unit t0
+            if (host_boundary(total, tile_cost, KT, G, b + 1) >= t1) continue;         // whole: register epilogue in MM
+            int nseg = 1;
+            while (host_boundary(total, tile_cost, KT, G, b + nseg) < t1) ++nseg;      // CTAs b .. b + nseg - 1 hold its segments
+            split.push_back(make_int4(t, b, nseg, 0));
+        }
+        break;
     }
     if ((int)split.size() > RS_MAX_SPLIT) return RFOE_ERR_UNSUPPORTED;
     h->rs_m = 0;
-    if (!split.empty()) CK(cudaMemcpyAsync(h->d_split, split.data(), split.size() * sizeof(int2), cudaMemcpyHostToDevice, st));
-    const size_t nrec = (size_t)h->n_tiles + (size_t)RS_BANDS * split.size();
+    if (!split.empty()) CK(cudaMemcpyAsync(h->d_split, split.data(), split.size() * sizeof(int4), cudaMemcpyHostToDevice, st));
+    const size_t nrec = (size_t)h->n_tiles + (size_t)G;
     CK(cudaMemsetAsync(h->d_rec[0], 0, nrec * SQ_NPART * sizeof(double), st));   // the tile records of split tiles stay zero
     CK(cudaMemsetAsync(h->d_rec[1], 0, nrec * SQ_NPART * sizeof(double), st));
     CK(cudaStreamSynchronize(st));   // `split` is pageable and dies here
-    h->rs_m = m; h->rs_G = G; h->rs_n_split = (int)split.size();
+    h->rs_m = m; h->rs_G = G; h->rs_n_split = (int)split.size(); h->rs_tile_cost = tile_cost;
     return RFOE_OK;
 }
 
@@ -729,7 +755,8 @@ static int expand_impl(rfoe_handle_t h, const double* Hp, int64_t k64, int64_t n
     // the whole recursion in one persistent launch when the problem is small enough to live on chip (resident.cuh)
     const bool use_resident = h->resident && h->coop_ok && !sh && n <= RS_MAX_N &&
                               (variant == RFOE_VARIANT_SP2 || variant == RFOE_VARIANT_SP2_ACCEL || variant == RFOE_VARIANT_TRUNC);
-    if (use_resident) {
+    const bool use_small = use_resident && n <= RT_MAX_N;      // latency-bound sizes: 32 x 32 tiles, one grid barrier per step
+    if (use_resident && !use_small) {
         if ((rc = ensure_resident_plan(h, m, n / SQ_BK, st)) != RFOE_OK) return fail(rc);
         if ((rc = ensure_ws(h, (size_t)2 * h->rs_G * RS_TILE_ELEMS * sizeof(double))) != RFOE_OK) return fail(rc);
     }
@@ -793,15 +820,29 @@ static int expand_impl(rfoe_handle_t h, const double* Hp, int64_t k64, int64_t n
         ResidentPlan rp = {};
         rp.n = n; rp.ld = ld; rp.kvalid = k; rp.KT = n / SQ_BK;
         rp.n_tiles = h->n_tiles; rp.n_split = h->rs_n_split; rp.G = h->rs_G;
-        rp.U = (long long)h->n_tiles * rp.KT;
+        rp.tile_cost = h->rs_tile_cost;
+        rp.cost_total = (long long)h->n_tiles * rp.tile_cost;
         rp.tile_map = h->d_tiles; rp.split = h->d_split;
         rp.W0 = h->W[0]; rp.W1 = h->W[1]; rp.ws = h->ws;
         rp.rec0 = h->d_rec[0]; rp.rec1 = h->d_rec[1];
         rp.flags = h->d_flags; rp.ctrl = h->d_ctrl; rp.timing = h->d_timing;
         CK(cudaMemsetAsync(h->d_flags, 0, 256 * sizeof(unsigned), st));
-        CK(cudaMemsetAsync(h->d_timing, 0, 2 * sizeof(unsigned long long), st));
-        void* args[3] = {(void*)&tm[0], (void*)&tm[1], (void*)&rp};
-        CK(cudaLaunchCooperativeKernel((const void*)resident_recursion_kernel, dim3(h->rs_G), dim3(SQ_THREADS), args, RS_SMEM_BYTES, st));
+        CK(cudaMemsetAsync(h->d_timing, 0, 8 * sizeof(unsigned long long), st));
+        if (use_small) {
+            CUtensorMap ts[2];
+            for (int i = 0; i < 2; ++i)
+                if ((rc = make_map(h, &ts[i], h->W[i], n, ld, RT_BM)) != RFOE_OK) return fail(rc);
+            SmallPlan sp = {};
+            sp.n = n; sp.ld = ld; sp.kvalid = k; sp.m32 = n / RT_BM;
+            sp.n_tiles = sp.m32 * (sp.m32 + 1) / 2;
+            sp.W0 = h->W[0]; sp.W1 = h->W[1]; sp.rec0 = h->d_rec[0]; sp.rec1 = h->d_rec[1];
+            sp.flags = h->d_flags; sp.ctrl = h->d_ctrl; sp.timing = h->d_timing;
+            void* args[3] = {(void*)&ts[0], (void*)&ts[1], (void*)&sp};
+            CK(cudaLaunchCooperativeKernel((const void*)resident_small_kernel, dim3(sp.n_tiles), dim3(SQ_THREADS), args, RT_SMEM_BYTES, st));
+        } else {
+            void* args[3] = {(void*)&tm[0], (void*)&tm[1], (void*)&rp};
+            CK(cudaLaunchCooperativeKernel((const void*)resident_recursion_kernel, dim3(h->rs_G), dim3(SQ_THREADS), args, RS_SMEM_BYTES, st));
+        }
         h->launches++;
         copy_out_select_kernel<<<hbm_grid(h, k), HBM_THREADS, 0, st>>>(h->W[0], h->W[1], &h->d_ctrl->step, k, ld, Hp, P, h->rows[0]);
         h->launches++;
@@ -811,13 +852,15 @@ static int expand_impl(rfoe_handle_t h, const double* Hp, int64_t k64, int64_t n
         CK(cudaGetLastError());
         CK(cudaEventRecord(h->ev1, st));
         CK(cudaMemcpyAsync(&C, h->d_ctrl, sizeof(Ctrl), cudaMemcpyDeviceToHost, st));
-        CK(cudaMemcpyAsync((void*)h->hp->scalars, h->d_timing, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+        CK(cudaMemcpyAsync((void*)h->hp->scalars, h->d_timing, 8 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
         CK(cudaStreamSynchronize(st));
         if ((rc = check_prologue()) != RFOE_OK) return fail(rc);
         float ms = 0.f;
         CK(cudaEventElapsedTime(&ms, h->ev0, h->ev1));
-        unsigned long long step_ns = 0;
-        memcpy(&step_ns, (const void*)h->hp->scalars, sizeof(step_ns));
+        unsigned long long tim[8];
+        memcpy(tim, (const void*)h->hp->scalars, sizeof(tim));
+        const unsigned long long step_ns = tim[0];
+        for (int i = 0; i < 5; ++i) S.resident_phase_ms[i] = (double)tim[1 + i] * 1e-6;
         S.iterations = C.step; S.multiplications = C.multiplications; S.mcweeny_steps = C.mcweeny_steps;
         S.fp32_steps = C.fp32_steps; S.converged = C.converged; S.tr_PH = C.tr_PH; S.device_ms = ms;
         S.gpu_launches = h->launches;

@@ -133,15 +133,6 @@ apply_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CU
         }
     };
     if (warp == 0) issue_loads(min(KT, SQ_STAGES));
-    // warp 0 (producer and consumer) never blocks on a full-barrier: it polls and keeps issuing (see sym_square.cuh)
-    auto wait_full = [&](uint32_t bar, uint32_t parity, int kt_now) {
-        if (mbar_try(bar, parity)) return;          // the common case, the same instructions for every warp
-        if (warp == 0) {
-            do { issue_loads(min(KT, kt_now + SQ_STAGES)); } while (!mbar_test(bar, parity));
-        } else {
-            mbar_wait_bounded(bar, parity);
-        }
-    };
 
     const int warp_m = warp >> 2;      // 0..1 -> 64 tile rows
     const int warp_n = warp & 3;       // 0..3 -> 32 tile cols
@@ -187,11 +178,17 @@ apply_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CU
     int s = 0;
     uint32_t ph = 0;
     double a0[8], b0[4], a1[8], b1[4];
-    wait_full(full0, 0, 0);
+    mbar_wait(full0, 0);
     uint32_t st = smem_base;
     load_frag(a0, b0, st, 0);
     for (int kt = 0; kt < KT; ++kt) {
-        if (warp == 0) issue_loads(min(KT, kt + SQ_STAGES));
+        if (warp == 0) {
+            issue_loads(min(KT, kt + SQ_STAGES));
+            // Warp 0 is the only producer AND a consumer, and it blocks on chunk kt+1 further down: that chunk must have been
+            // issued by then, or nobody ever would.  It normally was, five iterations ago; if another warp still holds its stage
+            // (a 5-chunk skew, which the 6-stage ring permits), wait HERE, where waiting cannot deadlock (that warp has its data).
+            while (ld_kt < min(KT, kt + 2)) issue_loads(min(KT, kt + SQ_STAGES));
+        }
         int s1 = s + 1;
         uint32_t ph1 = ph;
         if (s1 == SQ_STAGES) { s1 = 0; ph1 ^= 1u; }
@@ -201,7 +198,7 @@ apply_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CU
         load_frag(a0, b0, st, 2);
         mma_step(a1, b1);
         load_frag(a1, b1, st, 3);
-        if (kt + 1 < KT) wait_full(full0 + 8 * s1, ph1, kt);
+        if (kt + 1 < KT) mbar_wait(full0 + 8 * s1, ph1);
         mma_step(a0, b0);
         load_frag(a0, b0, stn, 0);      // after the last stage this reads stale smem; unused
         mma_step(a1, b1);

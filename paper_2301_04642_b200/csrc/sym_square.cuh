@@ -123,18 +123,6 @@ sym_square_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
         }
     };
     if (warp == 0) issue_loads(min(KT, SQ_STAGES));
-    // Waiting for a stage to fill.  Warp 0 is the only producer AND a consumer: if it blocked here while another warp
-    // still held the stage that chunk kt+1 must go into (a 5-chunk skew, which the 6-stage ring permits), nobody would
-    // ever issue that chunk.  So warp 0 polls and keeps issuing; the other warps wait (bounded: a pipeline bug traps
-    // instead of hanging the GPU).
-    auto wait_full = [&](uint32_t bar, uint32_t parity, int kt_now) {
-        if (mbar_try(bar, parity)) return;          // the common case, the same instructions for every warp
-        if (warp == 0) {
-            do { issue_loads(min(KT, kt_now + SQ_STAGES)); } while (!mbar_test(bar, parity));
-        } else {
-            mbar_wait_bounded(bar, parity);
-        }
-    };
     {
         // ===== consumers =====
         const int warp_m = warp >> 2;      // 0..1  -> 64 tile rows
@@ -177,11 +165,17 @@ sym_square_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
         int s = 0;
         uint32_t ph = 0;
         double a0[8], b0[4], a1[8], b1[4];
-        wait_full(full0, 0, 0);
+        mbar_wait(full0, 0);
         uint32_t st = smem_base;
         load_frag(a0, b0, st + rowA, st + rowB, off[0]);
         for (int kt = 0; kt < KT; ++kt) {
-            if (warp == 0) issue_loads(min(KT, kt + SQ_STAGES));
+            if (warp == 0) {
+                issue_loads(min(KT, kt + SQ_STAGES));
+                // Warp 0 is the only producer AND a consumer, and it blocks on chunk kt+1 further down: that chunk must have been
+                // issued by then, or nobody ever would.  It normally was, five iterations ago; if another warp still holds its stage
+                // (a 5-chunk skew, which the 6-stage ring permits), wait HERE, where waiting cannot deadlock (that warp has its data).
+                while (ld_kt < min(KT, kt + 2)) issue_loads(min(KT, kt + SQ_STAGES));
+            }
             const uint32_t aB = st + rowA, bB = st + rowB;
             int s1 = s + 1;
             uint32_t ph1 = ph;
@@ -192,7 +186,7 @@ sym_square_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
             load_frag(a0, b0, aB, bB, off[2]);
             mma_step(a1, b1);
             load_frag(a1, b1, aB, bB, off[3]);
-            if (kt + 1 < KT) wait_full(full0 + 8 * s1, ph1, kt);
+            if (kt + 1 < KT) mbar_wait(full0 + 8 * s1, ph1);
             mma_step(a0, b0);
             // first fragments of the next stage (after the last stage this reads stale smem; unused)
             load_frag(a0, b0, stn + rowA, stn + rowB, off[0]);

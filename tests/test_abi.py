@@ -30,7 +30,7 @@ def test_header_symbols_are_exported():
 def test_stats_struct_matches_header():
     # sizeof(rfoe_stats_t) computed from the header's field list
     n = rfoe.MAX_STEPS
-    expect = 12 * 4 + 3 * 8 + 6 * 8 + (n + 1) * 8 * 2 + n * 8 * 2 + (n + 8)
+    expect = 12 * 4 + 3 * 8 + 11 * 8 + (n + 1) * 8 * 2 + n * 8 * 2 + (n + 8)
     expect = (expect + 7) // 8 * 8
     assert ctypes.sizeof(rfoe._Stats) == expect
 
