@@ -258,7 +258,24 @@ def run_ours(args) -> int:
         dist.broadcast(H, src=0)         # one problem, the same bytes on every rank
 
     if args.shard == "p2p":
-        h.shard_connect()                # CUDA IPC handles of the work buffers, exchanged over the process group
+        # CUDA IPC handles of the work buffers, exchanged over the process group; every rank must agree on the outcome
+        ok = 1
+        try:
+            h.shard_connect()
+        except rfoe.RfoeError as e:
+            if e.status != rfoe.ERR_NO_PEER_ACCESS:
+                raise
+            ok = 0
+            why = str(e)
+        if world > 1:
+            flag = torch.tensor([ok], device=dev)
+            dist.all_reduce(flag, op=dist.ReduceOp.MIN)
+            ok = int(flag.item())
+        if not ok:
+            if rank == 0:
+                print("bench.py: --shard p2p: a peer GPU's buffers cannot be mapped (no P2P access"
+                      + (": " + why if "why" in dir() else "") + "); falling back to --shard allgather", file=sys.stderr)
+            args.shard = "allgather"
 
     def p2p_barrier(stream_ptr):         # every rank's enqueued work complete, then a cross-rank barrier
         stream.synchronize()

@@ -17,7 +17,7 @@ import numpy as np
 
 from . import build as _build
 
-__all__ = ["Rfoe", "RfoeError", "ExpandResult", "load_library", "shard_range", "torch_distributed_allgather", "SP2", "MCWEENY", "SP2_MIXED", "SP2_ACCEL",
+__all__ = ["Rfoe", "RfoeError", "ExpandResult", "load_library", "shard_range", "torch_distributed_allgather", "gather_ipc_handles", "SP2", "MCWEENY", "SP2_MIXED", "SP2_ACCEL",
            "TRUNC", "TRUNC_MIXED", "RULE_A", "RULE_B", "EXPORTS"]
 
 SP2, MCWEENY, SP2_MIXED, SP2_ACCEL, TRUNC, TRUNC_MIXED = 0, 1, 2, 3, 4, 5
@@ -244,6 +244,21 @@ def shard_range(n_tiles: int, rank: int, world: int):
     if rc != OK:
         raise RfoeError(rc, "rfoe_shard_range: invalid argument")
     return b.value, c.value
+
+
+def gather_ipc_handles(mine: bytes, group=None) -> bytes:
+    """The layout rfoe_shard_ipc_import expects: every rank's 4 x 64-byte CUDA IPC handles (W0, W1, records of even /
+    odd steps), concatenated in RANK order.  Any torch.distributed backend (the handles are host bytes)."""
+    import torch.distributed as dist
+
+    if len(mine) != 4 * IPC_HANDLE_BYTES:
+        raise ValueError("4 x 64 bytes of IPC handles expected")
+    world = dist.get_world_size(group)
+    gathered = [None] * world
+    dist.all_gather_object(gathered, bytes(mine), group=group)
+    out = b"".join(gathered)
+    assert len(out) == 4 * IPC_HANDLE_BYTES * world
+    return out
 
 
 class _DevBytes:
@@ -520,14 +535,12 @@ class Rfoe:
             self._raise(rc)
 
     def shard_connect(self, group=None):
-        """One process per GPU: exchange CUDA IPC handles of the work buffers over torch.distributed and map the peers."""
+        """One process per GPU: exchange CUDA IPC handles of the work buffers over torch.distributed and map the peers.
+        Raises RfoeError(ERR_NO_PEER_ACCESS) when a peer's buffers cannot be reached (fall back to expand_sharded)."""
         import torch.distributed as dist
 
         world, rank = dist.get_world_size(group), dist.get_rank(group)
-        mine = self.shard_ipc_export()
-        gathered = [None] * world
-        dist.all_gather_object(gathered, mine, group=group)
-        self.shard_ipc_import(rank, world, b"".join(gathered))
+        self.shard_ipc_import(rank, world, gather_ipc_handles(self.shard_ipc_export(), group))
         return rank, world
 
     def expand_sharded_p2p(self, Hp, nocc: int, variant: int = SP2, tol: float = 1e-12, P=None, *, barrier=None,

@@ -90,3 +90,41 @@ def test_squaring_launch_plan():
     assert rfoe.plan_squaring(4096)[:3] == (528, 444, 7)
     with pytest.raises(rfoe.RfoeError):
         rfoe.plan_squaring(0)
+
+
+def _ipc_layout_worker(rank, world, port, out):
+    sys.path.insert(0, ROOT)
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    import paper_2301_04642_b200 as rfoe
+
+    # stand-ins for the four 64-byte CUDA IPC handles of a rank (W0, W1, records of even / odd steps): byte (q, i) of
+    # rank r is 64 r + 16 q + (i % 16), so that every position of the gathered buffer names its source
+    mine = bytes((64 * rank + 16 * q + (i % 16)) & 0xFF for q in range(4) for i in range(rfoe.IPC_HANDLE_BYTES))
+    out[rank] = rfoe.gather_ipc_handles(mine)
+    try:
+        rfoe.gather_ipc_handles(mine[:-1])
+        out[f"err{rank}"] = False
+    except ValueError:
+        out[f"err{rank}"] = True
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_ipc_handle_gather_layout_world2():
+    """rfoe_shard_ipc_import reads `world x 4 x 64` bytes, rank-major (include/rfoe.h): the buffer shard_connect builds over
+    the process group must have exactly that order, on every rank."""
+    import paper_2301_04642_b200 as rfoe
+
+    world, port = 2, _free_port()
+    with mp.Manager() as mgr:
+        out = mgr.dict()
+        mp.spawn(_ipc_layout_worker, args=(world, port, out), nprocs=world, join=True)
+        res = dict(out)
+    hb = rfoe.IPC_HANDLE_BYTES
+    assert res[0] == res[1] and len(res[0]) == world * 4 * hb
+    for r in range(world):
+        for q in range(4):
+            seg = res[0][(4 * r + q) * hb:(4 * r + q + 1) * hb]
+            assert seg == bytes((64 * r + 16 * q + (i % 16)) & 0xFF for i in range(hb))
+    assert res["err0"] and res["err1"]
