@@ -387,6 +387,7 @@ def run_ours(args) -> int:
             line["hbm_kernels"] = hbm_report(h, H, stream)
             line["lanczos_bounds"] = lanczos_report(h, rfoe, w, H, P, stream, ms_total / args.steps)
         if world == 1 and not shard and not args.no_many:
+            line["small_configs_single_expand"] = small_configs_report(rfoe, rfoe_inputs, local, peak_probe)
             line["many_small_problems"] = many_report(rfoe, rfoe_inputs, local)
         if want_reduced:
             line["reduced_precision"] = reduced_report(h, rfoe, w, H, P, stream, ms_total / args.steps)
@@ -405,6 +406,38 @@ def run_ours(args) -> int:
     if dist.is_initialized():
         dist.destroy_process_group()
     return 0
+
+
+def small_configs_report(rfoe, rfoe_inputs, local, peak_tflops):
+    """BASELINE configs 1 and 2 (k=256, k=2048) as ONE rfoe_expand each -- the call north_star specifies -- on the default
+    path (the whole recursion in one persistent launch, RFOE_OPT_RESIDENT) and on the launch-per-step path, CUDA-event time
+    of the best of 5 warm runs; executed-flop rate against the probe's FP64 peak."""
+    import torch
+
+    out = {}
+    for c in (1, 2):
+        w = rfoe_inputs.make_workload(c)
+        H = torch.from_numpy(w.H).cuda(local)
+        P = torch.empty_like(H)
+        fl = executed_flops_per_squaring(w.k)
+        row = {}
+        with rfoe.Rfoe(w.k, device=local) as h:
+            for name, resident in (("resident", True), ("launch_per_step", False)):
+                h.configure(resident=resident)
+                best = None
+                for i in range(7):
+                    r = h.expand(H, w.nocc, rfoe.SP2, w.tol, P=P)
+                    if i >= 2 and (best is None or r.device_ms < best.device_ms):
+                        best = r
+                tf = best.iterations * fl / (best.device_ms * 1e-3) / 1e12
+                row[name] = {"ms_per_expansion": best.device_ms, "squarings": best.iterations,
+                             "us_per_step": best.device_ms / best.iterations * 1e3, "tflops_executed": tf,
+                             "frac_of_fp64_peak": tf / peak_tflops, "gpu_launches": best.gpu_launches,
+                             "converged": bool(best.converged)}
+                if resident:
+                    row[name]["phase_us_per_step"] = [x / best.iterations * 1e3 for x in best.resident_phase_ms]
+        out[f"config{c}_k{w.k}"] = row
+    return out
 
 
 def many_report(rfoe, rfoe_inputs, local):

@@ -161,12 +161,12 @@ def test_full_oracle_expansion_every_element(c, variant):
         f.write(repr(out) + "\n")
 
 
-@pytest.mark.parametrize("m", [3, pytest.param(5, marks=pytest.mark.slow)])
+@pytest.mark.parametrize("m", [3])
 def test_headline_size_first_steps_every_element(m):
     """k=16384 (config 4, the size bench.py times): the whole naive oracle expansion would take hours of host time, so the
     first m recursion steps are run on both sides (RFOE_VARIANT_TRUNC with m steps) and EVERY element of
     X_m is compared, with the scalars of every step; both SP2 branches occur in these steps (`LLS...`).  m = 3 runs in the
-    default suite (about 130 s of oracle per step on 16 host threads), m = 5 with RFOE_SLOW=1."""
+    default suite (about 130 s of oracle per step on 16 host threads; round 1 ran m = 5: profiles/r01g_oracle_runs.md)."""
     import time
 
     w = rfoe_inputs.make_workload(4, device="cuda")
