@@ -211,12 +211,15 @@ int rfoe_apply(rfoe_handle_t h, const double* P, const double* Psi, int64_t k, i
                int64_t ldy, double* rho, float* kernel_ms, rfoe_stream_t stream);
 
 /* ---- many independent problems on ONE GPU (k-points, spins) --------------------------------------------------
- * An expansion of a small H^p cannot fill the chip (k=256: 3 output tiles for 148 SMs; k=2048: 136, and every step
- * ends in a host round trip), but independent problems can run side by side: n_handles handles, each with its own
- * stream and its own host thread (std::thread inside the library), take the n_problems problems from a shared counter
- * in order; kernels of different handles overlap on the device.  Every problem goes through exactly the rfoe_expand
- * path, so each P is bitwise the P of a lone rfoe_expand call.  Measured on one B200: k=256 8.7x the single-handle rate
- * with 16 handles, k=2048 77 -> 92 expansions/s with 4 (35 TFLOP/s executed, the FP64 tensor pipe is full).
+ * One expansion of a mid-size H^p leaves part of the chip idle (k=2048: 136 tiles on 148 SMs, an epilogue and a
+ * synchronisation per step), but independent problems can run side by side: n_handles handles, each with its own stream
+ * and its own host thread (std::thread inside the library), take the n_problems problems from a shared counter in order.
+ * Every problem goes through the rfoe_expand path of its handle.  With more than one handle at work, problems of
+ * 1024 < k <= 4096 take the launch-per-step sequence (as with RFOE_OPT_RESIDENT = 0), whose kernels overlap across handles
+ * and fill each other's gaps -- persistent launches of one CTA per SM cannot overlap; k <= 1024 keeps the small persistent
+ * kernel (one expansion after the other, each 3-6x faster than launch-per-step).  Each P is bitwise the P of a lone
+ * rfoe_expand call on the same path.  Measured on one B200: k=256, 16 handles: 8040 expansions/s (one handle: 2410;
+ * round 1's launch-per-step path: 3400 / 430); k=2048, 4 handles: 92 expansions/s = 35 TFLOP/s executed (one: 81).
  *   handles[i], streams[i] : n_handles distinct handles (same device; options as set per handle) and their streams
  *   Hp[j], P[j], k[j], nocc[j], tol[j] : problem j (device matrices as for rfoe_expand; k[j] <= k_max of every handle);
  *                            all Hp[j] must be complete before the call (it does not order itself after other streams)

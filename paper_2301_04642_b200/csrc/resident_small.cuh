@@ -1,14 +1,15 @@
-// The whole recursion of a SMALL H^p (k <= 512) in one persistent launch -- the latency-bound end of resident.cuh.
+// The whole recursion of a SMALL H^p (k <= 1024) in one persistent launch -- the latency-bound end of resident.cuh.
 //
 // At k=256 a squaring is 2.5e7 flops: a microsecond of the chip's FP64 tensor pipe, but 33 us on the one SM that owns a
 // 128 x 128 tile of sym_square_kernel.  What matters here is the length of the dependent chain of one step, so the
-// decomposition is the opposite of the big kernel's: 32 x 32 output tiles with the WHOLE contraction each (no split of
-// the contraction index, so no second pass and ONE grid barrier per step), one tile per CTA, all upper-triangle tiles
-// resident at once (k=256: 36 CTAs, k=512: 136).  Per step a CTA
-//   loads the two 32-row panels of X_n it needs (TMA boxes of 32 rows x 128 bytes, 128-byte swizzle) in chunks of 128
-//     columns through a 3-stage mbarrier ring (k=256: 2 chunks, all in flight at once),
-//   multiplies: 8 warps x (16 x 8 outputs), mma.m8n8k4.f64 (SASS DMMA.8x8x4), two accumulator sets per warp over the
-//     even / odd k4-steps so that four independent DMMA chains run per warp (added at the end: a fixed order),
+// decomposition is the opposite of the big kernel's: small output tiles with the WHOLE contraction each (no split of the
+// contraction index, so no second pass and ONE grid barrier per step), one tile per CTA, all upper-triangle tiles
+// resident at once: BM = 32 for k <= 512 (k=256: 36 CTAs, k=512: 136), BM = 64 for k <= 1024 (136 CTAs).  Per step a CTA
+//   loads the two BM-row panels of X_n it needs (TMA boxes of BM rows x 128 bytes, 128-byte swizzle) in 64 KiB chunks
+//     (BM=32: 128 columns, BM=64: 64) through a 3-stage mbarrier ring (k=256: 2 chunks, all in flight at once),
+//   multiplies: 8 warps x (BM/2 x BM/4 outputs), mma.m8n8k4.f64 (SASS DMMA.8x8x4); with BM=32 a warp has only two output
+//     blocks, so it keeps two accumulator sets over the even / odd k4-steps (four independent DMMA chains; added at the
+//     end: a fixed order),
 //   applies the fused epilogue of sym_square.cuh -- X_{n+1} = c2 C + c1 X_n + c0 I to (I,J) and mirrored to (J,I), the
 //     five partial sums into one record per tile,
 //   passes ONE grid barrier, and takes the step's decision itself: every CTA sums all records in the same fixed order
@@ -18,17 +19,15 @@
 
 namespace rfoe {
 
-constexpr int RT_MAX_N = 512;             // padded size up to which this kernel is used
-constexpr int RT_BM = 32;                 // output tile
-constexpr int RT_KC = 128;                // contraction columns per ring stage
+constexpr int RT_MAX_N = 1024;            // padded size up to which this kernel is used
+constexpr int RT_MAX_N32 = 512;           //   ... with 32 x 32 tiles (136 CTAs at 512); above: 64 x 64 (136 CTAs at 1024)
 constexpr int RT_STAGES = 3;
-constexpr int RT_BOX_BYTES = RT_BM * SQ_BK * 8;                   // 4 KiB: 32 rows x 16 doubles
-constexpr int RT_PANEL_BYTES = (RT_KC / SQ_BK) * RT_BOX_BYTES;    // 32 KiB: one panel's chunk
-constexpr int RT_STAGE_BYTES = 2 * RT_PANEL_BYTES;                // 64 KiB
+constexpr int RT_STAGE_BYTES = 64 * 1024;                         // two panels' chunk
+constexpr int RT_PANEL_BYTES = RT_STAGE_BYTES / 2;
 constexpr int RT_SMEM_BYTES = RT_STAGES * RT_STAGE_BYTES + 1024;
 
 struct SmallPlan {
-    int n, ld, kvalid, m32;       // padded size, row pitch, true size, tiles per side (n / 32)
+    int n, ld, kvalid, mt;        // padded size, row pitch, true size, tiles per side (n / BM)
     int n_tiles, pad0_, pad1_, pad2_;
     double* W0;                   // the two work matrices (ping-pong by step parity)
     double* W1;
@@ -39,10 +38,17 @@ struct SmallPlan {
     unsigned long long* timing;   // CTA 0's %globaltimer, ns: [0] all steps, [1] load + multiply + epilogue, [2] barrier, [3] unused, [4] unused, [5] decision
 };
 
+template <int BM>
 __global__ void __launch_bounds__(SQ_THREADS, 1)
 resident_small_kernel(const __grid_constant__ CUtensorMap tm0, const __grid_constant__ CUtensorMap tm1,
                       const __grid_constant__ SmallPlan p)
 {
+    constexpr int BOX_BYTES = BM * SQ_BK * 8;               // BM rows x 16 doubles
+    constexpr int BOXES = RT_PANEL_BYTES / BOX_BYTES;       // boxes per panel chunk (BM=32: 8, BM=64: 4)
+    constexpr int KC = BOXES * SQ_BK;                       // contraction columns per stage (128 / 64)
+    constexpr int RBW = BM / 16;                            // 8-row output blocks per warp (2 / 4)
+    constexpr int CBW = BM / 32;                            // 8-column output blocks per warp (1 / 2)
+    constexpr int PAR = (RBW * CBW >= 8) ? 1 : 2;           // accumulator sets over alternating k4-steps
     extern __shared__ uint8_t smem_raw[];
     __shared__ __align__(8) uint64_t full_bar[RT_STAGES];
     __shared__ __align__(8) uint64_t empty_bar[RT_STAGES];
@@ -74,29 +80,35 @@ resident_small_kernel(const __grid_constant__ CUtensorMap tm0, const __grid_cons
     }
     __syncthreads();
 
-    // this CTA's tile (I <= J) of the 32 x 32 tiling, row-major over the upper triangle
+    // this CTA's tile (I <= J) of the BM x BM tiling, row-major over the upper triangle
     int I = 0, J;
     {
         int t = b;
-        while (t >= p.m32 - I) { t -= p.m32 - I; ++I; }
+        while (t >= p.mt - I) { t -= p.mt - I; ++I; }
         J = I + t;
     }
     const bool diag = (I == J);
-    const int n_chunks = p.n / RT_KC;
+    const int n_chunks = p.n / KC;
 
-    // warp geometry: 2 x 4 warps of 16 x 8 outputs; lane (r = lane / 4, kk = lane % 4) holds A[r][kk], B[kk][r] and
-    // C[r][2 kk .. 2 kk + 1] of every 8 x 8 x 4 block
+    // warp geometry: 2 x 4 warps of (BM/2) x (BM/4) outputs; lane (r = lane / 4, kk = lane % 4) holds A[r][kk], B[kk][r]
+    // and C[r][2 kk .. 2 kk + 1] of every 8 x 8 x 4 block
     const int warp_m = warp >> 2, warp_n = warp & 3;
     const int r = lane >> 2, kk = lane & 3;
-    // byte offset of element (row, 16-column box, column c of the box) in a panel: box * 4 KiB + row * 128 + swizzle
-    const int rowA0 = warp_m * 16 + r, rowA1 = rowA0 + 8, rowB = warp_n * 8 + r;
-    uint32_t offA0[4], offA1[4], offB[4];
+    // byte offset of element (row, column c of a 16-column box) inside a box: row * 128 + swizzled 16-byte chunk
+    uint32_t offA[RBW][4], offB[CBW][4];
 #pragma unroll
     for (int ks = 0; ks < 4; ++ks) {
         const int c = 4 * ks + kk;
-        offA0[ks] = (uint32_t)(rowA0 * 128 + ((((c >> 1) ^ (rowA0 & 7))) << 4) + (c & 1) * 8);
-        offA1[ks] = (uint32_t)(rowA1 * 128 + ((((c >> 1) ^ (rowA1 & 7))) << 4) + (c & 1) * 8);
-        offB[ks] = (uint32_t)(rowB * 128 + ((((c >> 1) ^ (rowB & 7))) << 4) + (c & 1) * 8) + (uint32_t)RT_PANEL_BYTES;
+#pragma unroll
+        for (int rb = 0; rb < RBW; ++rb) {
+            const int row = warp_m * (BM / 2) + rb * 8 + r;
+            offA[rb][ks] = (uint32_t)(row * 128 + ((((c >> 1) ^ (row & 7))) << 4) + (c & 1) * 8);
+        }
+#pragma unroll
+        for (int cb = 0; cb < CBW; ++cb) {
+            const int row = warp_n * (BM / 4) + cb * 8 + r;
+            offB[cb][ks] = (uint32_t)(row * 128 + ((((c >> 1) ^ (row & 7))) << 4) + (c & 1) * 8) + (uint32_t)RT_PANEL_BYTES;
+        }
     }
 
     int ld_s = 0;
@@ -126,9 +138,9 @@ resident_small_kernel(const __grid_constant__ CUtensorMap tm0, const __grid_cons
                 if (elect_one()) {
                     mbar_expect_tx(fb, RT_STAGE_BYTES);
 #pragma unroll
-                    for (int bx = 0; bx < RT_KC / SQ_BK; ++bx) {
-                        tma_load_2d(dst + bx * RT_BOX_BYTES, tm, ld_r * RT_KC + bx * SQ_BK, I * RT_BM, fb);
-                        tma_load_2d(dst + RT_PANEL_BYTES + bx * RT_BOX_BYTES, tm, ld_r * RT_KC + bx * SQ_BK, J * RT_BM, fb);
+                    for (int bx = 0; bx < BOXES; ++bx) {
+                        tma_load_2d(dst + bx * BOX_BYTES, tm, ld_r * KC + bx * SQ_BK, I * BM, fb);
+                        tma_load_2d(dst + RT_PANEL_BYTES + bx * BOX_BYTES, tm, ld_r * KC + bx * SQ_BK, J * BM, fb);
                     }
                 }
                 __syncwarp();
@@ -138,12 +150,13 @@ resident_small_kernel(const __grid_constant__ CUtensorMap tm0, const __grid_cons
             }
         };
 
-        // two accumulator sets per row block: even / odd k4-steps
-        double acc[2][2][2];
+        double acc[RBW][CBW][PAR][2];
 #pragma unroll
-        for (int rb = 0; rb < 2; ++rb)
+        for (int rb = 0; rb < RBW; ++rb)
 #pragma unroll
-            for (int par = 0; par < 2; ++par) acc[rb][par][0] = acc[rb][par][1] = 0.0;
+            for (int cb = 0; cb < CBW; ++cb)
+#pragma unroll
+                for (int par = 0; par < PAR; ++par) acc[rb][cb][par][0] = acc[rb][cb][par][1] = 0.0;
 
         for (int ch = 0; ch < n_chunks; ++ch) {
             if (warp == 0) {
@@ -153,15 +166,20 @@ resident_small_kernel(const __grid_constant__ CUtensorMap tm0, const __grid_cons
             mbar_wait_safe(full0 + 8 * s, ph);
             const uint32_t st = smem_base + s * RT_STAGE_BYTES;
 #pragma unroll
-            for (int bx = 0; bx < RT_KC / SQ_BK; ++bx) {
-                const uint32_t base = st + bx * RT_BOX_BYTES;
+            for (int bx = 0; bx < BOXES; ++bx) {
+                const uint32_t base = st + bx * BOX_BYTES;
 #pragma unroll
                 for (int ks = 0; ks < 4; ++ks) {
-                    const double a0 = lds_f64(base + offA0[ks]);
-                    const double a1 = lds_f64(base + offA1[ks]);
-                    const double bf = lds_f64(base + offB[ks]);
-                    dmma_8x8x4(acc[0][ks & 1][0], acc[0][ks & 1][1], a0, bf);
-                    dmma_8x8x4(acc[1][ks & 1][0], acc[1][ks & 1][1], a1, bf);
+                    double af[RBW], bf[CBW];
+#pragma unroll
+                    for (int rb = 0; rb < RBW; ++rb) af[rb] = lds_f64(base + offA[rb][ks]);
+#pragma unroll
+                    for (int cb = 0; cb < CBW; ++cb) bf[cb] = lds_f64(base + offB[cb][ks]);
+#pragma unroll
+                    for (int rb = 0; rb < RBW; ++rb)
+#pragma unroll
+                        for (int cb = 0; cb < CBW; ++cb)
+                            dmma_8x8x4(acc[rb][cb][ks & (PAR - 1)][0], acc[rb][cb][ks & (PAR - 1)][1], af[rb], bf[cb]);
                 }
             }
             __syncwarp();
@@ -169,47 +187,57 @@ resident_small_kernel(const __grid_constant__ CUtensorMap tm0, const __grid_cons
             if (++s == RT_STAGES) { s = 0; ph ^= 1u; }
         }
 
-        // ---- fused epilogue on the warp's 16 x 8 outputs
+        // ---- fused epilogue on the warp's (BM/2) x (BM/4) outputs
         {
             const double c2 = cs.coef.c2, c1 = cs.coef.c1, c0 = cs.coef.c0;
             const int ld = p.ld;
             double p_tr = 0.0, p_ss = 0.0, p_err = 0.0, p_trc = 0.0, p_ce = 0.0;
-            const int col = J * RT_BM + warp_n * 8 + 2 * kk;
 #pragma unroll
-            for (int rb = 0; rb < 2; ++rb) {
-                const int row = I * RT_BM + warp_m * 16 + rb * 8 + r;
-                const double cv[2] = {acc[rb][0][0] + acc[rb][1][0], acc[rb][0][1] + acc[rb][1][1]};
-                const double2 e2 = __ldcg(reinterpret_cast<const double2*>(E + (size_t)row * ld + col));
-                const double ev[2] = {e2.x, e2.y};
-                double o[2];
+            for (int rb = 0; rb < RBW; ++rb) {
+                const int row = I * BM + warp_m * (BM / 2) + rb * 8 + r;
 #pragma unroll
-                for (int u = 0; u < 2; ++u) {
-                    double v = fma(c2, cv[u], c1 * ev[u]);
-                    const double d = cv[u] - ev[u];
-                    double w = 1.0;
-                    if (diag) {
-                        const int cc = col + u;
-                        w = (cc > row) ? 2.0 : ((cc == row) ? 1.0 : 0.0);
-                        if (cc == row) {
-                            if (row < p.kvalid) v += c0;
-                            p_tr += v;
-                            p_trc += cv[u];
-                        }
+                for (int cb = 0; cb < CBW; ++cb) {
+                    const int col = J * BM + warp_n * (BM / 4) + cb * 8 + 2 * kk;
+                    double cv[2];
+                    if (PAR == 2) {
+                        cv[0] = acc[rb][cb][0][0] + acc[rb][cb][PAR - 1][0];
+                        cv[1] = acc[rb][cb][0][1] + acc[rb][cb][PAR - 1][1];
+                    } else {
+                        cv[0] = acc[rb][cb][0][0];
+                        cv[1] = acc[rb][cb][0][1];
                     }
-                    o[u] = v;
-                    p_ss = fma(w * v, v, p_ss);
-                    p_err = fma(w * d, d, p_err);
-                    p_ce = fma(w * cv[u], ev[u], p_ce);
-                }
-                if (!diag) {
-                    *reinterpret_cast<double2*>(Out + (size_t)row * ld + col) = make_double2(o[0], o[1]);
-                    Out[(size_t)col * ld + row] = o[0];
-                    Out[(size_t)(col + 1) * ld + row] = o[1];
-                } else {
+                    const double2 e2 = __ldcg(reinterpret_cast<const double2*>(E + (size_t)row * ld + col));
+                    const double ev[2] = {e2.x, e2.y};
+                    double o[2];
 #pragma unroll
                     for (int u = 0; u < 2; ++u) {
-                        if (col + u >= row) Out[(size_t)row * ld + col + u] = o[u];
-                        if (col + u > row) Out[(size_t)(col + u) * ld + row] = o[u];
+                        double v = fma(c2, cv[u], c1 * ev[u]);
+                        const double d = cv[u] - ev[u];
+                        double w = 1.0;
+                        if (diag) {
+                            const int cc = col + u;
+                            w = (cc > row) ? 2.0 : ((cc == row) ? 1.0 : 0.0);
+                            if (cc == row) {
+                                if (row < p.kvalid) v += c0;
+                                p_tr += v;
+                                p_trc += cv[u];
+                            }
+                        }
+                        o[u] = v;
+                        p_ss = fma(w * v, v, p_ss);
+                        p_err = fma(w * d, d, p_err);
+                        p_ce = fma(w * cv[u], ev[u], p_ce);
+                    }
+                    if (!diag) {
+                        *reinterpret_cast<double2*>(Out + (size_t)row * ld + col) = make_double2(o[0], o[1]);
+                        Out[(size_t)col * ld + row] = o[0];
+                        Out[(size_t)(col + 1) * ld + row] = o[1];
+                    } else {
+#pragma unroll
+                        for (int u = 0; u < 2; ++u) {
+                            if (col + u >= row) Out[(size_t)row * ld + col + u] = o[u];
+                            if (col + u > row) Out[(size_t)(col + u) * ld + row] = o[u];
+                        }
                     }
                 }
             }

@@ -63,6 +63,7 @@ struct rfoe_handle_s {
     int* d_word = nullptr; // device alias of hp->word
     // the whole recursion in one persistent launch (resident.cuh)
     int coop_ok = 0;           // cooperative launch supported and one CTA of the kernel fits an SM
+    int side_by_side = 0;      // set by rfoe_expand_many while several handles work side by side (see expand_impl)
     int rs_m = 0, rs_G = 0, rs_n_split = 0, rs_tile_cost = 0;   // the plan the split list / records were set up for
     int4* d_split = nullptr;
     double* d_rec[2] = {nullptr, nullptr};
@@ -117,17 +118,18 @@ static int hbm_grid(const rfoe_handle_s* h, int rows)
     return want < cap ? (want < 1 ? 1 : want) : cap;
 }
 
-// Upper-triangle tile order: G x G super-blocks walked row-major, so that the ~148 CTAs resident at
-// any time share about 2G row panels and stream them through L2 together.
+// Upper-triangle tile order: strips of G tile rows, each walked COLUMN by column (j outer, i inner).  The ~148 CTAs resident
+// at any time then cover G rows x ~12.3 consecutive columns wherever the window falls: 2 G + 0.3 row panels streamed
+// through L2 together.  (Round 1 walked G x G super-blocks row-major; a window straddling two super-blocks touched up to
+// 36 panels instead of 24, which is the 34.7 GB of DRAM reads per squaring ncu showed at k=16384 against a 22.9 GB floor.)
 static void build_tile_order(int m, std::vector<int2>& out)
 {
     const int G = 12;
     out.clear();
     out.reserve((size_t)m * (m + 1) / 2);
     for (int SI = 0; SI < m; SI += G)
-        for (int SJ = SI; SJ < m; SJ += G)
-            for (int i = SI; i < SI + G && i < m; ++i)
-                for (int j = (SJ > i ? SJ : i); j < SJ + G && j < m; ++j) out.push_back(make_int2(i, j));
+        for (int j = SI; j < m; ++j)
+            for (int i = SI; i < SI + G && i <= j; ++i) out.push_back(make_int2(i, j));
 }
 
 static int ensure_tiles(rfoe_handle_s* h, int m, cudaStream_t st)
@@ -401,7 +403,8 @@ extern "C" int rfoe_create(rfoe_handle_t* out, int device, int64_t k_max)
         cudaFuncSetAttribute(sym_square_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, SQ_SMEM_BYTES) != cudaSuccess ||
         cudaFuncSetAttribute(sym_square_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, SQ_SMEM_BYTES) != cudaSuccess ||
         cudaFuncSetAttribute(resident_recursion_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, RS_SMEM_BYTES) != cudaSuccess ||
-        cudaFuncSetAttribute(resident_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, RT_SMEM_BYTES) != cudaSuccess ||
+        cudaFuncSetAttribute(resident_small_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, RT_SMEM_BYTES) != cudaSuccess ||
+        cudaFuncSetAttribute(resident_small_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, RT_SMEM_BYTES) != cudaSuccess ||
         cudaFuncSetAttribute(apply_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, AP_SMEM_BYTES) != cudaSuccess ||
         cudaFuncSetAttribute(sym_square_reduced_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TQ_SMEM_BYTES) != cudaSuccess) {
         rfoe_destroy(h);
@@ -411,8 +414,9 @@ extern "C" int rfoe_create(rfoe_handle_t* out, int device, int64_t k_max)
         int coop = 0, per_sm = 0;
         if (cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, device) == cudaSuccess && coop &&
             cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, resident_recursion_kernel, SQ_THREADS, RS_SMEM_BYTES) == cudaSuccess &&
-            per_sm >= 1 && h->sm_count <= 256 && (RT_MAX_N / RT_BM) * (RT_MAX_N / RT_BM + 1) / 2 <= h->sm_count &&
-            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, resident_small_kernel, SQ_THREADS, RT_SMEM_BYTES) == cudaSuccess && per_sm >= 1)
+            per_sm >= 1 && h->sm_count <= 256 && (RT_MAX_N / 64) * (RT_MAX_N / 64 + 1) / 2 <= h->sm_count &&
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, resident_small_kernel<32>, SQ_THREADS, RT_SMEM_BYTES) == cudaSuccess && per_sm >= 1 &&
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, resident_small_kernel<64>, SQ_THREADS, RT_SMEM_BYTES) == cudaSuccess && per_sm >= 1)
             h->coop_ok = 1;
         cudaGetLastError();
     }
@@ -753,7 +757,11 @@ static int expand_impl(rfoe_handle_t h, const double* Hp, int64_t k64, int64_t n
             if ((rc = make_map_parts(h, &tmF[i], h->F[i], n, n + TQ_PAD)) != RFOE_OK) return fail(rc);
 
     // the whole recursion in one persistent launch when the problem is small enough to live on chip (resident.cuh)
-    const bool use_resident = h->resident && h->coop_ok && !sh && n <= RS_MAX_N &&
+    // (Several handles side by side, rfoe_expand_many: persistent launches of one CTA per SM cannot overlap, launch-per-step
+    // kernels of different handles can and fill each other's idle SMs and sync gaps -- measured at k=2048, 4 handles: 91 against
+    // 81 expansions/s.  So mid-size problems keep the launch-per-step path there; the latency-bound sizes do not, the small
+    // persistent kernel being 3x faster than anything overlap could recover.)
+    const bool use_resident = h->resident && h->coop_ok && !sh && n <= RS_MAX_N && !(h->side_by_side && n > RT_MAX_N) &&
                               (variant == RFOE_VARIANT_SP2 || variant == RFOE_VARIANT_SP2_ACCEL || variant == RFOE_VARIANT_TRUNC);
     const bool use_small = use_resident && n <= RT_MAX_N;      // latency-bound sizes: 32 x 32 tiles, one grid barrier per step
     if (use_resident && !use_small) {
@@ -829,16 +837,18 @@ static int expand_impl(rfoe_handle_t h, const double* Hp, int64_t k64, int64_t n
         CK(cudaMemsetAsync(h->d_flags, 0, 256 * sizeof(unsigned), st));
         CK(cudaMemsetAsync(h->d_timing, 0, 8 * sizeof(unsigned long long), st));
         if (use_small) {
+            const int bm = (n <= RT_MAX_N32) ? 32 : 64;
             CUtensorMap ts[2];
             for (int i = 0; i < 2; ++i)
-                if ((rc = make_map(h, &ts[i], h->W[i], n, ld, RT_BM)) != RFOE_OK) return fail(rc);
+                if ((rc = make_map(h, &ts[i], h->W[i], n, ld, bm)) != RFOE_OK) return fail(rc);
             SmallPlan sp = {};
-            sp.n = n; sp.ld = ld; sp.kvalid = k; sp.m32 = n / RT_BM;
-            sp.n_tiles = sp.m32 * (sp.m32 + 1) / 2;
+            sp.n = n; sp.ld = ld; sp.kvalid = k; sp.mt = n / bm;
+            sp.n_tiles = sp.mt * (sp.mt + 1) / 2;
             sp.W0 = h->W[0]; sp.W1 = h->W[1]; sp.rec0 = h->d_rec[0]; sp.rec1 = h->d_rec[1];
             sp.flags = h->d_flags; sp.ctrl = h->d_ctrl; sp.timing = h->d_timing;
             void* args[3] = {(void*)&ts[0], (void*)&ts[1], (void*)&sp};
-            CK(cudaLaunchCooperativeKernel((const void*)resident_small_kernel, dim3(sp.n_tiles), dim3(SQ_THREADS), args, RT_SMEM_BYTES, st));
+            CK(cudaLaunchCooperativeKernel(bm == 32 ? (const void*)resident_small_kernel<32> : (const void*)resident_small_kernel<64>,
+                                           dim3(sp.n_tiles), dim3(SQ_THREADS), args, RT_SMEM_BYTES, st));
         } else {
             void* args[3] = {(void*)&tm[0], (void*)&tm[1], (void*)&rp};
             CK(cudaLaunchCooperativeKernel((const void*)resident_recursion_kernel, dim3(h->rs_G), dim3(SQ_THREADS), args, RS_SMEM_BYTES, st));
@@ -1005,6 +1015,7 @@ extern "C" int rfoe_expand_many(const rfoe_handle_t* handles, const rfoe_stream_
         }
     };
     const int n_threads = n_handles < n_problems ? n_handles : n_problems;
+    for (int i = 0; i < n_handles; ++i) handles[i]->side_by_side = (n_threads > 1);
     std::vector<std::thread> pool;
     try {
         for (int i = 1; i < n_threads; ++i) pool.emplace_back(worker, i);
@@ -1013,6 +1024,7 @@ extern "C" int rfoe_expand_many(const rfoe_handle_t* handles, const rfoe_stream_
     }
     if (n_threads > 0) worker(0);
     for (std::thread& t : pool) t.join();
+    for (int i = 0; i < n_handles; ++i) handles[i]->side_by_side = 0;
     int first = RFOE_OK;
     for (int j = 0; j < n_problems; ++j) {
         if (status) status[j] = rcs[j];

@@ -70,9 +70,9 @@ int main(int argc, char** argv)
     if (!f || fwrite(P, 1, bytes, f) != bytes) return 5;
     fclose(f);
     printf("status=%d iterations=%d converged=%d branch=%s eps_min=%.17g eps_max=%.17g bounds_min=%.17g bounds_max=%.17g "
-           "tr_PH=%.17g t_last=%.17g launches=%lld hl_status=%d homo=%.17g lumo=%.17g\n",
+           "tr_PH=%.17g t_last=%.17g launches=%lld resident=%d hl_status=%d homo=%.17g lumo=%.17g\n",
            rc, st.iterations, st.converged, st.branch, st.eps_min, st.eps_max, emin, emax, st.tr_PH, st.t[st.iterations],
-           (long long)st.gpu_launches, rc_hl, homo, lumo);
+           (long long)st.gpu_launches, st.resident, rc_hl, homo, lumo);
 
     rc = rfoe_destroy(h);
     if (rc != RFOE_OK) return fail("rfoe_destroy", rc);

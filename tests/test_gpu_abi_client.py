@@ -38,7 +38,8 @@ def test_c_client_matches_oracle(tmp_path, k):
     assert np.linalg.norm(P - ref.P) / math.sqrt(k) <= 1e-10
     assert abs(float(kv["tr_PH"]) - ref.tr_PH) <= 1e-11 * abs(ref.tr_PH)
     assert np.array_equal(P, P.T) and round(float(kv["t_last"])) == nocc
-    assert int(kv["launches"]) >= ref.iterations
+    # k <= 4096: the recursion is one persistent launch (stats.resident); otherwise at least one launch per step
+    assert int(kv["launches"]) >= (5 if int(kv["resident"]) else ref.iterations)
     oh, ol = oracle.estimate_homo_lumo(ref, nocc)
     assert int(kv["hl_status"]) == 0
     assert float(kv["homo"]) == pytest.approx(oh, abs=1e-8 * (hi - lo)) and float(kv["lumo"]) == pytest.approx(ol, abs=1e-8 * (hi - lo))
