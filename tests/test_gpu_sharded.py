@@ -180,8 +180,16 @@ def _ipc_worker(rank, world, port, k, c, out):
     H = torch.from_numpy(w.H).cuda()
     with rfoe.Rfoe(k) as h:
         h.shard_connect()
+        first = h.expand_sharded_p2p(H, w.nocc, rfoe.SP2, w.tol)
+        P_first = first.P.clone()
+        # a second expansion straight after the first, one rank late: the entry barrier of rfoe_expand_sharded_p2p must keep
+        # the early rank's first stores out of buffers the late rank's previous call could still be reading
+        if rank == 1:
+            import time
+            time.sleep(0.05)
         res = h.expand_sharded_p2p(H, w.nocc, rfoe.SP2, w.tol)
         torch.cuda.synchronize()
+        out[f"repeat{rank}"] = bool(torch.equal(res.P, P_first)) and res.branch == first.branch
         dist.barrier()
         if rank == 0:
             h.configure(resident=False)
@@ -209,7 +217,7 @@ def test_p2p_sharded_two_processes_ipc_handles():
         mp.spawn(_ipc_worker, args=(world, port, k, c, out), nprocs=world, join=True)
         res = dict(out)
     w = rfoe_inputs.make_workload(c, k=k)
-    assert res["equal"]
+    assert res["equal"] and res["repeat0"] and res["repeat1"]      # the second of two back-to-back calls gives the same bits
     for r in range(world):
         it, br, conv, tr = res[r]
         assert conv and (it, br) == res["single"] and abs(tr - w.nocc) < 1e-9
