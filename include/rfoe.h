@@ -284,6 +284,20 @@ int rfoe_shard_range(int64_t n_tiles, int rank, int world, int64_t* begin, int64
  * empty last wave fills the SMs (slices = 1: no tail, plain launch).  DESIGN.md "Tail of a launch". */
 int rfoe_plan_squaring(int64_t k, int sm_count, int64_t* n_tiles, int64_t* n_main, int* slices, int* kt_per_slice);
 
+/* Host-only introspection (no device needed): how rfoe_expand runs the recursion of a k x k problem on a GPU with sm_count
+ * SMs when RFOE_OPT_RESIDENT is on (variants SP2, SP2_ACCEL, TRUNC).  DESIGN.md section 13.
+ *   path      0: one launch sequence per recursion step (k > 4096, or too few SMs)
+ *             1 / 2: the whole recursion in one persistent launch of `grid` CTAs, one 32 x 32 (k <= 512) / 64 x 64
+ *                (k <= 1024) output tile each with the whole contraction
+ *             3: one persistent launch of `grid` CTAs sharing the n_tiles x kt chunk units (128 x 128 tile, 16-wide slice
+ *                of the contraction) of a step in contiguous ranges of equal cost (stream-K)
+ *   path 3 only: kt = chunks per tile; boundaries (grid + 1 ints, may be null): CTA b works on chunk units
+ *             [boundaries[b], boundaries[b+1]) of the stream tile 0 chunks 0..kt-1, tile 1, ...; n_split = tiles not wholly
+ *             inside one range, finished in the fix-up phase; split_tiles (3 ints per split tile, may be null; at most
+ *             3 * grid + 3): tile, first CTA holding a segment of it, number of CTAs holding one. */
+int rfoe_plan_resident(int64_t k, int sm_count, int* path, int* grid, int* kt, int64_t* n_tiles, int* n_split,
+                       int* boundaries, int* split_tiles);
+
 /* HOMO / LUMO estimates for A-Z-RFOE from the history of a finished Z-RFOE run (host only, no device needed).
  * The paper chooses the accelerated polynomials "based on HOMO ... and LUMO ... eigenvalues" and does not
  * say where they come from; in an SCF loop they come from the previous expansion (its refs. 31, 38; DESIGN.md reading

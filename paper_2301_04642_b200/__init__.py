@@ -32,7 +32,7 @@ MAX_STEPS = 256
 
 # every symbol include/rfoe.h declares
 EXPORTS = ("rfoe_create", "rfoe_bounds", "rfoe_bounds_lanczos", "rfoe_expand", "rfoe_expand_host", "rfoe_square", "rfoe_square_reduced",
-           "rfoe_symm_product", "rfoe_probe_fp64_peak", "rfoe_project", "rfoe_apply", "rfoe_expand_sharded", "rfoe_shard_range", "rfoe_plan_squaring",
+           "rfoe_symm_product", "rfoe_probe_fp64_peak", "rfoe_project", "rfoe_apply", "rfoe_expand_sharded", "rfoe_shard_range", "rfoe_plan_squaring", "rfoe_plan_resident",
            "rfoe_shard_local_ptrs", "rfoe_shard_set_peers", "rfoe_shard_ipc_export", "rfoe_shard_ipc_import",
            "rfoe_expand_sharded_p2p", "rfoe_expand_many",
            "rfoe_estimate_homo_lumo", "rfoe_set_option", "rfoe_get_stats", "rfoe_destroy", "rfoe_strerror", "rfoe_version")
@@ -104,6 +104,8 @@ def load_library(path: str | None = None):
     L.rfoe_expand_many.argtypes = [C.POINTER(vp), C.POINTER(vp), C.c_int, C.c_int, C.POINTER(vp), C.POINTER(i64), C.POINTER(i64),
                                    C.c_int, dp, C.POINTER(vp), C.POINTER(C.c_int), C.POINTER(_Stats)]
     L.rfoe_plan_squaring.argtypes = [i64, C.c_int, C.POINTER(i64), C.POINTER(i64), C.POINTER(C.c_int), C.POINTER(C.c_int)]
+    L.rfoe_plan_resident.argtypes = [i64, C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(i64),
+                                     C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_int)]
     L.rfoe_shard_range.argtypes = [i64, C.c_int, C.c_int, C.POINTER(i64), C.POINTER(i64)]
     L.rfoe_set_option.argtypes = [vp, C.c_int, dbl]
     L.rfoe_get_stats.argtypes = [vp, C.POINTER(_Stats)]
@@ -235,6 +237,22 @@ def plan_squaring(k: int, sm_count: int = 148):
     if rc != OK:
         raise RfoeError(rc, "rfoe_plan_squaring: invalid argument")
     return nt.value, nm.value, sl.value, per.value
+
+
+def plan_resident(k: int, sm_count: int = 148):
+    """rfoe_plan_resident (host-only C call): dict(path, grid, kt, n_tiles, n_split, boundaries, split_tiles)."""
+    path, grid, kt, ns = C.c_int(), C.c_int(), C.c_int(), C.c_int()
+    nt = C.c_int64()
+    bounds = (C.c_int * (sm_count + 2))()
+    split = (C.c_int * (3 * sm_count + 6))()
+    rc = load_library().rfoe_plan_resident(int(k), int(sm_count), C.byref(path), C.byref(grid), C.byref(kt), C.byref(nt), C.byref(ns),
+                                           bounds, split)
+    if rc != OK:
+        raise RfoeError(rc, "rfoe_plan_resident: invalid argument")
+    g = grid.value
+    return dict(path=path.value, grid=g, kt=kt.value, n_tiles=nt.value, n_split=ns.value,
+                boundaries=list(bounds[: g + 1]) if path.value == 3 else [],
+                split_tiles=[tuple(split[3 * i: 3 * i + 3]) for i in range(ns.value)] if path.value == 3 else [])
 
 
 def shard_range(n_tiles: int, rank: int, world: int):

@@ -637,40 +637,84 @@ static int host_boundary(long long cost_total, int tile_cost, int KT, int G, int
     return tile * KT + (off < KT ? off : KT);
 }
 
-static int ensure_resident_plan(rfoe_handle_s* h, int m, int KT, cudaStream_t st)
+struct ResidentHostPlan {
+    int G = 0, tile_cost = 0;
+    std::vector<int4> split;     // (tile, first CTA holding a segment of it, number of segments, 0)
+};
+
+// pure host arithmetic (no device): also behind rfoe_plan_resident, so that CPU tests can check the partition
+static ResidentHostPlan compute_resident_plan(int n_tiles, int KT, int sm_count)
 {
-    const long long U = (long long)h->n_tiles * KT;
-    const int G = (int)(U < h->sm_count ? U : h->sm_count);
-    if (h->rs_m == m && h->rs_G == G) return RFOE_OK;
+    ResidentHostPlan pl;
+    const long long U = (long long)n_tiles * KT;
+    const int G = (int)(U < sm_count ? U : sm_count);
     // register epilogues are counted into the ranges only where a CTA holds several whole tiles; where nearly every tile
     // is split (FIX finishes those) the ranges are equal in chunk units
     int tile_cost = (U / G >= 2LL * KT) ? KT + RS_EPI_COST : KT;
-    std::vector<int4> split;
     for (int attempt = 0; attempt < 2; ++attempt) {
-        const long long total = (long long)h->n_tiles * tile_cost;
+        const long long total = (long long)n_tiles * tile_cost;
         bool empty = false;
         for (int b = 0; b < G && !empty; ++b) empty = host_boundary(total, tile_cost, KT, G, b + 1) <= host_boundary(total, tile_cost, KT, G, b);
         if (empty && tile_cost != KT) { tile_cost = KT; continue; }      // (cannot happen with ranges >= 2 tiles; belt and braces)
-        split.clear();
+        pl.split.clear();
         int b = 0;
-        for (int t = 0; t < h->n_tiles; ++t) {
+        for (int t = 0; t < n_tiles; ++t) {
             const int t0 = t * KT, t1 = t0 + KT;
             while (host_boundary(total, tile_cost, KT, G, b + 1) <= t0) ++b;          // b: the CTA whose range holds unit t0
             if (host_boundary(total, tile_cost, KT, G, b + 1) >= t1) continue;         // whole: register epilogue in MM
             int nseg = 1;
             while (host_boundary(total, tile_cost, KT, G, b + nseg) < t1) ++nseg;      // CTAs b .. b + nseg - 1 hold its segments
-            split.push_back(make_int4(t, b, nseg, 0));
+            pl.split.push_back(make_int4(t, b, nseg, 0));
         }
         break;
     }
+    pl.G = G; pl.tile_cost = tile_cost;
+    return pl;
+}
+
+static int ensure_resident_plan(rfoe_handle_s* h, int m, int KT, cudaStream_t st)
+{
+    const long long U = (long long)h->n_tiles * KT;
+    const int G = (int)(U < h->sm_count ? U : h->sm_count);
+    if (h->rs_m == m && h->rs_G == G) return RFOE_OK;
+    const ResidentHostPlan pl = compute_resident_plan(h->n_tiles, KT, h->sm_count);
+    const std::vector<int4>& split = pl.split;
     if ((int)split.size() > RS_MAX_SPLIT) return RFOE_ERR_UNSUPPORTED;
     h->rs_m = 0;
     if (!split.empty()) CK(cudaMemcpyAsync(h->d_split, split.data(), split.size() * sizeof(int4), cudaMemcpyHostToDevice, st));
-    const size_t nrec = (size_t)h->n_tiles + (size_t)G;
+    const size_t nrec = (size_t)h->n_tiles + (size_t)pl.G;
     CK(cudaMemsetAsync(h->d_rec[0], 0, nrec * SQ_NPART * sizeof(double), st));   // the tile records of split tiles stay zero
     CK(cudaMemsetAsync(h->d_rec[1], 0, nrec * SQ_NPART * sizeof(double), st));
     CK(cudaStreamSynchronize(st));   // `split` is pageable and dies here
-    h->rs_m = m; h->rs_G = G; h->rs_n_split = (int)split.size(); h->rs_tile_cost = tile_cost;
+    h->rs_m = m; h->rs_G = pl.G; h->rs_n_split = (int)split.size(); h->rs_tile_cost = pl.tile_cost;
+    return RFOE_OK;
+}
+
+extern "C" int rfoe_plan_resident(int64_t k, int sm_count, int* path, int* grid, int* kt, int64_t* n_tiles, int* n_split,
+                                  int* boundaries, int* split_tiles)
+{
+    if (k < 1 || k > (1 << 20) || sm_count < 1 || sm_count > 256 || !path || !grid || !kt || !n_tiles || !n_split) return RFOE_ERR_INVALID_ARG;
+    const int n = round_up(k, SQ_BM);
+    *kt = 0; *n_split = 0;
+    if (n > RS_MAX_N) { *path = 0; *grid = 0; *n_tiles = (int64_t)(n / SQ_BM) * (n / SQ_BM + 1) / 2; return RFOE_OK; }
+    if (n <= RT_MAX_N) {
+        const int bm = (n <= RT_MAX_N32) ? 32 : 64, mt = n / bm;
+        *path = (bm == 32) ? 1 : 2;
+        *n_tiles = (int64_t)mt * (mt + 1) / 2;
+        *grid = (int)*n_tiles;
+        if (*grid > sm_count) { *path = 0; *grid = 0; }      // (the library requires one CTA per tile to be co-resident)
+        return RFOE_OK;
+    }
+    const int m = n / SQ_BM, nt = m * (m + 1) / 2, KT = n / SQ_BK;
+    const ResidentHostPlan pl = compute_resident_plan(nt, KT, sm_count);
+    *path = 3; *grid = pl.G; *kt = KT; *n_tiles = nt; *n_split = (int)pl.split.size();
+    const long long total = (long long)nt * pl.tile_cost;
+    if (boundaries)
+        for (int b = 0; b <= pl.G; ++b) boundaries[b] = host_boundary(total, pl.tile_cost, KT, pl.G, b);
+    if (split_tiles)
+        for (size_t i = 0; i < pl.split.size(); ++i) {
+            split_tiles[3 * i] = pl.split[i].x; split_tiles[3 * i + 1] = pl.split[i].y; split_tiles[3 * i + 2] = pl.split[i].z;
+        }
     return RFOE_OK;
 }
 
