@@ -16,8 +16,11 @@
 // + c0 I written to (I,J) and mirrored, five FP64 partial sums per tile -- so the recursion, its
 // scalars and its control flow are unchanged; only the product is reduced precision.
 //
-// Roles (192 threads): warp 0 = TMA producer, warp 1 = TMEM allocator + MMA issuer (both warps stay converged
-// and one elected lane issues, so the TMA / tcgen05 operands live in uniform registers), warps 2..5 = epilogue (each reads its own 32 TMEM lanes = 32 tile rows).
+// Roles (320 threads): warp 0 = TMA producer, warp 1 = TMEM allocator + MMA issuer (both warps stay converged
+// and one elected lane issues, so the TMA / tcgen05 operands live in uniform registers), warps 2..9 = epilogue: warp w reads
+// the 32 TMEM lanes (tile rows) of quarter w % 4 and owns 64 of the tile's 128 columns (two warps per quarter: 64 FP32 head
+// sums per thread instead of 128 -- no spills -- and twice the threads behind the FP64 epilogue's memory latency; round 1's
+// four warps spent 38 % of the kernel there at k=8192).
 // Clusters of two CTAs own the tiles (I, J0) and (I, J0+1): they share the row panels Zh(I), Zl(I), each
 // CTA fetches half of them and TMA-multicasts it to both (25 % fewer L2 requests per CTA; measured: no
 // change in time -- the kernel runs into the 1 kW power cap).
@@ -60,7 +63,12 @@ constexpr double TQ_UNSCALE_CROSS = 1.0 / (TQ_SCALE_HI * TQ_SCALE_LO);
 constexpr int TQ_BM = 128;                 // tile rows = cols (UMMA M = N = 128, cta_group::1)
 constexpr int TQ_BK = 128 / (int)sizeof(tq_elem_t);   // elements per K chunk = one 128-byte swizzle row (32 tf32 / 64 f16)
 constexpr int TQ_STAGES = 3;
-constexpr int TQ_THREADS = 192;
+#ifndef TQ_EPI_WARPS_N
+#define TQ_EPI_WARPS_N 8
+#endif
+constexpr int TQ_EPI_WARPS = TQ_EPI_WARPS_N;             // 4 TMEM lane quarters x (TQ_EPI_WARPS / 4) column ranges
+constexpr int TQ_THREADS = 64 + 32 * TQ_EPI_WARPS;
+constexpr int TQ_EPI_COLS = TQ_BM / (TQ_EPI_WARPS / 4);  // columns per epilogue warp
 constexpr int TQ_PANEL_BYTES = TQ_BM * 128;                       // 16 KiB
 constexpr int TQ_STAGE_BYTES = 4 * TQ_PANEL_BYTES;               // A_hi, A_lo, B_hi, B_lo
 constexpr int TQ_SMEM_BYTES = TQ_STAGES * TQ_STAGE_BYTES + 1024; // + slack for 1024-byte alignment
@@ -130,7 +138,7 @@ sym_square_reduced_kernel(const __grid_constant__ CUtensorMap tmHi, const __grid
     __shared__ __align__(8) uint64_t hfull_bar[2];    // head accumulator b holds a finished chunk
     __shared__ __align__(8) uint64_t hempty_bar[2];   // head accumulator b has been drained
     __shared__ uint32_t tmem_base_sh;
-    __shared__ double red[4][5];
+    __shared__ double red[TQ_EPI_WARPS][5];
 
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
@@ -154,7 +162,7 @@ sym_square_reduced_kernel(const __grid_constant__ CUtensorMap tmHi, const __grid
         }
         for (int b = 0; b < 2; ++b) {
             mbar_init(hfull0 + 8 * b, 1);
-            mbar_init(hempty0 + 8 * b, 4);     // lane 0 of each of the four epilogue warps
+            mbar_init(hempty0 + 8 * b, TQ_EPI_WARPS);     // lane 0 of each epilogue warp
         }
         mbar_fence_init();
         tma_prefetch_desc(&tmHi);
@@ -236,10 +244,12 @@ sym_square_reduced_kernel(const __grid_constant__ CUtensorMap tmHi, const __grid
     } else {
         // ===== epilogue warps: TMEM -> registers -> fused FP64 update, mirror, partial sums =====
         const int q = warp & 3;                   // TMEM lane quarter this warp may access
+        const int ew = warp - 2;                  // 0..7
+        const int c_lo = (ew >> 2) * TQ_EPI_COLS; // this warp's 64 columns of the tile
         const int row = I * TQ_BM + q * 32 + lane;
         const uint32_t trow = tmem + ((uint32_t)(q * 32) << 16);
         // ---- drain the head accumulator chunk by chunk into FP32 register sums (round-to-nearest adds)
-        float hsum[TQ_BM];
+        float hsum[TQ_EPI_COLS];
         const int NC = (KT + TQ_CHUNK_KT - 1) / TQ_CHUNK_KT;
 #pragma unroll 1
         for (int ch = 0; ch < NC; ++ch) {
@@ -247,9 +257,9 @@ sym_square_reduced_kernel(const __grid_constant__ CUtensorMap tmHi, const __grid
             mbar_wait_bounded(hfull0 + 8 * hb, (uint32_t)(ch >> 1) & 1u);
             tc_fence_after();
 #pragma unroll
-            for (int cb = 0; cb < TQ_BM; cb += 16) {
+            for (int cb = 0; cb < TQ_EPI_COLS; cb += 16) {
                 float v[16];
-                tmem_ld16(trow + hb * TQ_BM + cb, v);
+                tmem_ld16(trow + hb * TQ_BM + c_lo + cb, v);
 #pragma unroll
                 for (int u = 0; u < 16; ++u) hsum[cb + u] = (ch == 0) ? v[u] : __fadd_rn(hsum[cb + u], v[u]);
             }
@@ -259,24 +269,50 @@ sym_square_reduced_kernel(const __grid_constant__ CUtensorMap tmHi, const __grid
         }
         // ---- the last chunk's commit also covers every cross-term MMA: finish in FP64
         if (phantom) {
-            if (lane == 0) { red[q][0] = red[q][1] = red[q][2] = red[q][3] = red[q][4] = 0.0; }
+            if (lane == 0) { red[ew][0] = red[ew][1] = red[ew][2] = red[ew][3] = red[ew][4] = 0.0; }
         } else {
         const double d = *trace / (double)kvalid;
         const double c2 = coef->c2, c1 = coef->c1, c0 = coef->c0;
         double p_tr = 0.0, p_ss = 0.0, p_err = 0.0, p_trc = 0.0, p_ce = 0.0;
-        const double* erow = E + (size_t)row * ld + (size_t)J * TQ_BM;
-        double* orow = Out + (size_t)row * ld + (size_t)J * TQ_BM;
+        const double* erow = E + (size_t)row * ld + (size_t)J * TQ_BM + c_lo;
+        double* orow = Out + (size_t)row * ld + (size_t)J * TQ_BM + c_lo;
+        // Global accesses of the 32 x 16 block a warp handles per step go through a staging patch in the operand ring (free
+        // by now: the last commit covers every MMA of this CTA, and the peer's multicasts into this CTA were needed by them):
+        // with lane = row (the TMEM layout) a 16-byte load or store touches 32 rows -- 32 sectors for 512 bytes; staged, 8
+        // lanes cover one row's 128 bytes and an instruction covers 4 whole rows.  Patch layout: element (r, c) at
+        // r * 16 + 2 * ((c / 2) ^ (r & 7)) + (c & 1): conflict-free 16-byte accesses both by row (lane = r) and by quarter
+        // warp (8 lanes = one row).
+        double* const stg_e = reinterpret_cast<double*>(smem_raw + (smem_base - smem_u32(smem_raw))) + ew * 1024;
+        double* const stg_o = stg_e + 512;
+        const int srow = lane >> 3, sch = lane & 7;            // coalesced side: row inside a group of 4, 16-byte chunk of the row
+        const double* eblk = E + (size_t)(I * TQ_BM + q * 32) * ld + (size_t)J * TQ_BM + c_lo;
+        double* oblk = Out + (size_t)(I * TQ_BM + q * 32) * ld + (size_t)J * TQ_BM + c_lo;
 #pragma unroll
-        for (int cb = 0; cb < TQ_BM; cb += 16) {
+        for (int cb = 0; cb < TQ_EPI_COLS; cb += 16) {
             float xx[16];
-            tmem_ld16(trow + 2 * TQ_BM + cb, xx);
+            tmem_ld16(trow + 2 * TQ_BM + c_lo + cb, xx);
             double ev[16], o[16];
+            if (!diag) {
 #pragma unroll
-            for (int u = 0; u < 16; u += 2) {
-                const double2 e2 = *reinterpret_cast<const double2*>(erow + cb + u);
-                ev[u] = e2.x; ev[u + 1] = e2.y;
+                for (int i = 0; i < 8; ++i) {
+                    const int rr = 4 * i + srow;
+                    const double2 v = *reinterpret_cast<const double2*>(eblk + (size_t)rr * ld + cb + 2 * sch);
+                    *reinterpret_cast<double2*>(stg_e + rr * 16 + 2 * (sch ^ (rr & 7))) = v;
+                }
+                __syncwarp();
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                    const double2 e2 = *reinterpret_cast<const double2*>(stg_e + lane * 16 + 2 * (j ^ (lane & 7)));
+                    ev[2 * j] = e2.x; ev[2 * j + 1] = e2.y;
+                }
+            } else {
+#pragma unroll
+                for (int u = 0; u < 16; u += 2) {
+                    const double2 e2 = *reinterpret_cast<const double2*>(erow + cb + u);
+                    ev[u] = e2.x; ev[u + 1] = e2.y;
+                }
             }
-            const int col = J * TQ_BM + cb;
+            const int col = J * TQ_BM + c_lo + cb;
 #pragma unroll
             for (int u = 0; u < 16; ++u) {
                 // X^2 = Z^2 + 2 d X - d^2 I   (Z = X - d I on rows < kvalid)
@@ -305,9 +341,18 @@ sym_square_reduced_kernel(const __grid_constant__ CUtensorMap tmHi, const __grid
             }
             if (!diag) {
 #pragma unroll
-                for (int u = 0; u < 16; u += 2) *reinterpret_cast<double2*>(orow + cb + u) = make_double2(o[u], o[u + 1]);
+                for (int j = 0; j < 8; ++j)
+                    *reinterpret_cast<double2*>(stg_o + lane * 16 + 2 * (j ^ (lane & 7))) = make_double2(o[2 * j], o[2 * j + 1]);
 #pragma unroll
                 for (int u = 0; u < 16; ++u) Out[(size_t)(col + u) * ld + row] = o[u];   // mirror: lanes = consecutive rows
+                __syncwarp();
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    const int rr = 4 * i + srow;
+                    const double2 v = *reinterpret_cast<const double2*>(stg_o + rr * 16 + 2 * (sch ^ (rr & 7)));
+                    *reinterpret_cast<double2*>(oblk + (size_t)rr * ld + cb + 2 * sch) = v;
+                }
+                __syncwarp();
             } else {
 #pragma unroll
                 for (int u = 0; u < 16; ++u) {
@@ -326,7 +371,7 @@ sym_square_reduced_kernel(const __grid_constant__ CUtensorMap tmHi, const __grid
             p_ce += __shfl_xor_sync(0xffffffffu, p_ce, m);
         }
         if (lane == 0) {
-            red[q][0] = p_tr; red[q][1] = p_ss; red[q][2] = p_err; red[q][3] = p_trc; red[q][4] = p_ce;
+            red[ew][0] = p_tr; red[ew][1] = p_ss; red[ew][2] = p_err; red[ew][3] = p_trc; red[ew][4] = p_ce;
         }
         }
     }
@@ -335,8 +380,12 @@ sym_square_reduced_kernel(const __grid_constant__ CUtensorMap tmHi, const __grid
     cluster_sync_all();                         // the peer's commits / multicasts into this CTA are over
     if (warp == 1) tmem_dealloc<TQ_TMEM_COLS>(tmem);
     if (threadIdx.x < 5)
-        partials[(size_t)blockIdx.x * SQ_NPART + threadIdx.x] =
-            (red[0][threadIdx.x] + red[1][threadIdx.x]) + (red[2][threadIdx.x] + red[3][threadIdx.x]);
+    {
+        double v = 0.0;
+#pragma unroll
+        for (int w = 0; w < TQ_EPI_WARPS; ++w) v += red[w][threadIdx.x];      // fixed order
+        partials[(size_t)blockIdx.x * SQ_NPART + threadIdx.x] = v;
+    }
 }
 
 }  // namespace rfoe
