@@ -501,7 +501,7 @@ def hbm_report(h, H, stream):
         pass
     gbs = 8.0 * k * k / (best * 1e-3) / 1e9
     return {"rfoe_bounds_ms": best, "gershgorin_gbs": gbs, "peak_gbs": peak, "frac": gbs / peak if peak else None,
-            "note": "whole rfoe_bounds call (rows kernel + reduction + 16-byte D2H); per-kernel figures: profiles/r01f_launches_k16384.md"}
+            "note": "whole rfoe_bounds call (rows kernel + reduction + 16-byte D2H); per-kernel figures: profiles/r02_launches_k16384.md"}
 
 
 def lanczos_report(h, rfoe, w, H, P, stream, fp64_ms, m=24):
