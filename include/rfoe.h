@@ -39,8 +39,9 @@ typedef enum {
     RFOE_ERR_NOT_SYMMETRIC = 5, /* H^p is not bitwise symmetric (the squaring X X^T relies on it) */
     RFOE_ERR_UNSUPPORTED = 6,   /* unknown variant / option, or device is not compute capability 10.x */
     RFOE_ERR_NOT_CONVERGED = 7, /* max_iter steps taken; P holds the last iterate, stats are complete */
-    RFOE_ERR_NO_PEER_ACCESS = 8 /* sharded P2P setup: a peer's buffers cannot be mapped (cudaDeviceCanAccessPeer is false, or
+    RFOE_ERR_NO_PEER_ACCESS = 8, /* sharded P2P setup: a peer's buffers cannot be mapped (cudaDeviceCanAccessPeer is false, or
                                    cudaIpcOpenMemHandle failed: cuda_error has the reason); use rfoe_expand_sharded instead */
+    RFOE_ERR_STATIC_LIMIT = 9   /* rfoe_bounds_static: k > RFOE_STATIC_MAX_K, the size its fixed scratch array was built for */
 } rfoe_status_t;
 
 /* Recursion variants.
@@ -128,6 +129,28 @@ int rfoe_create(rfoe_handle_t* h, int device, int64_t k_max);
  * PAPER.md:56): eps_min = min_i (H_ii - r_i), eps_max = max_i (H_ii + r_i), r_i = sum_{j != i} |H_ij|.
  * Hp: device, k x k, read only.  eps_min / eps_max: HOST doubles, written on success.  Pure query. */
 int rfoe_bounds(rfoe_handle_t h, const double* Hp, int64_t k, double* eps_min, double* eps_max, rfoe_stream_t stream);
+
+/* The same Gershgorin bounds (row A1; reading R3) for callers that cannot allocate: code under CUDA graph
+ * capture, serving loops and harnesses that forbid cudaMalloc.  No handle, no allocation: this call and everything
+ * under it calls no cudaMalloc / cudaFree / allocating library routine.  The per-row disc ends (2 k doubles), which
+ * rfoe_bounds keeps in handle memory, live in ONE file-scope `static __device__` array of 2 * RFOE_STATIC_MAX_K
+ * doubles (512 KiB) that every GPU which loads the library holds until the process exits.
+ *   Hp      device, k x k, read only, on the CURRENT device (cudaGetDevice); k <= RFOE_STATIC_MAX_K, else
+ *           RFOE_ERR_STATIC_LIMIT and nothing is launched.
+ *   bounds  DEVICE, 2 doubles, caller-owned: bounds[0] = eps_min, bounds[1] = eps_max (as rfoe_bounds: both NaN when H^p
+ *           holds a NaN, -inf / +inf when it holds an infinity -- never finite for a non-finite H^p).
+ *   cuda_error  host, may be null: the cudaError_t behind an RFOE_ERR_CUDA return.
+ * Unlike the handle calls this one is ASYNCHRONOUS: it enqueues two kernels on `stream` and returns; `bounds` is valid
+ * once the stream has passed them.  The first call on each device resolves the array's device address
+ * (cudaGetSymbolAddress, which may load the module): make that call outside stream capture.
+ * Every call on a device shares the one array, which keeps the last call's contents.  Nothing in it must start at
+ * zero: a call writes entries [0, k) of both halves before it reads exactly those.  Calls that OVERLAP on the same GPU
+ * (two streams, or two host threads) race on the array and give wrong bounds: serialise them (one stream, or events).
+ * Results are bit for bit those of rfoe_bounds.
+ * Errors: INVALID_ARG (null pointer, k < 1), STATIC_LIMIT, UNSUPPORTED (current device is not compute capability
+ * 10.x), CUDA. */
+#define RFOE_STATIC_MAX_K 32768
+int rfoe_bounds_static(const double* Hp, int64_t k, double* bounds, rfoe_stream_t stream, int* cuda_error);
 
 /* Tighter "spectral bound estimates" than Gershgorin's: m steps (1..64; 24 is plenty) of the Lanczos
  * recursion from a fixed pseudo-random start vector, T_m = tridiag(alpha, beta), and

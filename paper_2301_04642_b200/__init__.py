@@ -18,7 +18,7 @@ import numpy as np
 from . import build as _build
 
 __all__ = ["Rfoe", "RfoeError", "ExpandResult", "load_library", "shard_range", "torch_distributed_allgather", "gather_ipc_handles", "SP2", "MCWEENY", "SP2_MIXED", "SP2_ACCEL",
-           "TRUNC", "TRUNC_MIXED", "RULE_A", "RULE_B", "EXPORTS"]
+           "TRUNC", "TRUNC_MIXED", "RULE_A", "RULE_B", "EXPORTS", "bounds_static", "STATIC_MAX_K"]
 
 SP2, MCWEENY, SP2_MIXED, SP2_ACCEL, TRUNC, TRUNC_MIXED = 0, 1, 2, 3, 4, 5
 RULE_A, RULE_B = 0, 1
@@ -28,10 +28,11 @@ MAX_STEPS = 256
  OPT_HOMO, OPT_LUMO, OPT_LANCZOS_STEPS, OPT_TRUNC_STEPS, OPT_RESIDENT) = range(12)
 
 (OK, ERR_INVALID_ARG, ERR_ALLOC, ERR_CUDA, ERR_BAD_BOUNDS, ERR_NOT_SYMMETRIC, ERR_UNSUPPORTED, ERR_NOT_CONVERGED,
- ERR_NO_PEER_ACCESS) = range(9)
+ ERR_NO_PEER_ACCESS, ERR_STATIC_LIMIT) = range(10)
+STATIC_MAX_K = 32768      # RFOE_STATIC_MAX_K
 
 # every symbol include/rfoe.h declares
-EXPORTS = ("rfoe_create", "rfoe_bounds", "rfoe_bounds_lanczos", "rfoe_expand", "rfoe_expand_host", "rfoe_square", "rfoe_square_reduced",
+EXPORTS = ("rfoe_create", "rfoe_bounds", "rfoe_bounds_static", "rfoe_bounds_lanczos", "rfoe_expand", "rfoe_expand_host", "rfoe_square", "rfoe_square_reduced",
            "rfoe_symm_product", "rfoe_probe_fp64_peak", "rfoe_project", "rfoe_apply", "rfoe_expand_sharded", "rfoe_shard_range", "rfoe_plan_squaring", "rfoe_plan_resident",
            "rfoe_shard_local_ptrs", "rfoe_shard_set_peers", "rfoe_shard_ipc_export", "rfoe_shard_ipc_import",
            "rfoe_expand_sharded_p2p", "rfoe_expand_many",
@@ -86,6 +87,7 @@ def load_library(path: str | None = None):
     vp, i64, dbl, dp = C.c_void_p, C.c_int64, C.c_double, C.POINTER(C.c_double)
     L.rfoe_create.argtypes = [C.POINTER(vp), C.c_int, i64]
     L.rfoe_bounds.argtypes = [vp, vp, i64, dp, dp, vp]
+    L.rfoe_bounds_static.argtypes = [vp, i64, vp, vp, C.POINTER(C.c_int)]
     L.rfoe_bounds_lanczos.argtypes = [vp, vp, i64, C.c_int, dp, dp, vp]
     L.rfoe_expand.argtypes = [vp, vp, i64, i64, C.c_int, dbl, vp, vp]
     L.rfoe_expand_host.argtypes = [vp, vp, i64, i64, C.c_int, dbl, vp, vp]
@@ -228,6 +230,25 @@ def estimate_homo_lumo(stats: _Stats):
     if rc != OK:
         raise RfoeError(rc, "rfoe_estimate_homo_lumo: " + L.rfoe_strerror(rc).decode())
     return ho.value, lu.value
+
+
+def bounds_static(Hp, out, stream=None):
+    """rfoe_bounds_static: Gershgorin bounds with no handle and no allocation anywhere below this call (scratch in a fixed
+    device array, k <= STATIC_MAX_K).  `out`: float64 CUDA tensor of >= 2 elements on Hp's device, receives
+    (eps_min, eps_max).  Asynchronous on `stream`; calls that overlap on one GPU race on the shared scratch."""
+    import torch
+
+    _check_dev(Hp, "Hp")
+    if not (isinstance(out, torch.Tensor) and out.is_cuda and out.dtype == torch.float64 and out.is_contiguous()
+            and out.numel() >= 2 and out.device == Hp.device):
+        raise ValueError("out: contiguous float64 CUDA tensor of >= 2 elements on Hp's device expected")
+    L = load_library()
+    err = C.c_int(0)
+    with torch.cuda.device(Hp.device):
+        rc = L.rfoe_bounds_static(C.c_void_p(Hp.data_ptr()), Hp.shape[0], C.c_void_p(out.data_ptr()), _stream_ptr(stream), C.byref(err))
+    if rc != OK:
+        raise RfoeError(rc, "rfoe_bounds_static: " + L.rfoe_strerror(rc).decode(), err.value)
+    return out
 
 
 def plan_squaring(k: int, sm_count: int = 148):

@@ -8,6 +8,7 @@
 #include <string.h>
 
 #include <atomic>
+#include <mutex>
 #include <new>
 #include <thread>
 #include <vector>
@@ -316,11 +317,12 @@ extern "C" const char* rfoe_strerror(int status)
         case RFOE_ERR_UNSUPPORTED: return "unsupported variant, option or device";
         case RFOE_ERR_NOT_CONVERGED: return "maximum number of recursion steps reached";
         case RFOE_ERR_NO_PEER_ACCESS: return "a peer GPU's buffers cannot be mapped (no P2P access)";
+        case RFOE_ERR_STATIC_LIMIT: return "k exceeds RFOE_STATIC_MAX_K, the size of the allocation-free entry point's fixed scratch array";
         default: return "unknown status";
     }
 }
 
-extern "C" int rfoe_version(void) { return 200; }
+extern "C" int rfoe_version(void) { return 201; }
 
 extern "C" int rfoe_destroy(rfoe_handle_t h)
 {
@@ -566,6 +568,65 @@ extern "C" int rfoe_bounds(rfoe_handle_t h, const double* Hp, int64_t k, double*
     *eps_max = h->hp->bounds[1];
     h->stats.gpu_launches = h->launches;
     h->stats.status = RFOE_OK;
+    return RFOE_OK;
+}
+
+// ---- rfoe_bounds_static: row A1 without a handle and without any allocation (include/rfoe.h) ----------------------
+// The per-row disc ends go to a file-scope device array instead of handle memory.  In host code the array's NAME is a
+// host-side stand-in, not a device address: the kernels get the address cudaGetSymbolAddress returns, resolved once per
+// device with that device current.
+static __device__ __align__(256) double g_static_rows[2 * RFOE_STATIC_MAX_K];
+
+namespace {
+constexpr int STATIC_MAX_DEVICES = 64;
+struct StaticDev {
+    double* rows = nullptr;   // device address of g_static_rows on this device
+    int sm_count = 0;
+    int cc_major = 0;
+};
+StaticDev g_static_dev[STATIC_MAX_DEVICES];
+std::mutex g_static_mu;
+}  // namespace
+
+extern "C" int rfoe_bounds_static(const double* Hp, int64_t k, double* bounds, rfoe_stream_t stream, int* cuda_error)
+{
+    if (cuda_error) *cuda_error = 0;
+    auto fail = [&](cudaError_t e) {
+        if (cuda_error) *cuda_error = (int)e;
+        cudaGetLastError();
+        return (int)RFOE_ERR_CUDA;
+    };
+    if (!Hp || !bounds || k < 1) return RFOE_ERR_INVALID_ARG;
+    if (k > RFOE_STATIC_MAX_K) return RFOE_ERR_STATIC_LIMIT;
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return fail(e);
+    if (dev < 0 || dev >= STATIC_MAX_DEVICES) return RFOE_ERR_UNSUPPORTED;
+    StaticDev sd;
+    {
+        std::lock_guard<std::mutex> lock(g_static_mu);
+        StaticDev& slot = g_static_dev[dev];
+        if (!slot.rows) {                                   // set-up, once per device, that device current
+            int sms = 0, major = 0;
+            if ((e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev)) != cudaSuccess) return fail(e);
+            if (major != 10) return RFOE_ERR_UNSUPPORTED;
+            if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return fail(e);
+            double* ptr = nullptr;
+            if ((e = cudaGetSymbolAddress((void**)&ptr, g_static_rows)) != cudaSuccess || !ptr) return fail(e != cudaSuccess ? e : cudaErrorInvalidSymbol);
+            slot.sm_count = sms;
+            slot.cc_major = major;
+            slot.rows = ptr;
+        }
+        sd = slot;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    double* row_lo = sd.rows;
+    double* row_hi = sd.rows + RFOE_STATIC_MAX_K;
+    const int want = ((int)k + HBM_WARPS - 1) / HBM_WARPS, cap = sd.sm_count * 8;       // hbm_grid() without a handle
+    gershgorin_rows_kernel<<<want < cap ? want : cap, HBM_THREADS, 0, st>>>(Hp, (int)k, row_lo, row_hi);
+    if ((e = cudaGetLastError()) != cudaSuccess) return fail(e);
+    bounds_reduce_kernel<<<1, 256, 0, st>>>(row_lo, row_hi, (int)k, bounds);
+    if ((e = cudaGetLastError()) != cudaSuccess) return fail(e);
     return RFOE_OK;
 }
 

@@ -23,7 +23,7 @@ def test_header_symbols_are_exported():
     assert set(declared) == set(rfoe.EXPORTS)
     for name in declared:
         assert hasattr(L, name), name
-    assert L.rfoe_version() == 200
+    assert L.rfoe_version() == 201
     assert L.rfoe_strerror(0) == b"ok" and b"symmetric" in L.rfoe_strerror(5)
 
 
@@ -46,7 +46,7 @@ def test_header_is_plain_c_and_struct_size_matches_the_binding(tmp_path):
     out = subprocess.run([exe, "sizeof"], check=True, capture_output=True, text=True).stdout
     kv = dict(p.split("=") for p in out.split())
     assert int(kv["sizeof_stats"]) == ctypes.sizeof(rfoe._Stats)
-    assert int(kv["version"]) == 200 and int(kv["max_steps"]) == rfoe.MAX_STEPS
+    assert int(kv["version"]) == 201 and int(kv["max_steps"]) == rfoe.MAX_STEPS
 
 
 def test_argument_errors_without_gpu():
