@@ -43,7 +43,7 @@ FP64_PEAK_TFLOPS = FP64_PEAK_DERIVED_TFLOPS
 
 # dram__bytes_read.sum + dram__bytes_write.sum of one sym_square_kernel launch, from the `ncu --set full` captures
 # summarised in profiles/ (ncu cannot run inside a timed bench: the figure is quoted, with its source, not re-measured).
-NCU_TRAFFIC_BYTES = {16384: (24.327044e9 + 2.129401e9, "profiles/r02_sym_square_k16384.md")}
+NCU_TRAFFIC_BYTES = {16384: (24.629606e9 + 2.129160e9, "profiles/r02c_sym_square_k16384.md")}
 
 
 def fp64_peaks(h, torch, stream, n_gemm=8192):

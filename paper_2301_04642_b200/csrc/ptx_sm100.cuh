@@ -85,6 +85,21 @@ __device__ __forceinline__ double lds_f64(uint32_t addr)
     return v;
 }
 
+// 16-byte asynchronous copies global -> shared through L2 only (the source may have been written by another SM this launch)
+__device__ __forceinline__ void cp_async_cg16(uint32_t dst, const void* src)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
+__device__ __forceinline__ double2 lds_f64x2(uint32_t addr)
+{
+    double2 v;
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
+    return v;
+}
+
 __device__ __forceinline__ float lds_f32(uint32_t addr)
 {
     float v;

@@ -17,6 +17,9 @@
 // and lane 0 of warp 0 doubles as the TMA producer: it refills a stage as soon as a non-blocking
 // mbarrier test shows all eight warps have released it (2 warps per SMSP keep the 255-register budget).
 // Fragment row m of a 16-row group maps to tile row 2m + p (p = 0, 1): with the 128B swizzle this makes every 64-bit fragment load bank-conflict free.
+// The epilogue's own operand, the 128 x 128 tile of X_n, rides the same ring: four more entries of two boxes each are requested
+// while the last chunks are multiplied and land in the stages those chunks free, so the update reads X_n from shared memory
+// instead of waiting for eight dependent trips to DRAM (k=16384: 122.06 -> 121.69 ms per squaring, same bits).
 #pragma once
 #include "ptx_sm100.cuh"
 
@@ -67,6 +70,12 @@ sym_square_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
 {
     constexpr bool TWO_OP = (MODE == 1 || MODE == 2);
     constexpr bool P2P = (MODE == 3);
+    // E_SMEM (squarings: E = X_n is the matrix tmA describes): the epilogue's 128 x 128 tile of X_n arrives by TMA as four
+    // more ring entries ("chunks" KT .. KT+3: boxes 2v, 2v+1 of the tile in entry v) into the stages the last chunks free,
+    // so it is in shared memory when the main loop ends (r02b profile: half of the epilogue was spent waiting for these
+    // 128 KiB, one dependent DRAM round trip per 16 x 32 block, with the tensor pipe idle)
+    constexpr bool E_SMEM = (MODE == 0 || MODE == 3);
+    constexpr int E_CHUNKS = E_SMEM ? (SQ_BM * SQ_BM * 8) / (2 * SQ_PANEL_BYTES) : 0;      // 4
     // MODE 3 has no single output matrix: `Out` carries a pointer to the PeerSet in device memory instead (the
     // parameter list is kept as it is because any change to it perturbs ptxas' schedule of the MODE 0 main loop)
     const PeerSet& peers = *reinterpret_cast<const PeerSet*>(Out);
@@ -112,7 +121,14 @@ sym_square_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
             if (ld_kt >= SQ_STAGES && !mbar_test(empty0 + 8 * ld_s, ld_ph ^ 1u)) break;
             const uint32_t fb = full0 + 8 * ld_s;
             const uint32_t dstA = smem_base + ld_s * (2 * SQ_PANEL_BYTES);
-            if (elect_one()) {
+            if (E_SMEM && ld_kt >= KT) {
+                // entry v = ld_kt - KT of the X_n tile: columns J*128 + 32 v .. + 31 of rows I*128 .. + 127, as two boxes
+                if (elect_one()) {
+                    mbar_expect_tx(fb, 2 * SQ_PANEL_BYTES);
+                    tma_load_2d(dstA, &tmA, J * SQ_BM + (ld_kt - KT) * 2 * SQ_BK, I * SQ_BM, fb);
+                    tma_load_2d(dstA + SQ_PANEL_BYTES, &tmA, J * SQ_BM + (ld_kt - KT) * 2 * SQ_BK + SQ_BK, I * SQ_BM, fb);
+                }
+            } else if (elect_one()) {
                 mbar_expect_tx(fb, stage_bytes);
                 tma_load_2d(dstA, &tmA, (kt0 + ld_kt) * SQ_BK, I * SQ_BM, fb);
                 if (two_panels) tma_load_2d(dstA + SQ_PANEL_BYTES, TWO_OP ? &tmB : &tmA, (kt0 + ld_kt) * SQ_BK, J * SQ_BM, fb);
@@ -170,11 +186,11 @@ sym_square_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
         load_frag(a0, b0, st + rowA, st + rowB, off[0]);
         for (int kt = 0; kt < KT; ++kt) {
             if (warp == 0) {
-                issue_loads(min(KT, kt + SQ_STAGES));
+                issue_loads(min(KT + E_CHUNKS, kt + SQ_STAGES));
                 // Warp 0 is the only producer AND a consumer, and it blocks on chunk kt+1 further down: that chunk must have been
                 // issued by then, or nobody ever would.  It normally was, five iterations ago; if another warp still holds its stage
                 // (a 5-chunk skew, which the 6-stage ring permits), wait HERE, where waiting cannot deadlock (that warp has its data).
-                while (ld_kt < min(KT, kt + 2)) issue_loads(min(KT, kt + SQ_STAGES));
+                while (ld_kt < min(KT, kt + 2)) issue_loads(min(KT + E_CHUNKS, kt + SQ_STAGES));
             }
             const uint32_t aB = st + rowA, bB = st + rowB;
             int s1 = s + 1;
@@ -212,6 +228,19 @@ sym_square_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
             return;
         }
         // ===== fused epilogue =====
+        // E_SMEM: this warp's 64 x 32 block of X_n lies in ring entry KT + warp_n (box h = columns 16 h .. 16 h + 15 of the
+        // block; rows 128 bytes, 16-byte chunks swizzled by the row as everywhere).  Warp 0 first makes sure all four entries
+        // are on their way: their stages free up as the other warps leave the main loop, which needs nothing from warp 0 any more.
+        uint32_t e_base = 0;
+        if (E_SMEM) {
+            if (warp == 0)
+                while (ld_kt < KT + E_CHUNKS) issue_loads(KT + E_CHUNKS);
+            int se = s + warp_n;
+            uint32_t phe = ph;
+            if (se >= SQ_STAGES) { se -= SQ_STAGES; phe ^= 1u; }
+            mbar_wait(full0 + 8 * se, phe);
+            e_base = smem_base + (uint32_t)se * (2 * SQ_PANEL_BYTES) + (uint32_t)(warp_m * 64 + 2 * r) * 128u;
+        }
         const double c2 = coef->c2, c1 = coef->c1, c0 = coef->c0;
         double p_tr = 0.0, p_ss = 0.0, p_err = 0.0, p_trc = 0.0, p_ce = 0.0;
         const int row_base = I * SQ_BM + warp_m * 64 + 2 * r;       // + 16 g + p
@@ -227,8 +256,17 @@ sym_square_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
                     const int row = row_base + 16 * g + p;
                     const int mi = 2 * g + p;
                     const double cv[4] = {acc[mi][2 * h][0], acc[mi][2 * h + 1][0], acc[mi][2 * h][1], acc[mi][2 * h + 1][1]};
-                    const double2 e01 = *reinterpret_cast<const double2*>(E + (size_t)row * ld + col);
-                    const double2 e23 = *reinterpret_cast<const double2*>(E + (size_t)row * ld + col + 2);
+                    double2 e01, e23;
+                    if (E_SMEM) {
+                        // tile row 2r + 16g + p (+ 64 warp_m), box h, columns 4 kk .. 4 kk + 3 = 16-byte chunks 2 kk, 2 kk + 1
+                        const uint32_t a = e_base + (uint32_t)(h * SQ_PANEL_BYTES + (16 * g + p) * 128);
+                        const uint32_t sw = (uint32_t)((2 * r + p) & 7);
+                        e01 = lds_f64x2(a + ((((uint32_t)(2 * kk)) ^ sw) << 4));
+                        e23 = lds_f64x2(a + ((((uint32_t)(2 * kk + 1)) ^ sw) << 4));
+                    } else {
+                        e01 = *reinterpret_cast<const double2*>(E + (size_t)row * ld + col);
+                        e23 = *reinterpret_cast<const double2*>(E + (size_t)row * ld + col + 2);
+                    }
                     const double ev[4] = {e01.x, e01.y, e23.x, e23.y};
 #pragma unroll
                     for (int u = 0; u < 4; ++u) {

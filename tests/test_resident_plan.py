@@ -51,6 +51,9 @@ def test_stream_k_ranges_partition_the_step(k, sm):
             holders[t].append(b)
     split = {t: (b0, n) for t, b0, n in d["split_tiles"]}
     assert d["n_split"] == len(split)
+    # a boundary between two CTAs cuts at most one tile: fewer split tiles than CTAs, hence at most ONE 16-row fix-up band per
+    # warp (8 bands per split tile, 8 warps per CTA) -- resident.cuh's FIX phase relies on it
+    assert d["n_split"] < G
     for t in range(nt):
         hs = holders[t]
         assert hs == list(range(hs[0], hs[0] + len(hs)))                 # consecutive CTAs
