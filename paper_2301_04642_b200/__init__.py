@@ -25,7 +25,7 @@ RULE_A, RULE_B = 0, 1
 MAX_STEPS = 256
 
 (OPT_STOP_RULE, OPT_MAX_ITER, OPT_EPS_MIN, OPT_EPS_MAX, OPT_CHECK_SYMMETRY, OPT_MIXED_HEAD, OPT_MIXED_RELTR,
- OPT_HOMO, OPT_LUMO, OPT_LANCZOS_STEPS, OPT_TRUNC_STEPS, OPT_RESIDENT) = range(12)
+ OPT_HOMO, OPT_LUMO, OPT_LANCZOS_STEPS, OPT_TRUNC_STEPS, OPT_RESIDENT, OPT_REDUCED_PAIR) = range(13)
 
 (OK, ERR_INVALID_ARG, ERR_ALLOC, ERR_CUDA, ERR_BAD_BOUNDS, ERR_NOT_SYMMETRIC, ERR_UNSUPPORTED, ERR_NOT_CONVERGED,
  ERR_NO_PEER_ACCESS, ERR_STATIC_LIMIT) = range(10)
@@ -372,10 +372,11 @@ class Rfoe:
             raise RfoeError(rc, self._L.rfoe_strerror(rc).decode())
 
     def configure(self, *, stop_rule=None, max_iter=None, bounds=None, check_symmetry=None, mixed_head=None,
-                  mixed_reltr=None, homo=None, lumo=None, lanczos_steps=None, trunc_steps=None, resident=None):
+                  mixed_reltr=None, homo=None, lumo=None, lanczos_steps=None, trunc_steps=None, resident=None, reduced_pair=None):
         if lanczos_steps is not None: self.set_option(OPT_LANCZOS_STEPS, lanczos_steps)
         if trunc_steps is not None: self.set_option(OPT_TRUNC_STEPS, trunc_steps)
         if resident is not None: self.set_option(OPT_RESIDENT, 1.0 if resident else 0.0)
+        if reduced_pair is not None: self.set_option(OPT_REDUCED_PAIR, 1.0 if reduced_pair else 0.0)
         if stop_rule is not None: self.set_option(OPT_STOP_RULE, stop_rule)
         if max_iter is not None: self.set_option(OPT_MAX_ITER, max_iter)
         if bounds is not None:

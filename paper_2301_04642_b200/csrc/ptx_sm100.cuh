@@ -282,6 +282,66 @@ __device__ __forceinline__ void umma_commit_mc(uint32_t bar, uint16_t mask)
                  : "memory");
 }
 
+// ---- CTA pairs (cta_group::2): one tcgen05.mma of the leader CTA (cluster rank 0) drives the tensor cores of both SMs of a
+// TPC -- D is 256 x N, each CTA holds 128 rows of A and of D and HALF of B's N rows in its own shared memory, at the same
+// offsets in both CTAs -- so each SM reads half the B bytes per flop.  Allocation / deallocation are collective over the pair
+// (the same warp index in both CTAs); TMA loads of either CTA can complete on the LEADER's mbarrier; commits are multicast.
+template <int COLS>
+__device__ __forceinline__ void tmem_alloc_pair(uint32_t dst_smem)
+{
+    asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(dst_smem), "n"(COLS) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+}
+
+template <int COLS>
+__device__ __forceinline__ void tmem_dealloc_pair(uint32_t taddr)
+{
+    asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(taddr), "n"(COLS) : "memory");
+}
+
+// the shared::cluster address of the same shared-memory location in CTA `rank` of the cluster
+__device__ __forceinline__ uint32_t map_to_cta(uint32_t smem_addr, uint32_t rank)
+{
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(smem_addr), "r"(rank));
+    return r;
+}
+
+// arrive on an mbarrier anywhere in the cluster (address from map_to_cta)
+__device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_bar)
+{
+    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_bar) : "memory");
+}
+
+// TMA load into THIS CTA's shared memory whose bytes complete on an mbarrier given by its shared::cluster address (the leader's)
+__device__ __forceinline__ void tma_load_2d_pair(uint32_t dst, const CUtensorMap* map, int c0, int c1, uint32_t cluster_bar)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(dst),
+        "l"(reinterpret_cast<uint64_t>(map)), "r"(c0), "r"(c1), "r"(cluster_bar)
+        : "memory");
+}
+
+__device__ __forceinline__ void umma_f16_pair(uint32_t tmem_d, uint64_t desc_a, uint64_t desc_b, uint32_t idesc, uint32_t accumulate)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "setp.ne.b32 p, %4, 0;\n"
+        "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n"
+        "}\n" ::"r"(tmem_d),
+        "l"(desc_a), "l"(desc_b), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+
+// all previously issued pair MMAs of this thread arrive, when complete, on the mbarrier at this offset in every CTA of `mask`
+__device__ __forceinline__ void umma_commit_pair_mc(uint32_t bar, uint16_t mask)
+{
+    asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(bar),
+                 "h"(mask)
+                 : "memory");
+}
+
 // one lane of a CONVERGED warp (the warp stays converged, so the elected lane's tcgen05 / TMA instructions
 // take their operands from uniform registers; an `if (lane == 0)` region makes ptxas emit an
 // ELECT + R2UR.BROADCAST loop of ~14 instructions in front of every UTCHMMA / UTMALDG instead)

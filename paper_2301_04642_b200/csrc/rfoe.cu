@@ -24,6 +24,7 @@
 #include "subspace.cuh"
 #include "sym_square.cuh"
 #include "sym_square_reduced.cuh"
+#include "sym_square_reduced_pair.cuh"
 #include "tail.cuh"
 
 using namespace rfoe;
@@ -94,7 +95,7 @@ struct rfoe_handle_s {
     int sq_n = 0;
     EncodeTiledFn encode = nullptr;
     // options
-    int stop_rule = 0, max_iter = 100, check_sym = 1, trunc_steps = 30, resident = 1;
+    int stop_rule = 0, max_iter = 100, check_sym = 1, trunc_steps = 30, resident = 1, reduced_pair = 1;
     double eps_min = NAN, eps_max = NAN, mixed_head = 0.0, mixed_reltr = 5e-4, homo = NAN, lumo = NAN;
     rfoe_stats_t stats;
     int64_t launches = 0;
@@ -199,7 +200,7 @@ static cudaError_t launch_square_reduced(rfoe_handle_s* h, const CUtensorMap& hi
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(2 * h->n_pairs);
     cfg.blockDim = dim3(TQ_THREADS);
-    cfg.dynamicSmemBytes = TQ_SMEM_BYTES;
+    cfg.dynamicSmemBytes = h->reduced_pair ? TP_SMEM_BYTES : TQ_SMEM_BYTES;
     cfg.stream = st;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeClusterDimension;
@@ -209,6 +210,10 @@ static cudaError_t launch_square_reduced(rfoe_handle_s* h, const CUtensorMap& hi
     cfg.attrs = attr;
     cfg.numAttrs = 1;
     h->launches++;
+    // CTA-pair form (tcgen05.mma.cta_group::2, sym_square_reduced_pair.cuh) unless RFOE_OPT_REDUCED_PAIR = 0
+    if (h->reduced_pair)
+        return cudaLaunchKernelEx(&cfg, sym_square_reduced_pair_kernel, hi, lo, Xin, Out, n, ld, k, trace, coef, (const int2*)h->d_pairs,
+                                  n / TQ_BM, partials);
     return cudaLaunchKernelEx(&cfg, sym_square_reduced_kernel, hi, lo, Xin, Out, n, ld, k, trace, coef, (const int2*)h->d_pairs,
                               n / TQ_BM, partials);
 }
@@ -408,7 +413,8 @@ extern "C" int rfoe_create(rfoe_handle_t* out, int device, int64_t k_max)
         cudaFuncSetAttribute(resident_small_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, RT_SMEM_BYTES) != cudaSuccess ||
         cudaFuncSetAttribute(resident_small_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, RT_SMEM_BYTES) != cudaSuccess ||
         cudaFuncSetAttribute(apply_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, AP_SMEM_BYTES) != cudaSuccess ||
-        cudaFuncSetAttribute(sym_square_reduced_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TQ_SMEM_BYTES) != cudaSuccess) {
+        cudaFuncSetAttribute(sym_square_reduced_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TQ_SMEM_BYTES) != cudaSuccess ||
+        cudaFuncSetAttribute(sym_square_reduced_pair_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TP_SMEM_BYTES) != cudaSuccess) {
         rfoe_destroy(h);
         return RFOE_ERR_CUDA;
     }
@@ -454,6 +460,9 @@ extern "C" int rfoe_set_option(rfoe_handle_t h, int key, double value)
         case RFOE_OPT_RESIDENT:
             if (value != 0.0 && value != 1.0) return RFOE_ERR_INVALID_ARG;
             h->resident = (int)value; return RFOE_OK;
+        case RFOE_OPT_REDUCED_PAIR:
+            if (value != 0.0 && value != 1.0) return RFOE_ERR_INVALID_ARG;
+            h->reduced_pair = (int)value; return RFOE_OK;
         case RFOE_OPT_HOMO: h->homo = value; return RFOE_OK;
         case RFOE_OPT_LUMO: h->lumo = value; return RFOE_OK;
         default: return RFOE_ERR_UNSUPPORTED;

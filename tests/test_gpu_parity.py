@@ -371,14 +371,20 @@ def test_error_paths(handle):
 
 
 # ------------------------------------------------------------------ A8: reduced-precision path (reported separately)
-@pytest.mark.parametrize("k", [1, 5, 128, 130, 257, 777])
-def test_square_reduced_error_bound(handle, k):
+@pytest.mark.parametrize("pair", [True, False])
+@pytest.mark.parametrize("k", [1, 5, 128, 130, 257, 777, 1100])
+def test_square_reduced_error_bound(handle, k, pair):
     """Three-part (scaled FP16 hi / lo) product with FP32 tensor-core accumulation against the FP64 oracle product.  Bound:
     dropped Zl Zl term and 11-bit rounding of Zl: 3 * 2^-22 per product; FP32 accumulation in tensor memory, one
     truncation per 8-wide MMA block plus the in-block tree, over chunks of 256: (k/8 + 8) * 2^-23 bounds it,
-    all relative to sum_l |z_il||z_lj| with Z = X - (Tr X / k) I."""
+    all relative to sum_l |z_il||z_lj| with Z = X - (Tr X / k) I.  Both forms of the kernel: CTA pairs (tcgen05.mma.cta_group::2,
+    the default) and one CTA per tile (RFOE_OPT_REDUCED_PAIR = 0); sizes with an odd number of tiles per row end in a phantom tile."""
     X = _sym(k, 100 + k, scale=1.0 / math.sqrt(k))
-    out, sc, ms = handle.square(_dev(X), -1.0, 2.0, 0.0, reduced=True)
+    handle.configure(reduced_pair=pair)
+    try:
+        out, sc, ms = handle.square(_dev(X), -1.0, 2.0, 0.0, reduced=True)
+    finally:
+        handle.configure(reduced_pair=True)
     out = out.cpu().numpy()
     Y = oracle.square(X)
     Z = X - np.trace(X) / k * np.eye(k)
@@ -413,6 +419,29 @@ def test_expand_mixed(handle, c, k):
     assert np.array_equal(P, P.T)
     assert abs(np.trace(P) - w.nocc) <= 1e-9
     assert np.linalg.norm(P @ P - P) <= 1e-10 * max(1.0, k / 256)
+
+
+def test_expand_mixed_single_cta_form_agrees(handle):
+    """RFOE_OPT_REDUCED_PAIR = 0 (one CTA per tile, the round-1 kernel) against the default CTA-pair kernel: the same products
+    in the same order per FP32 sum (the two differ in the last bits of those sums: 3e-12 on one squaring), so the whole
+    mixed expansion takes the same decisions, and the two P differ by less than the reduced-precision path's own 1e-6
+    (measured 3e-8: the recursion amplifies last-bit differences of the reduced steps up to their noise floor)."""
+    w = rfoe_inputs.make_workload(3, k=640)
+    handle.configure(mixed_head=0.0, mixed_reltr=5e-4)
+    Hd = _dev(w.H)
+    a = handle.expand(Hd, w.nocc, rfoe.SP2_MIXED, w.tol)
+    handle.configure(reduced_pair=False)
+    try:
+        b = handle.expand(Hd, w.nocc, rfoe.SP2_MIXED, w.tol)
+    finally:
+        handle.configure(reduced_pair=True)
+    assert a.converged and b.converged and a.iterations == b.iterations and a.fp32_steps == b.fp32_steps >= 2
+    assert a.branch == b.branch
+    assert (a.P - b.P).abs().max().item() <= 1e-6
+    assert np.allclose(a.t, b.t, rtol=0, atol=1e-5) and torch.equal(b.P, b.P.T)
+    Pex = _dev(w.exact_projector())
+    for r in (a, b):
+        assert torch.linalg.norm(r.P - Pex).item() / math.sqrt(640) <= 1e-6
 
 
 def test_expand_mixed_paper_schedule(handle):
