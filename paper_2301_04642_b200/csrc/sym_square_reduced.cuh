@@ -35,6 +35,9 @@
 // precision, and the three products run as tcgen05.mma.kind::f16 (K = 16 per instruction, twice the tf32 rate, half
 // the operand bytes through TMA and shared memory).  The scalings 2^-30 / 2^-41 are undone in the FP64 epilogue.
 // RFOE_REDUCED_F16 = 0 keeps the original tf32 parts (kind::tf32, K = 8).
+//
+// This file holds the split pass, the constants and the ONE-CTA-PER-TILE form of the kernel (RFOE_OPT_REDUCED_PAIR = 0); the
+// default form issues the same products as CTA-pair MMAs (tcgen05.mma.cta_group::2): sym_square_reduced_pair.cuh.
 #pragma once
 #include <cuda_fp16.h>
 
