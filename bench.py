@@ -533,6 +533,20 @@ def lanczos_report(h, rfoe, w, H, P, stream, fp64_ms, m=24):
             "trace_error": abs(float(torch.diagonal(P).sum()) - w.nocc)}
 
 
+_scratch = {}
+
+
+def H_scratch(like):
+    """a second matrix of the same shape (rfoe_square needs out != X); kept between calls"""
+    import torch
+
+    key = (tuple(like.shape), like.device)
+    if key not in _scratch:
+        _scratch.clear()
+        _scratch[key] = torch.empty_like(like)
+    return _scratch[key]
+
+
 def reduced_report(h, rfoe, w, H, P, stream, fp64_ms):
     """Row A8, reported separately from the FP64 headline: the same workload through RFOE_VARIANT_SP2_MIXED with
     the paper's schedule (reduced-precision squarings -- three FP16-part products on tcgen05 -- from the first step until
@@ -569,7 +583,23 @@ def reduced_report(h, rfoe, w, H, P, stream, fp64_ms):
             "errP_vs_exact_projector": torch.linalg.norm(P - Pex).item() / math.sqrt(k),
             "rel_band_energy_error": abs(r_late.tr_PH - eband) / abs(eband)}
     h.configure(mixed_reltr=5e-4)
+    # one reduced squaring (split pass + product kernel) of the final P, in both forms of the kernel, interleaved
+    sq = {"pair": [], "single_cta": []}
+    for it in range(6):
+        for name, flag in (("single_cta", False), ("pair", True)):
+            h.configure(reduced_pair=flag)
+            _, _, ms_sq = h.square(P, -1.0, 2.0, 0.0, out=H_scratch(P), stream=stream, reduced=True)
+            if it:
+                sq[name].append(ms_sq)
+    h.configure(reduced_pair=True)
+    flops3 = 3.0 * executed_flops_per_squaring(k)
+    squaring = {name: {"ms": sorted(v)[len(v) // 2], "tflops_executed_f16": flops3 / (sorted(v)[len(v) // 2] * 1e-3) / 1e12} for name, v in sq.items()}
+    _scratch.clear()
+    squaring["note"] = ("rfoe_square_reduced on the converged P, CUDA events around split pass + product kernel, median of 5; pair = "
+                        "tcgen05.mma.cta_group::2 (default), single_cta = RFOE_OPT_REDUCED_PAIR 0; a kernel timed alone, not the "
+                        "power-capped sustained rate of the expansion above")
     return {"variant": "SP2_MIXED, paper schedule (reduced precision until RelTr <= 5e-4)", "dtype": "3xFP16 parts (tcgen05 kind::f16, FP32 accumulate, FP64 epilogue) + f64",
+            "reduced_squaring": squaring,
             "seconds_per_expansion": ms / 1e3, "speedup_vs_fp64": fp64_ms / ms, "iterations": r.iterations,
             "reduced_steps": r.fp32_steps, "converged": bool(r.converged),
             "errP_vs_exact_projector": err, "rel_band_energy_error": abs(r.tr_PH - eband) / abs(eband),
