@@ -80,7 +80,9 @@ enum {
     RFOE_OPT_LANCZOS_STEPS = 9, /* 0 (default): Gershgorin bounds in rfoe_expand; m in 1..64: rfoe_bounds_lanczos with m steps */
     RFOE_OPT_TRUNC_STEPS = 10, /* TRUNC / TRUNC_MIXED: the number m of recursion steps, 1..RFOE_MAX_STEPS (default 30) */
     RFOE_OPT_RESIDENT = 11,    /* 1 (default): expansions small enough to stay on chip (see rfoe_expand) run the WHOLE recursion
-                                  in one persistent launch, no host round trip per step; 0: one launch sequence per step */
+                                  in one persistent launch, no host round trip per step; 0: one launch sequence per step;
+                                  2: as 1, but tiles cut between SMs are always finished in bands after a grid barrier (the
+                                  form 1 picks outside k = 1792 ... 2816), never by their first holder (tests, A/B) */
     RFOE_OPT_REDUCED_PAIR = 12 /* 1 (default): reduced-precision products as CTA-pair MMAs (tcgen05.mma.cta_group::2, the shared
                                   row panel split between the two SMs of a TPC); 0: one CTA per tile with TMA multicast.
                                   The same products in the same order; results agree to the last bits of the FP32 sums */

@@ -375,7 +375,7 @@ class Rfoe:
                   mixed_reltr=None, homo=None, lumo=None, lanczos_steps=None, trunc_steps=None, resident=None, reduced_pair=None):
         if lanczos_steps is not None: self.set_option(OPT_LANCZOS_STEPS, lanczos_steps)
         if trunc_steps is not None: self.set_option(OPT_TRUNC_STEPS, trunc_steps)
-        if resident is not None: self.set_option(OPT_RESIDENT, 1.0 if resident else 0.0)
+        if resident is not None: self.set_option(OPT_RESIDENT, float(int(resident)))      # True / False, or 2: band form only (rfoe.h)
         if reduced_pair is not None: self.set_option(OPT_REDUCED_PAIR, 1.0 if reduced_pair else 0.0)
         if stop_rule is not None: self.set_option(OPT_STOP_RULE, stop_rule)
         if max_iter is not None: self.set_option(OPT_MAX_ITER, max_iter)

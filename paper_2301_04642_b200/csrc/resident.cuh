@@ -38,6 +38,9 @@ constexpr int RS_TILE_ELEMS = SQ_BM * SQ_BM;
 constexpr int RS_MAX_SPLIT = 1024;
 constexpr int RS_SMEM_BYTES = SQ_SMEM_BYTES;
 constexpr int RS_EPI_COST = 10;                      // a register epilogue in chunk units (~39k cycles / 4096 per chunk)
+constexpr int RS_FLAG_WORDS = 256 + 256 * SQ_CONSUMER_WARPS;   // grid-barrier flags + donation flags (resident_fin.cuh)
+constexpr int RS_FIN_MIN_RANGE_TENTHS = 7;           // finisher form (resident_fin.cuh) when a CTA's range of the unit stream is between
+constexpr int RS_FIN_MAX_RANGE_TENTHS = 20;          //   0.7 and 2.0 tiles long (k = 1792 ... 2816 on 148 SMs): measured window, DESIGN.md section 13
 constexpr int RS_TW_PITCH = 129;                     // row pitch (doubles) of a warp's 16 x 128 transposition patch
 
 struct ResidentPlan {
@@ -52,6 +55,7 @@ struct ResidentPlan {
     double* rec0;                 // records of even / odd steps: n_tiles tile records (split tiles' stay zero) + one per CTA (its FIX bands)
     double* rec1;
     unsigned* flags;              // G grid-barrier flags, zero at launch
+    unsigned* dflags;             // resident_fin.cuh: G x 8 donation flags (one per CTA and warp), zero at launch
     Ctrl* ctrl;
     unsigned long long* timing;   // CTA 0's %globaltimer, ns: [0] all steps (rfoe_stats_t.square_ms), [1] MM, [2] first barrier, [3] FIX,
                                   // [4] second barrier, [5] CTL

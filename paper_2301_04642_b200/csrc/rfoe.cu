@@ -19,6 +19,7 @@
 #include "lanczos.cuh"
 #include "probe.cuh"
 #include "resident.cuh"
+#include "resident_fin.cuh"
 #include "resident_small.cuh"
 #include "shard.cuh"
 #include "subspace.cuh"
@@ -70,6 +71,7 @@ struct rfoe_handle_s {
     int4* d_split = nullptr;
     double* d_rec[2] = {nullptr, nullptr};
     unsigned* d_flags = nullptr;
+    int rs_rec_dirty = 0;          // the finisher form has written tile records the band form expects to be zero
     unsigned long long* d_timing = nullptr;
     // sharded expansion over peer memory (rfoe_shard_set_peers / rfoe_shard_ipc_import)
     int p2p_world = 0, p2p_rank = 0;
@@ -390,7 +392,7 @@ extern "C" int rfoe_create(rfoe_handle_t* out, int device, int64_t k_max)
         ok = ok && cudaMalloc(&h->d_split, RS_MAX_SPLIT * sizeof(int4)) == cudaSuccess;
         ok = ok && cudaMalloc(&h->d_rec[0], nrec * SQ_NPART * sizeof(double)) == cudaSuccess;
         ok = ok && cudaMalloc(&h->d_rec[1], nrec * SQ_NPART * sizeof(double)) == cudaSuccess;
-        ok = ok && cudaMalloc(&h->d_flags, 256 * sizeof(unsigned)) == cudaSuccess;
+        ok = ok && cudaMalloc(&h->d_flags, RS_FLAG_WORDS * sizeof(unsigned)) == cudaSuccess;
         ok = ok && cudaMalloc(&h->d_timing, 8 * sizeof(unsigned long long)) == cudaSuccess;
     }
     ok = ok && cudaHostAlloc((void**)&h->hp, sizeof(HostPage), cudaHostAllocMapped) == cudaSuccess;
@@ -410,6 +412,7 @@ extern "C" int rfoe_create(rfoe_handle_t* out, int device, int64_t k_max)
         cudaFuncSetAttribute(sym_square_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, SQ_SMEM_BYTES) != cudaSuccess ||
         cudaFuncSetAttribute(sym_square_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, SQ_SMEM_BYTES) != cudaSuccess ||
         cudaFuncSetAttribute(resident_recursion_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, RS_SMEM_BYTES) != cudaSuccess ||
+        cudaFuncSetAttribute(resident_finisher_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, RS_SMEM_BYTES) != cudaSuccess ||
         cudaFuncSetAttribute(resident_small_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, RT_SMEM_BYTES) != cudaSuccess ||
         cudaFuncSetAttribute(resident_small_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, RT_SMEM_BYTES) != cudaSuccess ||
         cudaFuncSetAttribute(apply_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, AP_SMEM_BYTES) != cudaSuccess ||
@@ -422,6 +425,8 @@ extern "C" int rfoe_create(rfoe_handle_t* out, int device, int64_t k_max)
         int coop = 0, per_sm = 0;
         if (cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, device) == cudaSuccess && coop &&
             cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, resident_recursion_kernel, SQ_THREADS, RS_SMEM_BYTES) == cudaSuccess &&
+            per_sm >= 1 &&
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, resident_finisher_kernel, SQ_THREADS, RS_SMEM_BYTES) == cudaSuccess &&
             per_sm >= 1 && h->sm_count <= 256 && (RT_MAX_N / 64) * (RT_MAX_N / 64 + 1) / 2 <= h->sm_count &&
             cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, resident_small_kernel<32>, SQ_THREADS, RT_SMEM_BYTES) == cudaSuccess && per_sm >= 1 &&
             cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, resident_small_kernel<64>, SQ_THREADS, RT_SMEM_BYTES) == cudaSuccess && per_sm >= 1)
@@ -458,7 +463,7 @@ extern "C" int rfoe_set_option(rfoe_handle_t h, int key, double value)
             if (!(value >= 1.0 && value <= (double)RFOE_MAX_STEPS)) return RFOE_ERR_INVALID_ARG;
             h->trunc_steps = (int)llround(value); return RFOE_OK;
         case RFOE_OPT_RESIDENT:
-            if (value != 0.0 && value != 1.0) return RFOE_ERR_INVALID_ARG;
+            if (value != 0.0 && value != 1.0 && value != 2.0) return RFOE_ERR_INVALID_ARG;
             h->resident = (int)value; return RFOE_OK;
         case RFOE_OPT_REDUCED_PAIR:
             if (value != 0.0 && value != 1.0) return RFOE_ERR_INVALID_ARG;
@@ -947,8 +952,8 @@ static int expand_impl(rfoe_handle_t h, const double* Hp, int64_t k64, int64_t n
         rp.tile_map = h->d_tiles; rp.split = h->d_split;
         rp.W0 = h->W[0]; rp.W1 = h->W[1]; rp.ws = h->ws;
         rp.rec0 = h->d_rec[0]; rp.rec1 = h->d_rec[1];
-        rp.flags = h->d_flags; rp.ctrl = h->d_ctrl; rp.timing = h->d_timing;
-        CK(cudaMemsetAsync(h->d_flags, 0, 256 * sizeof(unsigned), st));
+        rp.flags = h->d_flags; rp.dflags = h->d_flags + 256; rp.ctrl = h->d_ctrl; rp.timing = h->d_timing;
+        CK(cudaMemsetAsync(h->d_flags, 0, RS_FLAG_WORDS * sizeof(unsigned), st));
         CK(cudaMemsetAsync(h->d_timing, 0, 8 * sizeof(unsigned long long), st));
         if (use_small) {
             const int bm = (n <= RT_MAX_N32) ? 32 : 64;
@@ -965,7 +970,36 @@ static int expand_impl(rfoe_handle_t h, const double* Hp, int64_t k64, int64_t n
                                            dim3(sp.n_tiles), dim3(SQ_THREADS), args, RT_SMEM_BYTES, st));
         } else {
             void* args[3] = {(void*)&tm[0], (void*)&tm[1], (void*)&rp};
-            CK(cudaLaunchCooperativeKernel((const void*)resident_recursion_kernel, dim3(h->rs_G), dim3(SQ_THREADS), args, RS_SMEM_BYTES, st));
+            // ranges of about a tile or more: the first holder finishes a cut tile (one grid barrier per step, resident_fin.cuh);
+            // shorter ranges (tiles cut into many parts): all parts to the workspace, finished in bands (two barriers, resident.cuh)
+            const long long units = (long long)h->n_tiles * rp.KT;
+            const long long tile10 = (long long)h->rs_G * rp.KT;          // ten times a range, in tenths of a tile: units * 10 / tile10
+            const bool fin = h->resident == 1 && units * 10 >= tile10 * RS_FIN_MIN_RANGE_TENTHS && units * 10 < tile10 * RS_FIN_MAX_RANGE_TENTHS;
+            if (fin) {
+                // the workspace as a matrix of 128-column tiles, one below the other: donated parts travel through the operand ring
+                CUtensorMap tw;
+                cuuint64_t dims[2] = {(cuuint64_t)SQ_BM, (cuuint64_t)(2 * h->rs_G) * SQ_BM};
+                cuuint64_t strides[1] = {(cuuint64_t)SQ_BM * sizeof(double)};
+                cuuint32_t box[2] = {(cuuint32_t)SQ_BK, (cuuint32_t)SQ_BM};
+                cuuint32_t estr[2] = {1, 1};
+                if (h->encode(&tw, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, h->ws, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                              CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) {
+                    h->stats.cuda_error = (int)cudaErrorInvalidValue;
+                    return fail(RFOE_ERR_CUDA);
+                }
+                void* fargs[4] = {(void*)&tm[0], (void*)&tm[1], (void*)&tw, (void*)&rp};
+                h->rs_rec_dirty = 1;
+                CK(cudaLaunchCooperativeKernel((const void*)resident_finisher_kernel, dim3(h->rs_G), dim3(SQ_THREADS), fargs, RS_SMEM_BYTES, st));
+            } else {
+                // band form: the tile records of cut tiles are never written and must read zero (the finisher form writes them)
+                if (h->rs_rec_dirty) {
+                    const size_t nrec = (size_t)h->n_tiles + (size_t)h->rs_G;
+                    CK(cudaMemsetAsync(h->d_rec[0], 0, nrec * SQ_NPART * sizeof(double), st));
+                    CK(cudaMemsetAsync(h->d_rec[1], 0, nrec * SQ_NPART * sizeof(double), st));
+                    h->rs_rec_dirty = 0;
+                }
+                CK(cudaLaunchCooperativeKernel((const void*)resident_recursion_kernel, dim3(h->rs_G), dim3(SQ_THREADS), args, RS_SMEM_BYTES, st));
+            }
         }
         h->launches++;
         copy_out_select_kernel<<<hbm_grid(h, k), HBM_THREADS, 0, st>>>(h->W[0], h->W[1], &h->d_ctrl->step, k, ld, Hp, P, h->rows[0]);

@@ -20,6 +20,8 @@ import paper_2301_04642_b200 as rfoe  # noqa: E402
 
 
 def _dev(a):
+    if isinstance(a, torch.Tensor):
+        return a.cuda()
     return torch.from_numpy(np.ascontiguousarray(a)).cuda()
 
 
@@ -123,6 +125,39 @@ def test_resident_errors_are_settled_on_the_device():
         assert ei.value.status == rfoe.ERR_INVALID_ARG
         res = h.expand(Hd, w.nocc, rfoe.SP2, w.tol)                   # the handle is fine afterwards
         assert res.converged and res.resident
+
+
+@pytest.mark.parametrize("k", [1800, 2048, 2304, 2600])
+def test_resident_finisher_form_vs_band_form(k):
+    """k = 1792 ... 2816: a tile cut between SMs is finished by its first holder, from registers, with the other holders' parts
+    arriving through the operand ring (csrc/resident_fin.cuh; one grid barrier per step) -- against the band form
+    (RFOE_OPT_RESIDENT = 2: all parts to the workspace, finished in 16-row bands after a barrier), which adds the same parts in
+    the same order: X_{n+1} agrees bit for bit step by step until the trace reaches nocc to rounding; the tile records are
+    summed from differently shaped partial sums, so t_n differs in its last bits and an undecided late step may take the
+    other (equally valid) branch.  Both against the construction-exact projector."""
+    w = rfoe_inputs.make_workload(2, k=k)
+    Hd = _dev(w.H)
+    with rfoe.Rfoe(k) as h:
+        fin = h.expand(Hd, w.nocc, rfoe.SP2, w.tol)
+        again = h.expand(Hd, w.nocc, rfoe.SP2, w.tol)
+        h.configure(resident=2)
+        band = h.expand(Hd, w.nocc, rfoe.SP2, w.tol)
+        h.configure(trunc_steps=6)
+        b6 = h.expand(Hd, w.nocc, rfoe.TRUNC, 0.0)
+        h.configure(resident=1)
+        f6 = h.expand(Hd, w.nocc, rfoe.TRUNC, 0.0)
+    assert fin.resident and band.resident and fin.converged and band.converged and fin.iterations == band.iterations
+    assert torch.equal(f6.P, b6.P)                                     # six steps, all decided: the same bits
+    assert torch.equal(fin.P, again.P) and np.array_equal(fin.t, again.t)     # run to run: bitwise
+    decided = np.abs(band.t[: band.iterations] - w.nocc) > 1e-9 * max(1.0, k / 256)
+    assert all(a == b for a, b, d in zip(fin.branch, band.branch, decided) if d)
+    assert (fin.P - band.P).abs().max().item() <= 1e-12 and torch.equal(fin.P, fin.P.T)
+    assert np.allclose(fin.t, band.t, rtol=1e-13, atol=1e-11) and np.allclose(fin.e[:-3], band.e[:-3], rtol=1e-6, atol=1e-12)
+    Pex = _dev(w.exact_projector())
+    for r in (fin, band):
+        assert torch.linalg.norm(r.P - Pex).item() / math.sqrt(k) <= 1e-10
+    print(f"k={k}: finisher form {fin.device_ms:.3f} ms, band form {band.device_ms:.3f} ms, {fin.iterations} steps, phases (us/step) "
+          f"{[round(x * 1e3 / fin.iterations, 1) for x in fin.resident_phase_ms]}")
 
 
 @pytest.mark.parametrize("k", [3000, 4096])
