@@ -49,6 +49,27 @@ def test_header_is_plain_c_and_struct_size_matches_the_binding(tmp_path):
     assert int(kv["version"]) == 201 and int(kv["max_steps"]) == rfoe.MAX_STEPS
 
 
+def test_bounds_static_argument_errors_without_gpu():
+    """rfoe_bounds_static settles its arguments before it touches CUDA: null pointers, k < 1, and the size limit of its fixed
+    scratch array (RFOE_STATIC_MAX_K, with a message that names it) -- and on a box without a device the first CUDA call fails
+    loudly (RFOE_ERR_CUDA with the cudaError_t handed back), it does not fall back to anything."""
+    L = rfoe.load_library()
+    err = ctypes.c_int(-1)
+    fake = ctypes.c_void_p(4096)          # never dereferenced on these paths
+    assert L.rfoe_bounds_static(None, 16, fake, None, ctypes.byref(err)) == rfoe.ERR_INVALID_ARG and err.value == 0
+    assert L.rfoe_bounds_static(fake, 16, None, None, None) == rfoe.ERR_INVALID_ARG
+    assert L.rfoe_bounds_static(fake, 0, fake, None, None) == rfoe.ERR_INVALID_ARG
+    assert L.rfoe_bounds_static(fake, rfoe.STATIC_MAX_K + 1, fake, None, ctypes.byref(err)) == rfoe.ERR_STATIC_LIMIT and err.value == 0
+    assert b"RFOE_STATIC_MAX_K" in L.rfoe_strerror(rfoe.ERR_STATIC_LIMIT)
+    hdr = open(os.path.join(ROOT, "include", "rfoe.h")).read()
+    assert re.search(r"#define\s+RFOE_STATIC_MAX_K\s+(\d+)", hdr).group(1) == str(rfoe.STATIC_MAX_K)
+    import torch
+
+    if not torch.cuda.is_available():
+        rc = L.rfoe_bounds_static(fake, 16, fake, None, ctypes.byref(err))
+        assert rc in (rfoe.ERR_CUDA, rfoe.ERR_UNSUPPORTED) and (rc != rfoe.ERR_CUDA or err.value != 0)
+
+
 def test_argument_errors_without_gpu():
     L = rfoe.load_library()
     h = ctypes.c_void_p()
