@@ -1,5 +1,5 @@
 // The whole recursion in ONE persistent launch, FINISHER form (resident.cuh's kernel with one grid barrier per step instead of
-// two; used where a CTA's range of the chunk-unit stream is about a tile long or longer, i.e. k >= 2048).
+// two; used where a CTA's range of the chunk-unit stream is 0.7 ... 2.0 tiles long: k = 1792 ... 2816 on 148 SMs).
 //
 // Same stream-K partition (rs_boundary), same ring, same redundant decision.  What differs is who completes a tile that is cut
 // between CTAs.  In resident.cuh every holder stores its raw partial tile, everybody meets at a grid barrier, and the split
@@ -8,9 +8,12 @@
 //   the tail of tile a (a segment that continues somebody else's tile) is the first thing the CTA computes: it is DONATED
 //     at once -- raw accumulators to workspace slot b, one flag per warp -- more than 100 us before anybody needs it;
 //   the head of tile b (a segment that starts a tile) is the last thing it computes: its accumulators stay in registers,
-//     the parts of the following holders are added from the workspace in ascending order of the contraction index (the same
-//     order, hence the same bits, as resident.cuh's bands), and the ordinary fused epilogue runs from registers, with the
-//     tile of X_n it needs fetched through the operand ring behind the last chunks (as in sym_square_kernel).
+//     the parts of the following holders are added in ascending order of the contraction index (the same order, hence the
+//     same bits, as resident.cuh's bands), and the ordinary fused epilogue runs from registers.  Both the donated parts and
+//     the tile of X_n the epilogue needs arrive THROUGH THE OPERAND RING, behind the last chunks: the workspace is described
+//     by a third tensor map (tmW: 128-column tiles one below the other, the operands' box shape), so a part is four more ring
+//     entries and is added with the same swizzled shared-memory reads the epilogue uses for X_n -- 128 accumulator registers
+//     leave no room for global loads in flight (a version with 32 ld.global per thread took twice as long to finish a tile).
 // Only a CTA whose whole range lies inside one tile (k=2048: 12 of 148) donates at the END of its range; its finisher waits
 // for that one flag -- a store, a fence and an L2 round trip after everybody has finished multiplying anyway.
 // No block-level synchronisation in donating or finishing: finisher warp w needs exactly the 64 x 32 block donor warp w wrote.
